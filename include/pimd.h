@@ -1,0 +1,135 @@
+/*
+ * pimd.h -- C ABI of libpimd.so: the per-time-step force evaluation and the thermostatted
+ * velocity-Verlet update of bosonic / xi-particle path integral molecular dynamics as defined
+ * in arXiv 2404.02628 (cited as PAPER.md:<line>, Eq. <n>), hand-written CUDA for sm_100a.
+ *
+ * What is computed (units hbar = m = k_B = 1):
+ *   sampled potential  Phi = V_xi^{[1,N]} + U/P                       (Eq. 4)
+ *   V_xi^{[1,N]}       by the recursion of Eq. 6 over the cycle energies of
+ *                      Eq. 7, spring constant k_s = m omega_P^2 = P/beta^2
+ *   U                  sum_j [ sum_l 1/2 omega^2 |r_l^j|^2 + sum_{i<l} g exp(-|r_l^j-r_i^j|^2/s^2) ]
+ *                      (Eq. 5 :55, Eq. 18 :142, Eq. 19 :158, Eq. 20 :193 with g = g_paper/(pi s^2))
+ *   forces             F = -grad Phi: Eq. 15, 16 (beads 1 and P, through the connection
+ *                      probabilities of Eq. 12-14), Eq. 17 (interior beads, :136)
+ *                      and -(1/P) grad U
+ *   dynamics           velocity Verlet with a thermostat at T = 1/beta (R10)
+ *
+ * Conventions
+ *   - Every function returns PIMD_OK (0) or a negative PIMD_E* code; pimd_last_error() gives text.
+ *     No C++ type or exception crosses this boundary.
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are host pointers.  The caller owns
+ *     every buffer it passes; the library copies in/out and never keeps a caller pointer, except
+ *     the workspace given to pimd_set_workspace(), which the caller must keep alive until
+ *     pimd_destroy() or the next pimd_set_workspace().
+ *   - State layout: x[P][N][d], v[P][N][d], f[P][N][d], C-contiguous doubles, flat index
+ *     ((j*N)+l)*d+c for bead j (0..P-1 <-> the paper's 1..P), particle l (0..N-1), coordinate c.
+ *     Particle order is significant (the recursion threads cycles over consecutive indices).
+ *   - All work is enqueued on the stream given by pimd_set_stream() (default: the legacy default
+ *     stream) and on one internal helper stream that is fork/joined to it with events.  Calls that
+ *     return host scalars synchronise that stream; pimd_step() is asynchronous.
+ *   - One handle is not thread-safe; different handles are independent.
+ *   - There is no CPU fallback: without a CUDA device pimd_create() fails with PIMD_ECUDA.
+ */
+#ifndef PIMD_H
+#define PIMD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIMD_OK 0
+#define PIMD_EINVAL (-1)   /* bad argument (N<1, P<2, d not in {1,2,3}, beta<=0, s<=0, dt<=0, non-finite, ...) */
+#define PIMD_ENOMEM (-2)   /* host or device allocation failed / workspace too small */
+#define PIMD_ECUDA (-3)    /* a CUDA call failed; pimd_last_error() holds the CUDA error string */
+#define PIMD_ENUMERIC (-4) /* non-finite state, or e^{-beta V} summed to exactly zero (a node, xi<0) */
+
+#define PIMD_THERMOSTAT_NVE 0      /* none */
+#define PIMD_THERMOSTAT_LANGEVIN 1 /* OBABO, friction gamma (default 1), Philox4x32-10 noise */
+#define PIMD_THERMOSTAT_NHC 2      /* massive Nose-Hoover chains, length 4, Q = beta/P */
+#define PIMD_NHC_LENGTH 4
+
+typedef struct pimd_s *pimd_t; /* opaque; owns its device workspace unless one is supplied */
+
+/* Create a simulation of N particles x P beads in d dimensions at inverse temperature beta in an
+ * isotropic harmonic trap of frequency omega, pair potential g*exp(-r^2/s^2) between same-index
+ * beads, exchange parameter xi (1 bosons, 0 distinguishable, <0 fictitious particles; Eq. 2,
+ * PAPER.md:39-42), time step dt, thermostat PIMD_THERMOSTAT_*, noise seed.  State starts at zero;
+ * load it with pimd_set_state().  *out is NULL on failure (then pimd_last_error(NULL) has text). */
+int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, double g, double s,
+                double xi, double dt, int thermostat, uint64_t seed);
+int pimd_destroy(pimd_t h);
+
+/* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
+int pimd_set_stream(pimd_t h, void *cuda_stream);
+
+/* Device workspace.  pimd_workspace_bytes() is the size needed; pimd_set_workspace() hands the
+ * library caller-owned device memory (256-byte aligned, e.g. a torch uint8 tensor) to use instead
+ * of its own cudaMalloc.  Must be called before the first compute/state call. */
+size_t pimd_workspace_bytes(pimd_t h);
+int pimd_set_workspace(pimd_t h, void *dev_ptr, size_t bytes);
+
+/* Langevin friction gamma (>0; default 1).  Other thermostat parameters are fixed (R10). */
+int pimd_set_gamma(pimd_t h, double gamma);
+/* 1 (default): the exchange part and the pair part of a force evaluation run concurrently on two
+ * streams; 0: everything on the main stream (profiling / debugging). */
+int pimd_set_concurrency(pimd_t h, int on);
+
+/* Copy state in / out.  x_dev, v_dev: DEVICE pointers, [P][N][d] doubles; v_dev may be NULL
+ * (set: velocities zero; get: skipped).  Setting the state resets the Nose-Hoover variables to zero
+ * and invalidates cached forces.  *_host variants take HOST pointers (pageable or pinned). */
+int pimd_set_state(pimd_t h, const double *x_dev, const double *v_dev);
+int pimd_get_state(pimd_t h, double *x_dev, double *v_dev);
+int pimd_set_state_host(pimd_t h, const double *x_host, const double *v_host);
+int pimd_get_state_host(pimd_t h, double *x_host, double *v_host);
+/* Resume support: MD step counter (the Philox counter of the Langevin noise) and the Nose-Hoover
+ * chain variables nhc[PIMD_NHC_LENGTH][P*N*d] (DEVICE pointer). */
+int pimd_get_step_count(pimd_t h, uint64_t *step_host);
+int pimd_set_step_count(pimd_t h, uint64_t step);
+int pimd_get_nhc(pimd_t h, double *nhc_dev);
+int pimd_set_nhc(pimd_t h, const double *nhc_dev);
+
+/* One force evaluation at the current positions (steps 1-6 of the hot path).
+ *   f_dev  DEVICE [P][N][d] or NULL: F = -grad( V_xi^{[1,N]} + U/P )
+ *   vb     HOST out or NULL: V_xi^{[1,N]} = -(1/beta) ln|W_N|              (Eq. 6)
+ *   sign   HOST out or NULL: sign of W_N = e^{-beta V} (+1 whenever xi >= 0)
+ * Synchronises the stream.  PIMD_ENUMERIC if the state is non-finite or W_N == 0. */
+int pimd_forces(pimd_t h, double *f_dev, double *vb, int *sign);
+int pimd_forces_host(pimd_t h, double *f_host, double *vb, int *sign);
+
+/* Tables of the last force evaluation, HOST out (any may be NULL):
+ *   vfwd[n] = V_xi^{[1,n]}, n = 0..N  (N+1 doubles; Eq. 6)
+ *   vbwd[u] = V_xi^{[u,N]}, u = 1..N+1 stored at index u (N+2 doubles, index 0 unused; Eq. 11)
+ *   pnext[l] = Pr[G(l) = l+1], l = 1..N stored at l-1 (N doubles; Eq. 13). */
+int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext);
+
+/* Advance nsteps MD steps (asynchronous on the stream):
+ *   thermostat half step ; v += dt/2 F ; x += dt v ; F = F(x) ; v += dt/2 F ; thermostat half step
+ * Forces of the starting state are evaluated first if they are not cached. */
+int pimd_step(pimd_t h, int nsteps);
+
+/* Estimators at the current positions (R9, R15), HOST outputs:
+ *   e_prim = P d N/(2 beta) - <E_c> + Ubar   (thermodynamic estimator, -d ln Z/d beta of Eq. 4)
+ *   e_vir  = Ubar + 1/2 sum r.grad Ubar       (virial estimator; valid in the trap)
+ *   hist[b], b < nbins: number of beads with |r| in [b, b+1) * rmax/nbins (raw counts as doubles;
+ *   beads with |r| >= rmax are dropped).  nbins may be 0 (hist ignored).  Synchronises. */
+int pimd_estimators(pimd_t h, double *e_prim, double *e_vir, double *hist, int nbins, double rmax);
+
+/* Device time of the kernels of the last pimd_forces()/pimd_step() force evaluation is not
+ * recorded here; use CUDA events on the stream.  The number of kernel launches issued by the
+ * library since creation (for bench.py's gpu_launches): */
+uint64_t pimd_launch_count(pimd_t h);
+
+/* Measured FP64 FMA issue rate of the device (a register-resident DFMA loop over all SMs; used
+ * as the ALU roofline denominator).  tflops is HOST out (2 flop per DFMA). */
+int pimd_probe_fp64_peak(void *cuda_stream, double *tflops);
+
+const char *pimd_last_error(pimd_t h); /* h may be NULL: error of the last failed pimd_create */
+const char *pimd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIMD_H */

@@ -1,0 +1,875 @@
+// CUDA kernels of the PIMD hot path (sm_100a, FP64, no tensor cores: d <= 3 is not a contraction).
+// Notation follows arXiv 2404.02628 and DESIGN.md; 0-based indices in code.
+//
+// Exchange part in "generic recursion" form:
+//   both Eq. 6 (forward) and Eq. 11 (backward) are instances of
+//       R_i = log sum_{j<=i} sg_j exp( g_j - kk |rho_i - sig_j|^2 ),   g_{i+1} = R_i + cc_i,
+//   kk = beta k_s / 2 = P/(2 beta), with
+//   forward : rho_i = r_i^P, sig_j = r_j^1, g_j = a[j+1] = L_j + beta S[j] - (j+1) lambda
+//   backward: rho_i = r_u^1, sig_j = r_l^P with u = N-1-i, l = N-1-j, g_j = q[l] - q[N]
+//   cc = beta C(l,l+1) - lambda - ln(l+1)   (the same array, read in opposite order).
+#pragma once
+#include "pimd_math.cuh"
+
+namespace pimd {
+
+// ------------------------------------------------------------------------------------------
+// small vector helpers; coordinate arrays are [n][D] packed doubles
+// ------------------------------------------------------------------------------------------
+template <int D> struct Vec { double v[D]; };
+
+template <int D> PIMD_DEV Vec<D> ldvec(const double *p, size_t i)
+{
+    Vec<D> r;
+    if constexpr (D == 2) {
+        double2 t = *reinterpret_cast<const double2 *>(p + 2 * i);
+        r.v[0] = t.x; r.v[1] = t.y;
+    } else {
+#pragma unroll
+        for (int c = 0; c < D; ++c) r.v[c] = p[(size_t)D * i + c];
+    }
+    return r;
+}
+template <int D> PIMD_DEV void stvec(double *p, size_t i, const Vec<D> &a)
+{
+    if constexpr (D == 2) {
+        *reinterpret_cast<double2 *>(p + 2 * i) = make_double2(a.v[0], a.v[1]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < D; ++c) p[(size_t)D * i + c] = a.v[c];
+    }
+}
+template <int D> PIMD_DEV double dist2(const Vec<D> &a, const Vec<D> &b)
+{
+    double t = a.v[0] - b.v[0];
+    double r2 = t * t;
+#pragma unroll
+    for (int c = 1; c < D; ++c) { t = a.v[c] - b.v[c]; r2 = fma(t, t, r2); }
+    return r2;
+}
+
+PIMD_DEV int ld_acquire(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+PIMD_DEV void st_release(int *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+PIMD_DEV double2 ldcg2(const double2 *p) { return __ldcg(p); }
+PIMD_DEV double ldcg1(const double *p) { return __ldcg(p); }
+
+// status word bits (device -> host)
+enum { ST_NONFINITE = 1, ST_NODE = 2 };
+
+// ------------------------------------------------------------------------------------------
+// Block-wide sum of one double per thread (deterministic order); result valid in thread 0.
+// ------------------------------------------------------------------------------------------
+template <int NT> PIMD_DEV double block_sum(double v, double *sh /* NT/32 doubles */)
+{
+    v = warp_sum(v);
+    const int w = threadIdx.x >> 5, ln = threadIdx.x & 31;
+    __syncthreads();
+    if (ln == 0) sh[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (w == 0) {
+        r = (ln < NT / 32) ? sh[ln] : 0.0;
+        r = warp_sum(r);
+    }
+    return r;
+}
+
+// ==========================================================================================
+// Step 1+2 of the hot path: spring + trap + pair forces of every bead.
+//   F[j][l] = intra-ring springs (Eq. 17; for j = 1, P the intra-ring half of
+//             Eq. 15/16) - (1/P) omega^2 r (Eq. 4/19) + (1/P) sum_{i != l} (2g/s^2) e^{-r^2/s^2} (r_l - r_i)
+//             (Eq. 18 :142 with v(r) = g e^{-r^2/s^2})
+// grid (ceil(N/TB), P), block TB.  One thread owns one bead (j,l); the slice x[j][.][.] is
+// staged through shared memory in tiles of TB particles, read back as broadcasts.
+// Padding particles sit at +1e150 so that their Gaussian is exactly 0; the i == l term has
+// r = 0 and contributes no force (its energy g is subtracted analytically).
+// EST: also accumulate U_trap, U_pair and the pair virial sum_{i<l} (1 - r^2/s^2) g e^{-r^2/s^2},
+// and the radial histogram.
+// ==========================================================================================
+struct EstAccum {
+    double utrap, upair, virpair, ec, pad[4];
+};
+
+template <int D, bool PAIR, bool EST, int TB>
+__global__ void __launch_bounds__(TB) k_bead(const double *__restrict__ x, double *__restrict__ F, int N, int P,
+                                            double ks, double om2_over_P, double is2, double pair_coef /* 2g/(s^2 P) */,
+                                            double g, EstAccum *est, double *hist, int nbins, double rmax)
+{
+    __shared__ double tile[TB * D];
+    __shared__ double red[TB / 32];
+    const int j = blockIdx.y;
+    const int l = blockIdx.x * TB + threadIdx.x;
+    const bool valid = l < N;
+    const double *xs = x + (size_t)j * N * D;
+    Vec<D> r, f;
+#pragma unroll
+    for (int c = 0; c < D; ++c) { r.v[c] = 1e150; f.v[c] = 0.0; }
+    double r2self = 0.0;
+    if (valid) {
+        r = ldvec<D>(xs, l);
+        // ring-polymer springs inside particle l: neighbours j-1 and j+1 of the same particle.
+        // Beads 1 and P get only their intra-ring neighbour here; the closing springs come from
+        // the exchange kernels (Eq. 15, 16).
+#pragma unroll
+        for (int c = 0; c < D; ++c) f.v[c] = -om2_over_P * r.v[c];
+        if (j > 0) {
+            Vec<D> a = ldvec<D>(xs - (size_t)N * D, l);
+#pragma unroll
+            for (int c = 0; c < D; ++c) f.v[c] -= ks * (r.v[c] - a.v[c]);
+        }
+        if (j < P - 1) {
+            Vec<D> a = ldvec<D>(xs + (size_t)N * D, l);
+#pragma unroll
+            for (int c = 0; c < D; ++c) f.v[c] -= ks * (r.v[c] - a.v[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < D; ++c) r2self = fma(r.v[c], r.v[c], r2self);
+    }
+    double up = 0.0, vir = 0.0;
+    if constexpr (PAIR) {
+        Vec<D> acc;
+#pragma unroll
+        for (int c = 0; c < D; ++c) acc.v[c] = 0.0;
+        const double nis2 = -is2;
+        for (int t0 = 0; t0 < N; t0 += TB) {
+            __syncthreads();
+            {
+                const int i = t0 + threadIdx.x;
+                Vec<D> p;
+                if (i < N) p = ldvec<D>(xs, i);
+                else {
+#pragma unroll
+                    for (int c = 0; c < D; ++c) p.v[c] = -1e150;
+                }
+#pragma unroll
+                for (int c = 0; c < D; ++c) tile[threadIdx.x * D + c] = p.v[c];
+            }
+            __syncthreads();
+#pragma unroll 4
+            for (int k = 0; k < TB; ++k) {
+                Vec<D> dlt;
+#pragma unroll
+                for (int c = 0; c < D; ++c) dlt.v[c] = r.v[c] - tile[k * D + c];
+                double r2 = dlt.v[0] * dlt.v[0];
+#pragma unroll
+                for (int c = 1; c < D; ++c) r2 = fma(dlt.v[c], dlt.v[c], r2);
+                const double arg = r2 * nis2;
+                const double e = exp_fast(arg);
+#pragma unroll
+                for (int c = 0; c < D; ++c) acc.v[c] = fma(e, dlt.v[c], acc.v[c]);
+                if constexpr (EST) {
+                    up += e;
+                    vir = fma(e, arg, vir); // sum e * (-r^2/s^2)
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < D; ++c) f.v[c] = fma(pair_coef, acc.v[c], f.v[c]);
+    }
+    if (valid) stvec<D>(F + (size_t)j * N * D, l, f);
+    if constexpr (EST) {
+        // ordered pairs were summed, including i == l (e = 1, arg = 0): remove it, halve the rest
+        double utr = valid ? 0.5 * om2_over_P * r2self : 0.0; // (1/P) 1/2 omega^2 r^2
+        double upl = 0.0, virl = 0.0;
+        if (PAIR && valid) {
+            upl = 0.5 * g * (up - 1.0);
+            virl = 0.5 * g * (up - 1.0 + vir);
+        }
+        double s1 = block_sum<TB>(utr, red);
+        double s2 = block_sum<TB>(upl, red);
+        double s3 = block_sum<TB>(virl, red);
+        if (threadIdx.x == 0) {
+            atomicAdd(&est->utrap, s1);
+            atomicAdd(&est->upair, s2);
+            atomicAdd(&est->virpair, s3);
+        }
+        if (nbins > 0 && valid) {
+            const double rr = sqrt(r2self);
+            if (rr < rmax) {
+                int b = (int)(rr / rmax * nbins);
+                if (b >= nbins) b = nbins - 1;
+                atomicAdd(&hist[b], 1.0);
+            }
+        }
+    }
+}
+
+// ==========================================================================================
+// Step 3: closing springs the recursion needs outside the N x N part, E_int
+// (Eq. 9), and the generic-recursion inputs.  One thread per particle.
+// ==========================================================================================
+struct ExchPtrs {
+    double *rho[2], *sig[2], *cc[2];
+    double2 *g[2];
+    double *gs[2];
+    double *pan_m[2], *pan_s[2];
+    int *cols_ready;      // [2]
+    int *panel_ready[2];  // [NB]
+    double *acc[2];       // [N][D+2]: sum w, sum w*sig (D), sum w*kk*r2
+    double *eint, *cnext, *cself, *pnext;
+    double *tpart;        // [2*nprepblocks] per-block partial sums of E_int, cnext
+    double2 *rfin;        // [2]
+    double *rsgn;         // [2]
+    int *status;
+};
+
+template <int D, int TB>
+__global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N, int P, int NB, double ks, double kk,
+                                            double lambda, ExchPtrs p)
+{
+    __shared__ double red[TB / 32];
+    const int l = blockIdx.x * TB + threadIdx.x;
+    double e_int = 0.0, cn = 0.0;
+    if (l < N) {
+        const size_t sl = (size_t)N * D;
+        Vec<D> prev = ldvec<D>(x, l);
+        const Vec<D> x1 = prev;
+        double acc = 0.0;
+        for (int j = 1; j < P; ++j) {
+            Vec<D> cur = ldvec<D>(x + (size_t)j * sl, l);
+            acc += dist2<D>(cur, prev);
+            prev = cur;
+        }
+        const Vec<D> xP = prev;
+        e_int = 0.5 * ks * acc;
+        stvec<D>(p.rho[0], l, xP);
+        stvec<D>(p.sig[0], l, x1);
+        stvec<D>(p.rho[1], N - 1 - l, x1);
+        stvec<D>(p.sig[1], N - 1 - l, xP);
+        p.eint[l] = e_int;
+        p.cself[l] = kk * dist2<D>(xP, x1);
+        if (l < N - 1) {
+            Vec<D> x1n = ldvec<D>(x, l + 1);
+            cn = kk * dist2<D>(xP, x1n);
+            const double c = cn - lambda - log((double)(l + 1));
+            p.cc[0][l] = c;
+            p.cc[1][N - 2 - l] = c;
+        }
+        p.cnext[l] = cn;
+#pragma unroll
+        for (int c = 0; c < D + 2; ++c) {
+            p.acc[0][(size_t)l * (D + 2) + c] = 0.0;
+            p.acc[1][(size_t)l * (D + 2) + c] = 0.0;
+        }
+        if (l < NB) { p.panel_ready[0][l] = 0; p.panel_ready[1][l] = 0; }
+        if (l == 0) {
+            p.g[0][0] = make_double2(-lambda, 0.0);
+            p.g[1][0] = make_double2(0.0, 0.0);
+            p.gs[0][0] = 1.0;
+            p.gs[1][0] = 1.0;
+            p.cols_ready[0] = 1;
+            p.cols_ready[1] = 1;
+            *p.status = 0;
+        }
+    }
+    double s1 = block_sum<TB>(e_int, red);
+    double s2 = block_sum<TB>(cn, red);
+    if (threadIdx.x == 0) {
+        p.tpart[2 * blockIdx.x] = s1;
+        p.tpart[2 * blockIdx.x + 1] = s2;
+    }
+}
+
+// ==========================================================================================
+// Steps 4+5: the forward (Eq. 6) and backward (Eq. 11) recursions, blocked.
+//
+// grid (1 + nworkers, 2): blockIdx.y = direction, blockIdx.x == 0 the chain CTA, the others
+// panel workers.  Rows/columns are cut into blocks of 32.  For row block K the LSE over columns
+// j <= i is split into
+//   old panel   j < 32 (K - LOOK)          -> a worker CTA, ahead of the chain (log-domain partial)
+//   recent      32 (K - LOOK) <= j < 32 K  -> the chain CTA, all warps
+//   diagonal    32 K <= j <= i             -> the chain CTA, sequential (the dependent part)
+// The chain publishes g_j (double-double) and bumps cols_ready; workers publish (m, s) per row and
+// set panel_ready[K].  All CTAs are co-resident (cooperative launch), so the spins terminate.
+// ==========================================================================================
+constexpr int CH_THREADS = 512;
+constexpr int CH_WARPS = CH_THREADS / 32;
+constexpr int CH_MAXLOOK = 8;
+
+struct ChainArgs {
+    int N, NB, look, nworkers;
+    double kk, sx;
+    ExchPtrs p;
+};
+
+template <int D> PIMD_DEV size_t chain_smem_bytes(int look)
+{
+    const int RB = (look + 1) * 32;
+    size_t b = 0;
+    b += (size_t)RB * sizeof(double2);     // ring g
+    b += (size_t)RB * sizeof(double);      // ring sign
+    b += (size_t)RB * D * sizeof(double);  // ring sig
+    b += 32 * D * sizeof(double);          // rho block
+    b += (size_t)look * 32 * 33 * sizeof(double); // tau
+    b += 64 * sizeof(double);              // pm, ps
+    return b;
+}
+template <int D> size_t chain_smem_bytes_host(int look)
+{
+    const int RB = (look + 1) * 32;
+    size_t chain = (size_t)RB * 16 + (size_t)RB * 8 + (size_t)RB * D * 8 + 32 * D * 8 + (size_t)look * 32 * 33 * 8 + 64 * 8;
+    size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
+    return chain > worker ? chain : worker;
+}
+
+template <int D, bool SGN>
+__device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
+{
+    const int N = a.N, LOOK = a.look, RB = (a.look + 1) * 32;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    double2 *ring_g = reinterpret_cast<double2 *>(smem_raw);
+    double *ring_sg = reinterpret_cast<double *>(ring_g + RB);
+    double *ring_sig = ring_sg + RB;
+    double *rho_s = ring_sig + (size_t)RB * D;
+    double *tau_s = rho_s + 32 * D;
+    double *pm = tau_s + (size_t)LOOK * 32 * 33;
+    double *ps = pm + 32;
+
+    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
+    double2 *g = a.p.g[dir];
+    double *gs = a.p.gs[dir];
+    const double kk = a.kk;
+
+    if (tid == 0) {
+        ring_g[0] = g[0];
+        ring_sg[0] = 1.0;
+    }
+    // prefetch registers: thread t < 32 holds row/column t of the next block
+    Vec<D> pre_rho, pre_sig;
+    double pre_cc = 0.0;
+    auto prefetch = [&](int i0) {
+        const int i = i0 + tid;
+        if (tid < 32) {
+#pragma unroll
+            for (int c = 0; c < D; ++c) { pre_rho.v[c] = 0.0; pre_sig.v[c] = 0.0; }
+            pre_cc = 0.0;
+            if (i < N) {
+                pre_rho = ldvec<D>(rho, i);
+                pre_sig = ldvec<D>(sig, i);
+                if (i < N - 1) pre_cc = cc[i];
+            }
+        }
+    };
+    prefetch(0);
+    double my_cc = 0.0;
+
+    for (int K = 0; K < a.NB; ++K) {
+        const int i0 = K * 32;
+        const int nrows = min(32, N - i0);
+        const int jrec0 = max(0, 32 * (K - LOOK));
+        const int nrec = i0 - jrec0;
+        if (tid < 32) {
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                rho_s[tid * D + c] = pre_rho.v[c];
+                ring_sig[((i0 + tid) % RB) * D + c] = pre_sig.v[c];
+            }
+            my_cc = pre_cc;
+        }
+        prefetch(i0 + 32);
+        __syncthreads();
+        const double2 ref = ring_g[i0 % RB];
+
+        // ---- recent tiles: tau[c][r] = (g_j - ref) - kk |rho_r - sig_j|^2
+        for (int e = tid; e < nrec * 32; e += CH_THREADS) {
+            const int c = e >> 5, r = e & 31;
+            const int slot = (jrec0 + c) % RB;
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[r * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
+            tau_s[c * 33 + r] = dd_diff(ring_g[slot], ref) - kk * dist2<D>(pr, pc);
+        }
+        __syncthreads();
+        for (int r = warp; r < 32; r += CH_WARPS) {
+            double m = -INFINITY;
+            for (int c = lane; c < nrec; c += 32) m = fmax(m, tau_s[c * 33 + r]);
+            m = warp_max(m);
+            double s = 0.0;
+            for (int c = lane; c < nrec; c += 32) {
+                double e = exp_fast(tau_s[c * 33 + r] - m);
+                if constexpr (SGN) e *= ring_sg[(jrec0 + c) % RB];
+                s += e;
+            }
+            s = warp_sum(s);
+            if (lane == 0) { pm[r] = m; ps[r] = s; }
+        }
+        __syncthreads();
+
+        // ---- warp 0: merge the old panel, then the dependent diagonal part
+        if (warp == 0) {
+            const int r = lane;
+            Lse acc = Lse{pm[r], ps[r]};
+            if (nrec == 0) acc = lse_empty();
+            if (jrec0 > 0) {
+                if (lane == 0) {
+                    while (ld_acquire(&a.p.panel_ready[dir][K]) == 0) { }
+                }
+                __syncwarp();
+                Lse o = lse_empty();
+                if (i0 + r < N) {
+                    o.m = ldcg1(&a.p.pan_m[dir][i0 + r]);
+                    o.s = ldcg1(&a.p.pan_s[dir][i0 + r]);
+                }
+                lse_shift(o, dd_diff(ring_g[jrec0 % RB], ref)); // worker reference = g_{jrec0}
+                lse_merge(acc, o);
+            }
+            Vec<D> pr;
+#pragma unroll
+            for (int k = 0; k < D; ++k) pr.v[k] = rho_s[r * D + k];
+            double y = 0.0;
+            double ysg = SGN ? ring_sg[i0 % RB] : 1.0;
+            for (int rp = 0; rp < nrows; ++rp) {
+                Vec<D> pc;
+#pragma unroll
+                for (int k = 0; k < D; ++k) pc.v[k] = ring_sig[((i0 + rp) % RB) * D + k];
+                if (r >= rp) lse_add(acc, y - kk * dist2<D>(pr, pc), ysg);
+                const double Rv = acc.m + log(fabs(acc.s));
+                const double nsg = SGN ? ((acc.s < 0.0) ? -a.sx : a.sx) : 1.0;
+                const double ynext_l = Rv + my_cc;
+                if (lane == rp) {
+                    if (!(fabs(acc.s) > 0.0) || !(fabs(Rv) < INFINITY)) atomicOr(a.p.status, (acc.s == 0.0) ? ST_NODE : ST_NONFINITE);
+                    const int jn = i0 + rp + 1;
+                    if (jn < N) {
+                        const double2 gn = dd_add_d(ref, ynext_l);
+                        ring_g[jn % RB] = gn;
+                        ring_sg[jn % RB] = nsg;
+                        g[jn] = gn;
+                        gs[jn] = nsg;
+                    } else {
+                        a.p.rfin[dir] = dd_add_d(ref, Rv);
+                        a.p.rsgn[dir] = (acc.s < 0.0) ? -1.0 : 1.0;
+                    }
+                }
+                y = __shfl_sync(0xffffffffu, ynext_l, rp);
+                if constexpr (SGN) ysg = __shfl_sync(0xffffffffu, nsg, rp);
+            }
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 33));
+        }
+        __syncthreads();
+    }
+}
+
+template <int D, bool SGN>
+__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw)
+{
+    const int N = a.N, LOOK = a.look;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // per-warp staging of one column tile: g (dd), sign, sig
+    double2 *st_g = reinterpret_cast<double2 *>(smem_raw) + warp * 32;
+    double *st_sg = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + warp * 32;
+    double *st_sig = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + CH_WARPS * 32 + warp * 32 * D;
+    double *mg_m = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + CH_WARPS * 32 + CH_WARPS * 32 * D;
+    double *mg_s = mg_m + CH_WARPS * 32;
+
+    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir];
+    const double2 *g = a.p.g[dir];
+    const double *gs = a.p.gs[dir];
+    const int *cols_ready = &a.p.cols_ready[dir];
+    const double kk = a.kk;
+    int known_ready = 0;
+
+    for (int K = LOOK + 1 + widx; K < a.NB; K += a.nworkers) {
+        const int i = K * 32 + lane;
+        Vec<D> pr;
+#pragma unroll
+        for (int c = 0; c < D; ++c) pr.v[c] = 0.0;
+        if (i < N) pr = ldvec<D>(rho, i);
+        const int ntile = K - LOOK;
+        Lse acc = lse_empty();
+        double2 ref = make_double2(0.0, 0.0);
+        for (int J = warp; J < ntile; J += CH_WARPS) {
+            const int need = 32 * (J + 1);
+            if (known_ready < need) {
+                if (lane == 0) {
+                    int v;
+                    while ((v = ld_acquire(cols_ready)) < need) { }
+                    known_ready = v;
+                }
+                known_ready = __shfl_sync(0xffffffffu, known_ready, 0);
+            }
+            __syncwarp();
+            {
+                const int j = 32 * J + lane;
+                st_g[lane] = ldcg2(&g[j]);
+                if constexpr (SGN) st_sg[lane] = ldcg1(&gs[j]);
+                Vec<D> pc = ldvec<D>(sig, j);
+#pragma unroll
+                for (int c = 0; c < D; ++c) st_sig[lane * D + c] = pc.v[c];
+            }
+            __syncwarp();
+            const double2 nref = st_g[0];
+            lse_shift(acc, dd_diff(ref, nref));
+            ref = nref;
+#pragma unroll 1
+            for (int c0 = 0; c0 < 32; c0 += 8) {
+                double tau[8];
+                double cm = -INFINITY;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    Vec<D> pc;
+#pragma unroll
+                    for (int c = 0; c < D; ++c) pc.v[c] = st_sig[(c0 + k) * D + c];
+                    tau[k] = dd_diff(st_g[c0 + k], ref) - kk * dist2<D>(pr, pc);
+                    cm = fmax(cm, tau[k]);
+                }
+                if (cm > acc.m) {
+                    acc.s *= exp_fast(acc.m - cm);
+                    acc.m = cm;
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    double e = exp_fast(tau[k] - acc.m);
+                    if constexpr (SGN) e *= st_sg[c0 + k];
+                    acc.s += e;
+                }
+            }
+            __syncwarp();
+        }
+        // common reference of the published partial: g_{32 ntile} (first "recent" column of block K)
+        {
+            const int need = 32 * ntile + 1;
+            if (known_ready < need) {
+                if (lane == 0) {
+                    int v;
+                    while ((v = ld_acquire(cols_ready)) < need) { }
+                    known_ready = v;
+                }
+                known_ready = __shfl_sync(0xffffffffu, known_ready, 0);
+            }
+            __syncwarp();
+            const double2 pub = ldcg2(&g[32 * ntile]);
+            lse_shift(acc, dd_diff(ref, pub));
+        }
+        mg_m[warp * 32 + lane] = acc.m;
+        mg_s[warp * 32 + lane] = acc.s;
+        __syncthreads();
+        if (warp == 0) {
+            Lse t = lse_empty();
+            for (int w = 0; w < CH_WARPS; ++w) lse_merge(t, Lse{mg_m[w * 32 + lane], mg_s[w * 32 + lane]});
+            if (i < N) {
+                a.p.pan_m[dir][i] = t.m;
+                a.p.pan_s[dir][i] = t.s;
+            }
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release(&a.p.panel_ready[dir][K], 1);
+        }
+        __syncthreads();
+    }
+}
+
+template <int D, bool SGN>
+__global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int dir = blockIdx.y;
+    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw);
+}
+
+// ==========================================================================================
+// Step 6: connection probabilities (Eq. 12) and the sums the
+// exterior-bead forces need (Eq. 15, 16), no N x N storage:
+//   Pr[l -> l'] = sg exp( qhat[l] + a[l'] - kk |r_l^P - r_l'^1|^2 - R_N ),  l' <= l
+// In generic form, for direction dir and lane row i:
+//   w_ij = exp( g^{other}[N-1-i] + g^{dir}[j] - kk |rho_i - sig_j|^2 - R_N ),  j <= i
+//   acc[dir][i] = ( sum_j w, sum_j w sig_j, sum_j w kk r^2 )
+// dir 0 gives the row sums (bead P, Eq. 16), dir 1 the column sums (bead 1, Eq. 15).
+// grid (NT, NT, 2) over 128 x 128 tiles of the lower triangle; block 128.
+// ==========================================================================================
+constexpr int FP_TB = 128;
+
+template <int D, bool SGN>
+__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p)
+{
+    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
+    if (ct > rt) return;
+    __shared__ double2 sg_g[FP_TB];
+    __shared__ double sg_s[FP_TB];
+    __shared__ double sg_sig[FP_TB * D];
+    const double2 *gd = p.g[dir], *go = p.g[1 - dir];
+    const int i = rt * FP_TB + threadIdx.x;
+    const int j0 = ct * FP_TB;
+    {
+        const int j = j0 + threadIdx.x;
+        double2 gj = make_double2(-INFINITY, 0.0);
+        double sj = 1.0;
+        Vec<D> sc;
+#pragma unroll
+        for (int c = 0; c < D; ++c) sc.v[c] = 0.0;
+        if (j < N) {
+            gj = gd[j];
+            if constexpr (SGN) sj = p.gs[dir][j];
+            sc = ldvec<D>(p.sig[dir], j);
+        }
+        sg_g[threadIdx.x] = gj;
+        sg_s[threadIdx.x] = sj;
+#pragma unroll
+        for (int c = 0; c < D; ++c) sg_sig[threadIdx.x * D + c] = sc.v[c];
+    }
+    __syncthreads();
+    if (i >= N) return;
+    const Vec<D> pr = ldvec<D>(p.rho[dir], i);
+    // A = g^{other}[N-1-i] - R_N as dd, rounded once per element after adding g^{dir}[j]
+    const double2 A = dd_sub(go[N - 1 - i], p.rfin[0]);
+    double osg = 1.0;
+    if constexpr (SGN) osg = p.gs[1 - dir][N - 1 - i] * p.rsgn[0];
+    const int ncol = min(FP_TB, i - j0 + 1); // columns j0 .. min(j0+127, i)
+    double sw = 0.0, swc = 0.0;
+    Vec<D> sws;
+#pragma unroll
+    for (int c = 0; c < D; ++c) sws.v[c] = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < ncol; ++k) {
+        Vec<D> pc;
+#pragma unroll
+        for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
+        const double2 gj = sg_g[k];
+        const double kr2 = kk * dist2<D>(pr, pc);
+        double w = exp_fast(((A.x + gj.x) + (A.y + gj.y)) - kr2);
+        if constexpr (SGN) w *= sg_s[k];
+        sw += w;
+        swc = fma(w, kr2, swc);
+#pragma unroll
+        for (int c = 0; c < D; ++c) sws.v[c] = fma(w, pc.v[c], sws.v[c]);
+    }
+    double *o = p.acc[dir] + (size_t)i * (D + 2);
+    atomicAdd(&o[0], osg * sw);
+#pragma unroll
+    for (int c = 0; c < D; ++c) atomicAdd(&o[1 + c], osg * sws.v[c]);
+    atomicAdd(&o[D + 1], osg * swc);
+}
+
+// ==========================================================================================
+// Eq. 13 and the assembly of the exterior forces (Eq. 15, 16):
+//   Pr[l -> l+1] = 1 - xi (l+1) sg exp( qhat[l] + a[l+1] - beta C(l,l+1) - R_N )
+//   FexP[l] = -k_s ( r_l^P - sum_{l'} Pr[l -> l'] r_l'^1 ),  Fex1[l] = -k_s ( r_l^1 - sum_{l'} Pr[l' -> l] r_l'^P )
+// (the intra-ring halves -k_s (r^P - r^{P-1}), -k_s (r^1 - r^2) are in k_bead; rows sum to 1).
+// One thread per particle.  ecpart: per-block partial sums of sum_{l'} Pr[l->l'] beta C(l,l').
+// ==========================================================================================
+template <int D, bool SGN, int TB>
+__global__ void __launch_bounds__(TB) k_assemble(int N, double ks, double xi, ExchPtrs p, double *Fex1, double *FexP,
+                                                double *ecpart)
+{
+    __shared__ double red[TB / 32];
+    const int l = blockIdx.x * TB + threadIdx.x;
+    double ec = 0.0;
+    if (l < N) {
+        const double2 R = p.rfin[0];
+        const double rs = SGN ? p.rsgn[0] : 1.0;
+        auto pn = [&](int m) -> double { // Pr[m -> m+1], 0 <= m <= N-2
+            const double2 A = dd_sub(p.g[1][N - 1 - m], R);
+            const double2 B = p.g[0][m + 1];
+            double w = exp_fast(((A.x + B.x) + (A.y + B.y)) - p.cnext[m]);
+            if constexpr (SGN) w *= p.gs[1][N - 1 - m] * p.gs[0][m + 1] * rs;
+            return 1.0 - xi * (double)(m + 1) * w;
+        };
+        const double pl = (l < N - 1) ? pn(l) : 0.0;
+        const double pm1 = (l > 0) ? pn(l - 1) : 0.0;
+        p.pnext[l] = pl;
+        const Vec<D> xP = ldvec<D>(p.rho[0], l), x1 = ldvec<D>(p.sig[0], l);
+        const double *a0 = p.acc[0] + (size_t)l * (D + 2);
+        const double *a1 = p.acc[1] + (size_t)(N - 1 - l) * (D + 2);
+        Vec<D> fP, f1;
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            double sP = a0[1 + c];
+            if (l < N - 1) sP = fma(pl, p.sig[0][(size_t)(l + 1) * D + c], sP);
+            double s1 = a1[1 + c];
+            if (l > 0) s1 = fma(pm1, p.rho[0][(size_t)(l - 1) * D + c], s1);
+            fP.v[c] = -ks * (xP.v[c] - sP);
+            f1.v[c] = -ks * (x1.v[c] - s1);
+        }
+        stvec<D>(FexP, l, fP);
+        stvec<D>(Fex1, l, f1);
+        ec = a0[D + 1] + pl * p.cnext[l];
+    }
+    double s = block_sum<TB>(ec, red);
+    if (threadIdx.x == 0) ecpart[blockIdx.x] = s;
+}
+
+// xi = 0 (0^0 = 1): only k = 1 survives in Eq. 6, Pr is the identity, every ring closes
+// on itself.  V = sum_l E^{[l,l]} + (1/beta) ln N!.
+template <int D, int TB>
+__global__ void __launch_bounds__(TB) k_exch_xi0(int N, double ks, ExchPtrs p, double *Fex1, double *FexP, double *ecpart)
+{
+    __shared__ double red[TB / 32];
+    const int l = blockIdx.x * TB + threadIdx.x;
+    double ec = 0.0;
+    if (l < N) {
+        const Vec<D> xP = ldvec<D>(p.rho[0], l), x1 = ldvec<D>(p.sig[0], l);
+        Vec<D> fP, f1;
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            fP.v[c] = -ks * (xP.v[c] - x1.v[c]);
+            f1.v[c] = -ks * (x1.v[c] - xP.v[c]);
+        }
+        stvec<D>(FexP, l, fP);
+        stvec<D>(Fex1, l, f1);
+        p.pnext[l] = 0.0;
+        ec = p.cself[l];
+    }
+    double s = block_sum<TB>(ec, red);
+    if (threadIdx.x == 0) ecpart[blockIdx.x] = s;
+}
+
+// ==========================================================================================
+// Scalars of one evaluation: V_xi^{[1,N]} = T_N - (R_N + N lambda - ln N)/beta (from Eq. 6 with the
+// de-trended variable), its sign, <E_c> for the primitive estimator.  One block.
+// ==========================================================================================
+struct Scalars {
+    double vb, sign, ec, sum_eint, sum_cnext_beta, pad[3];
+};
+
+template <int TB>
+__global__ void __launch_bounds__(TB) k_finalize(int N, int nprep, int nasm, double beta, double lambda, double xi,
+                                                double lgammaN1, ExchPtrs p, const double *ecpart, Scalars *out)
+{
+    __shared__ double red[TB / 32];
+    double a = 0.0, b = 0.0, c = 0.0;
+    for (int i = threadIdx.x; i < nprep; i += TB) { a += p.tpart[2 * i]; b += p.tpart[2 * i + 1]; }
+    for (int i = threadIdx.x; i < nasm; i += TB) c += ecpart[i];
+    a = block_sum<TB>(a, red);
+    b = block_sum<TB>(b, red);
+    c = block_sum<TB>(c, red);
+    if (threadIdx.x == 0) {
+        out->sum_eint = a;
+        out->sum_cnext_beta = b;
+        out->ec = a + c / beta;
+        if (xi == 0.0) {
+            out->vb = a + c / beta + lgammaN1 / beta; // sum_l (E_int + C(l,l)) + ln N!/beta
+            out->sign = 1.0;
+        } else {
+            const double2 R = p.rfin[0];
+            const double TN = a + b / beta;
+            // L_N = R_N - beta T_N + N lambda - ln N
+            out->vb = TN - ((R.x + ((double)N * lambda - log((double)N))) + R.y) / beta;
+            const double sx = xi < 0.0 ? -1.0 : 1.0;
+            out->sign = p.rsgn[0] * (((N + 1) & 1) ? sx : 1.0);
+        }
+    }
+}
+
+// ==========================================================================================
+// Step 7: velocity Verlet + thermostat (R10), fused:
+//   [close step s: v += dt/2 F ; thermostat half]  [open step s+1: thermostat half ; v += dt/2 F ; x += dt v]
+// One thread per degree of freedom.  F_total = F + exterior exchange forces on beads 1 and P.
+// ==========================================================================================
+PIMD_DEV void nhc_half(double &vi, double *vx, double h, double kT, double Q)
+{
+    constexpr int M = 4;
+    double G;
+    G = (Q * vx[M - 2] * vx[M - 2] - kT) / Q;
+    vx[M - 1] += 0.5 * h * G;
+#pragma unroll
+    for (int k = M - 2; k >= 0; --k) {
+        const double a = exp(-0.25 * h * vx[k + 1]);
+        G = (k == 0) ? (vi * vi - kT) / Q : (Q * vx[k - 1] * vx[k - 1] - kT) / Q;
+        vx[k] = (vx[k] * a + 0.5 * h * G) * a;
+    }
+    vi *= exp(-h * vx[0]);
+#pragma unroll
+    for (int k = 0; k <= M - 2; ++k) {
+        const double a = exp(-0.25 * h * vx[k + 1]);
+        G = (k == 0) ? (vi * vi - kT) / Q : (Q * vx[k - 1] * vx[k - 1] - kT) / Q;
+        vx[k] = (vx[k] * a + 0.5 * h * G) * a;
+    }
+    G = (Q * vx[M - 2] * vx[M - 2] - kT) / Q;
+    vx[M - 1] += 0.5 * h * G;
+}
+
+template <int THERMO>
+__global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, double *__restrict__ v, const double *__restrict__ F,
+                                                  const double *__restrict__ Fex1, const double *__restrict__ FexP,
+                                                  double *__restrict__ nhc, size_t ndof, size_t slice /* N*d */, int P,
+                                                  double dt, double c1, double c2, double beta, double Q, uint64_t seed,
+                                                  uint64_t step_close, uint64_t step_open, int do_close, int do_open,
+                                                  int *status)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= ndof) return;
+    const size_t j = idx / slice, rem = idx - j * slice;
+    double f = F[idx];
+    if (j == 0) f += Fex1[rem];
+    if (j == (size_t)(P - 1)) f += FexP[rem];
+    double vi = v[idx];
+    double vx[4];
+    if constexpr (THERMO == 2) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) vx[k] = nhc[(size_t)k * ndof + idx];
+    }
+    const double hdt = 0.5 * dt;
+    if (do_close) {
+        vi = fma(hdt, f, vi);
+        if constexpr (THERMO == 1) {
+            double z0, z1;
+            philox_normal(seed, idx, step_close, z0, z1);
+            vi = c1 * vi + c2 * z1;
+        } else if constexpr (THERMO == 2) {
+            nhc_half(vi, vx, hdt, 1.0 / beta, Q);
+        }
+    }
+    if (do_open) {
+        if constexpr (THERMO == 1) {
+            double z0, z1;
+            philox_normal(seed, idx, step_open, z0, z1);
+            vi = c1 * vi + c2 * z0;
+        } else if constexpr (THERMO == 2) {
+            nhc_half(vi, vx, hdt, 1.0 / beta, Q);
+        }
+        vi = fma(hdt, f, vi);
+        const double xn = fma(dt, vi, x[idx]);
+        x[idx] = xn;
+        if (!(fabs(xn) < INFINITY)) atomicOr(status + 1, ST_NONFINITE);
+    }
+    v[idx] = vi;
+    if constexpr (THERMO == 2) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) nhc[(size_t)k * ndof + idx] = vx[k];
+    }
+}
+
+__global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const double *__restrict__ F,
+                                                const double *__restrict__ Fex1, const double *__restrict__ FexP, size_t ndof,
+                                                size_t slice, int P)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= ndof) return;
+    const size_t j = idx / slice, rem = idx - j * slice;
+    double f = F[idx];
+    if (j == 0) f += Fex1[rem];
+    if (j == (size_t)(P - 1)) f += FexP[rem];
+    out[idx] = f;
+}
+
+__global__ void k_zero(double *p, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = 0.0;
+}
+
+// FP64 FMA issue-rate probe: 8 independent chains per thread, register resident.
+__global__ void __launch_bounds__(256) k_dfma_probe(double *out, int iters, double a, double b)
+{
+    double c0 = threadIdx.x, c1 = c0 + 1, c2 = c0 + 2, c3 = c0 + 3, c4 = c0 + 4, c5 = c0 + 5, c6 = c0 + 6, c7 = c0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            c0 = fma(c0, a, b); c1 = fma(c1, a, b); c2 = fma(c2, a, b); c3 = fma(c3, a, b);
+            c4 = fma(c4, a, b); c5 = fma(c5, a, b); c6 = fma(c6, a, b); c7 = fma(c7, a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((c0 + c1) + (c2 + c3)) + ((c4 + c5) + (c6 + c7));
+}
+
+} // namespace pimd

@@ -1,0 +1,154 @@
+// Device math helpers of the PIMD hot path: exp for the log-sum-exp passes and the Gaussian pair
+// kernel, double-double differences, signed log-sum-exp accumulators, Philox4x32-10.
+// Nothing here is shared with oracle/ (the oracle has its own plain-C versions).
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#define PIMD_DEV __device__ __forceinline__
+
+namespace pimd {
+
+// ---------------------------------------------------------------------------------------------
+// exp(x) for x <= ~700, no special-case branches: 0 for x < -708 (and for -inf), garbage-in /
+// garbage-out for NaN (non-finite state is detected elsewhere).  Cody-Waite reduction
+// x = k ln2 + r, |r| <= ln2/2, degree-13 Taylor polynomial (truncation 4e-18), 2^k folded into
+// the exponent field.  17 FP64 instructions; max relative error ~2e-16.
+// ---------------------------------------------------------------------------------------------
+PIMD_DEV double exp_fast(double x)
+{
+    const double MAGIC = 6755399441055744.0; // 1.5 * 2^52
+    double t = fma(x, 1.4426950408889634074, MAGIC);
+    int k = __double2loint(t);
+    double kd = t - MAGIC;
+    double r = fma(kd, -6.93147180369123816490e-01, x);
+    r = fma(kd, -1.90821492927058770002e-10, r);
+    double p = 1.6059043836821613e-10;           // 1/13!
+    p = fma(p, r, 2.08767569878680989792e-09);   // 1/12!
+    p = fma(p, r, 2.50521083854417187751e-08);   // 1/11!
+    p = fma(p, r, 2.75573192239858906526e-07);   // 1/10!
+    p = fma(p, r, 2.75573192239858906526e-06);   // 1/9!
+    p = fma(p, r, 2.48015873015873015873e-05);   // 1/8!
+    p = fma(p, r, 1.98412698412698412698e-04);   // 1/7!
+    p = fma(p, r, 1.38888888888888888889e-03);   // 1/6!
+    p = fma(p, r, 8.33333333333333333333e-03);   // 1/5!
+    p = fma(p, r, 4.16666666666666666667e-02);   // 1/4!
+    p = fma(p, r, 1.66666666666666666667e-01);   // 1/3!
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    int hi = __double2hiint(p) + (k << 20);
+    double res = __hiloint2double(hi, __double2loint(p));
+    return (x < -708.0) ? 0.0 : res;
+}
+
+// ---------------------------------------------------------------------------------------------
+// double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
+// tables a[u], q[l] reach 1e5..1e7 in magnitude while only their DIFFERENCES enter an exp, so
+// they are carried as dd and differenced before rounding to double.
+// ---------------------------------------------------------------------------------------------
+PIMD_DEV double2 dd_add_d(double2 a, double b) // a + b, b a plain double
+{
+    double s = a.x + b;
+    double bb = s - a.x;
+    double e = (a.x - (s - bb)) + (b - bb); // TwoSum error
+    e += a.y;
+    double hi = s + e;
+    double lo = e - (hi - s);
+    return make_double2(hi, lo);
+}
+PIMD_DEV double2 dd_sub(double2 a, double2 b) // a - b as dd
+{
+    double s = a.x - b.x;
+    double bb = s - a.x;
+    double e = (a.x - (s - bb)) + (-b.x - bb);
+    e += (a.y - b.y);
+    double hi = s + e;
+    double lo = e - (hi - s);
+    return make_double2(hi, lo);
+}
+PIMD_DEV double dd_diff(double2 a, double2 b) // (a - b) rounded to double
+{
+    return (a.x - b.x) + (a.y - b.y);
+}
+
+// ---------------------------------------------------------------------------------------------
+// signed log-sum-exp accumulator: sum_i sg_i exp(t_i) = s * exp(m), m = running max of t_i.
+// ---------------------------------------------------------------------------------------------
+struct Lse {
+    double m, s;
+};
+PIMD_DEV Lse lse_empty() { return Lse{-INFINITY, 0.0}; }
+PIMD_DEV void lse_add(Lse &a, double t, double sg)
+{
+    double dlt = t - a.m;             // +inf when the accumulator is empty
+    double e = exp_fast(-fabs(dlt));  // exp(-inf) = 0
+    if (dlt > 0.0) {
+        a.s = fma(a.s, e, sg);
+        a.m = t;
+    } else {
+        a.s = fma(sg, e, a.s);
+    }
+}
+PIMD_DEV void lse_merge(Lse &a, const Lse &b)
+{
+    if (b.m == -INFINITY) return;
+    if (a.m == -INFINITY) { a = b; return; }
+    double dlt = b.m - a.m;
+    double e = exp_fast(-fabs(dlt));
+    if (dlt > 0.0) {
+        a.s = fma(a.s, e, b.s);
+        a.m = b.m;
+    } else {
+        a.s = fma(b.s, e, a.s);
+    }
+}
+PIMD_DEV void lse_shift(Lse &a, double delta) // re-reference: all t_i -> t_i + delta
+{
+    if (a.m != -INFINITY) a.m += delta;
+}
+
+// warp reductions (all 32 lanes participate)
+PIMD_DEV double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+PIMD_DEV double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11): counter (dof_lo, dof_hi, step_lo, step_hi), key
+// (seed_lo, seed_hi); 53-bit uniforms from word pairs; Box-Muller.  z0 opens MD step `step`,
+// z1 closes it.
+// ---------------------------------------------------------------------------------------------
+PIMD_DEV void philox_normal(uint64_t seed, uint64_t dof, uint64_t step, double &z0, double &z1)
+{
+    uint32_t c0 = (uint32_t)dof, c1 = (uint32_t)(dof >> 32), c2 = (uint32_t)step, c3 = (uint32_t)(step >> 32);
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    uint64_t a = ((uint64_t)c0 << 32) | c1, b = ((uint64_t)c2 << 32) | c3;
+    double u1 = ((double)(a >> 11) + 0.5) * 0x1.0p-53;
+    double u2 = ((double)(b >> 11) + 0.5) * 0x1.0p-53;
+    double r = sqrt(-2.0 * log(u1));
+    double sn, cs;
+    sincos(6.283185307179586476925286766559 * u2, &sn, &cs);
+    z0 = r * cs;
+    z1 = r * sn;
+}
+
+} // namespace pimd
