@@ -122,6 +122,22 @@ int pimd_estimators(pimd_t h, double *e_prim, double *e_vir, double *hist, int n
  * library since creation (for bench.py's gpu_launches): */
 uint64_t pimd_launch_count(pimd_t h);
 
+/* Per-kernel device time.  With profiling on, every kernel launch is bracketed by a pair of CUDA
+ * events on the stream it is launched on.  pimd_get_profile() synchronises, adds up the elapsed
+ * times per slot since the previous call (milliseconds, and launch counts), returns them in the
+ * HOST arrays ms_host / count_host (PIMD_PROF_NSLOTS entries each; either may be NULL) and resets. */
+#define PIMD_PROF_BEAD 0      /* spring + trap + pair forces (steps 1, 2) */
+#define PIMD_PROF_PREP 1      /* closing springs, E_int, recursion inputs (step 3) */
+#define PIMD_PROF_CHAIN 2     /* forward + backward recursions (steps 4, 5) */
+#define PIMD_PROF_FORCEPASS 3 /* connection probabilities and their sums (step 6) */
+#define PIMD_PROF_ASSEMBLE 4  /* Eq. 13 and exterior forces (step 6) */
+#define PIMD_PROF_FINALIZE 5  /* V_B, sign, <E_c> */
+#define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
+#define PIMD_PROF_COMBINE 7   /* force output */
+#define PIMD_PROF_NSLOTS 8
+int pimd_set_profiling(pimd_t h, int on);
+int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
+
 /* Measured FP64 FMA issue rate of the device (a register-resident DFMA loop over all SMs; used
  * as the ALU roofline denominator).  tflops is HOST out (2 flop per DFMA). */
 int pimd_probe_fp64_peak(void *cuda_stream, double *tflops);

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpimd.so")
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 THERMOSTAT_NVE, THERMOSTAT_LANGEVIN, THERMOSTAT_NHC = 0, 1, 2
 NHC_LENGTH = 4
+PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine")
 
 # every symbol include/pimd.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
@@ -41,6 +42,8 @@ _SYMBOLS = {
     "pimd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_estimators": (C.c_int, [C.c_void_p, _dp, _dp, C.c_void_p, C.c_int, C.c_double]),
     "pimd_launch_count": (C.c_uint64, [C.c_void_p]),
+    "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_get_profile": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_probe_fp64_peak": (C.c_int, [C.c_void_p, _dp]),
     "pimd_last_error": (C.c_char_p, [C.c_void_p]),
     "pimd_version": (C.c_char_p, []),
@@ -206,6 +209,16 @@ class Pimd:
         hist = np.zeros(max(int(nbins), 1))
         self._check(self._lib.pimd_estimators(self._h, C.byref(ep), C.byref(ev), _ptr(hist), int(nbins), float(rmax)))
         return ep.value, ev.value, hist[: int(nbins)].copy()
+
+    def set_profiling(self, on):
+        self._check(self._lib.pimd_set_profiling(self._h, int(bool(on))))
+
+    def get_profile(self):
+        """{slot name: (total ms, launches)} since the previous call."""
+        ms = (C.c_double * len(PROF_SLOTS))()
+        cnt = (C.c_uint64 * len(PROF_SLOTS))()
+        self._check(self._lib.pimd_get_profile(self._h, ms, cnt))
+        return {name: (float(ms[i]), int(cnt[i])) for i, name in enumerate(PROF_SLOTS)}
 
     def launch_count(self):
         return int(self._lib.pimd_launch_count(self._h))

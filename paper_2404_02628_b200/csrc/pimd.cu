@@ -55,6 +55,12 @@ struct pimd_s {
     int coop_max_blocks; // co-resident CTA limit of k_chain
     size_t chain_smem;
     uint64_t launches;
+    // per-kernel device timing (pimd_set_profiling)
+    bool profiling;
+    std::vector<cudaEvent_t> *prof_ev;   // pairs (start, stop)
+    std::vector<int> *prof_slot;
+    double prof_ms[PIMD_PROF_NSLOTS];
+    uint64_t prof_n[PIMD_PROF_NSLOTS];
     char err[512];
 };
 
@@ -75,6 +81,35 @@ int fail(pimd_t h, int code, const char *fmt, ...)
         cudaError_t e__ = (call);                                                                         \
         if (e__ != cudaSuccess) return fail(h, PIMD_ECUDA, "%s: %s", #call, cudaGetErrorString(e__));     \
     } while (0)
+
+// RAII bracket of one kernel launch with a pair of events on its stream (profiling mode only)
+struct ProfScope {
+    pimd_t h;
+    cudaStream_t st;
+    cudaEvent_t stop;
+    ProfScope(pimd_t h_, int slot, cudaStream_t st_) : h(h_), st(st_), stop(nullptr)
+    {
+        h->launches++;
+        if (!h->profiling) return;
+        cudaEvent_t a = nullptr, b = nullptr;
+        const size_t k = h->prof_slot->size();
+        if (h->prof_ev->size() >= 2 * k + 2) { // recycled pair
+            a = (*h->prof_ev)[2 * k];
+            b = (*h->prof_ev)[2 * k + 1];
+        } else {
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+            h->prof_ev->push_back(a);
+            h->prof_ev->push_back(b);
+        }
+        h->prof_slot->push_back(slot);
+        cudaEventRecord(a, st);
+        stop = b;
+    }
+    ~ProfScope()
+    {
+        if (stop) cudaEventRecord(stop, st);
+    }
+};
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -166,12 +201,14 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
     const bool pair = h->g != 0.0;
 #define LB(PAIR, EST) \
     k_bead<D, PAIR, EST, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, coef, h->g, h->est, h->hist, nbins, rmax)
-    if (pair && est) LB(true, true);
-    else if (pair) LB(true, false);
-    else if (est) LB(false, true);
-    else LB(false, false);
+    {
+        ProfScope ps(h, PIMD_PROF_BEAD, st);
+        if (pair && est) LB(true, true);
+        else if (pair) LB(true, false);
+        else if (est) LB(false, true);
+        else LB(false, false);
+    }
 #undef LB
-    h->launches++;
     CU(cudaGetLastError());
     return PIMD_OK;
 }
@@ -179,12 +216,16 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
 template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
 {
     const bool sgn = h->xi < 0.0;
-    k_prep<D, PREP_TB><<<h->nprep, PREP_TB, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
-    h->launches++;
+    {
+        ProfScope ps(h, PIMD_PROF_PREP, st);
+        k_prep<D, PREP_TB><<<h->nprep, PREP_TB, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
+    }
     CU(cudaGetLastError());
     if (h->xi == 0.0) {
-        k_exch_xi0<D, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->ex, h->Fex1, h->FexP, h->ecpart);
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
+            k_exch_xi0<D, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->ex, h->Fex1, h->FexP, h->ecpart);
+        }
         CU(cudaGetLastError());
     } else {
         ChainArgs a;
@@ -193,23 +234,31 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         void *args[] = {&a};
         const dim3 grid(1 + h->nworkers, 2), block(CH_THREADS);
         const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
-        CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_CHAIN, st);
+            CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
+        }
         const int NT = (h->N + FP_TB - 1) / FP_TB;
         const dim3 fgrid(NT, NT, 2);
-        if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
-        else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
+            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+        }
         CU(cudaGetLastError());
-        if (sgn) k_assemble<D, true, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
-        else k_assemble<D, false, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
+            if (sgn) k_assemble<D, true, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
+            else k_assemble<D, false, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
+        }
         CU(cudaGetLastError());
     }
     if (scalars) {
-        k_finalize<256><<<1, 256, 0, st>>>(h->N, h->nprep, h->nasm, h->beta, h->lambda, h->xi, std::lgamma((double)h->N + 1.0),
-                                           h->ex, h->ecpart, h->scal);
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_FINALIZE, st);
+            k_finalize<256><<<1, 256, 0, st>>>(h->N, h->nprep, h->nasm, h->beta, h->lambda, h->xi, std::lgamma((double)h->N + 1.0),
+                                               h->ex, h->ecpart, h->scal);
+        }
         CU(cudaGetLastError());
     }
     return PIMD_OK;
@@ -259,11 +308,13 @@ int launch_integrate(pimd_t h, bool do_close, bool do_open, uint64_t step_close,
 #define LI(T) \
     k_integrate<T><<<grid, 256, 0, h->s0>>>(h->x, h->v, h->F, h->Fex1, h->FexP, h->nhc, h->ndof, h->slice, h->P, h->dt, c1, c2, \
                                             h->beta, Q, h->seed, step_close, step_open, do_close ? 1 : 0, do_open ? 1 : 0, h->status)
-    if (h->thermostat == PIMD_THERMOSTAT_LANGEVIN) LI(1);
-    else if (h->thermostat == PIMD_THERMOSTAT_NHC) LI(2);
-    else LI(0);
+    {
+        ProfScope ps(h, PIMD_PROF_INTEGRATE, h->s0);
+        if (h->thermostat == PIMD_THERMOSTAT_LANGEVIN) LI(1);
+        else if (h->thermostat == PIMD_THERMOSTAT_NHC) LI(2);
+        else LI(0);
+    }
 #undef LI
-    h->launches++;
     CU(cudaGetLastError());
     return PIMD_OK;
 }
@@ -324,6 +375,8 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     h->nasm = (N + ASM_TB - 1) / ASM_TB;
     h->look = 1;
     h->concurrent = true;
+    h->prof_ev = new std::vector<cudaEvent_t>();
+    h->prof_slot = new std::vector<int>();
     int rc = PIMD_OK;
     auto bail = [&](int code) { std::snprintf(g_create_error, 512, "%s", h->err); pimd_destroy(h); return code; };
     switch (d) {
@@ -361,6 +414,11 @@ int pimd_destroy(pimd_t h)
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_est) cudaFreeHost(h->h_est);
     if (h->h_status) cudaFreeHost(h->h_status);
+    if (h->prof_ev) {
+        for (cudaEvent_t e : *h->prof_ev) cudaEventDestroy(e);
+        delete h->prof_ev;
+        delete h->prof_slot;
+    }
     delete h;
     return PIMD_OK;
 }
@@ -476,8 +534,10 @@ static int forces_impl(pimd_t h, double *f, bool host, double *vb, int *sign)
     if (rc) return rc;
     if (f) {
         double *dst = host ? h->Fout : f;
-        k_combine<<<(unsigned)((h->ndof + 255) / 256), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P);
-        h->launches++;
+        {
+            ProfScope ps(h, PIMD_PROF_COMBINE, h->s0);
+            k_combine<<<(unsigned)((h->ndof + 255) / 256), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P);
+        }
         CU(cudaGetLastError());
         if (host) CU(cudaMemcpyAsync(f, h->Fout, h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
     }
@@ -598,6 +658,34 @@ int pimd_estimators(pimd_t h, double *e_prim, double *e_vir, double *hist, int n
 }
 
 uint64_t pimd_launch_count(pimd_t h) { return h ? h->launches : 0; }
+
+int pimd_set_profiling(pimd_t h, int on)
+{
+    if (!h) return PIMD_EINVAL;
+    h->profiling = on != 0;
+    return PIMD_OK;
+}
+
+int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host)
+{
+    if (!h) return PIMD_EINVAL;
+    CU(cudaStreamSynchronize(h->s0));
+    CU(cudaStreamSynchronize(h->s1));
+    for (size_t i = 0; i < h->prof_slot->size(); ++i) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, (*h->prof_ev)[2 * i], (*h->prof_ev)[2 * i + 1]));
+        h->prof_ms[(*h->prof_slot)[i]] += ms;
+        h->prof_n[(*h->prof_slot)[i]]++;
+    }
+    h->prof_slot->clear(); // the events stay in the pool
+    for (int k = 0; k < PIMD_PROF_NSLOTS; ++k) {
+        if (ms_host) ms_host[k] = h->prof_ms[k];
+        if (count_host) count_host[k] = h->prof_n[k];
+        h->prof_ms[k] = 0.0;
+        h->prof_n[k] = 0;
+    }
+    return PIMD_OK;
+}
 
 int pimd_probe_fp64_peak(void *cuda_stream, double *tflops)
 {
