@@ -300,25 +300,21 @@ struct ChainArgs {
     ExchPtrs p;
 };
 
-template <int D> PIMD_DEV size_t chain_smem_bytes(int look)
-{
-    const int RB = (look + 1) * 32;
-    size_t b = 0;
-    b += (size_t)RB * sizeof(double2);     // ring g
-    b += (size_t)RB * sizeof(double);      // ring sign
-    b += (size_t)RB * D * sizeof(double);  // ring sig
-    b += 32 * D * sizeof(double);          // rho block
-    b += (size_t)look * 32 * 33 * sizeof(double); // tau
-    b += 64 * sizeof(double);              // pm, ps
-    return b;
-}
 template <int D> size_t chain_smem_bytes_host(int look)
 {
     const int RB = (look + 1) * 32;
-    size_t chain = (size_t)RB * 16 + (size_t)RB * 8 + (size_t)RB * D * 8 + 32 * D * 8 + (size_t)look * 32 * 33 * 8 + 64 * 8;
+    size_t chain = (size_t)RB * 16 + (size_t)RB * 8 + (size_t)RB * D * 8 + 32 * D * 8 + (size_t)look * 32 * 33 * 8 + 64 * 8 +
+                   (size_t)(32 * 32 + 40 + 32) * 8; // + diagonal tile, gauge t[0..32], row gauges
     size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
     return chain > worker ? chain : worker;
 }
+
+#ifdef PIMD_CHAIN_TIMING
+__device__ long long g_chain_cyc[16];
+#define CT(k) do { if (tid == 0 && dir == 0) { long long c__ = clock64(); g_chain_cyc[k] += c__ - tprev; tprev = c__; } } while (0)
+#else
+#define CT(k) do { } while (0)
+#endif
 
 template <int D, bool SGN>
 __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
@@ -332,6 +328,9 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
     double *tau_s = rho_s + 32 * D;
     double *pm = tau_s + (size_t)LOOK * 32 * 33;
     double *ps = pm + 32;
+    double *dg_s = ps + 32;        // diagonal tile [p][r]: tau, then M
+    double *ts_s = dg_s + 32 * 32; // column gauges t_0..t_32
+    double *mxf_s = ts_s + 40;     // row gauges G_r
 
     const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
     double2 *g = a.p.g[dir];
@@ -361,7 +360,11 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
     prefetch(0);
     double my_cc = 0.0;
 
+#ifdef PIMD_CHAIN_TIMING
+    long long tprev = clock64();
+#endif
     for (int K = 0; K < a.NB; ++K) {
+        CT(0);
         const int i0 = K * 32;
         const int nrows = min(32, N - i0);
         const int jrec0 = max(0, 32 * (K - LOOK));
@@ -376,9 +379,11 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
         }
         prefetch(i0 + 32);
         __syncthreads();
+        CT(1);
         const double2 ref = ring_g[i0 % RB];
 
-        // ---- recent tiles: tau[c][r] = (g_j - ref) - kk |rho_r - sig_j|^2
+        // ---- recent tiles: tau[c][r] = (g_j - ref) - kk |rho_r - sig_j|^2, and the diagonal
+        // tile dg[p][r] = -kk |rho_r - sig_{i0+p}|^2 (p <= r; -inf above the diagonal)
         for (int e = tid; e < nrec * 32; e += CH_THREADS) {
             const int c = e >> 5, r = e & 31;
             const int slot = (jrec0 + c) % RB;
@@ -387,7 +392,16 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
             for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[r * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
             tau_s[c * 33 + r] = dd_diff(ring_g[slot], ref) - kk * dist2<D>(pr, pc);
         }
+        for (int e = tid; e < 32 * 32; e += CH_THREADS) {
+            const int p = e >> 5, r = e & 31;
+            const int slot = (i0 + p) % RB;
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[r * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
+            dg_s[e] = (p <= r) ? -kk * dist2<D>(pr, pc) : -INFINITY;
+        }
         __syncthreads();
+        CT(2);
         for (int r = warp; r < 32; r += CH_WARPS) {
             double m = -INFINITY;
             for (int c = lane; c < nrec; c += 32) m = fmax(m, tau_s[c * 33 + r]);
@@ -403,7 +417,16 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
         }
         __syncthreads();
 
-        // ---- warp 0: merge the old panel, then the dependent diagonal part
+        // ---- the dependent 32 x 32 diagonal part, warp 0, lane = row r.
+        // With Z_p = exp(g_{i0+p} - ref) and A_r = the sum over all earlier columns (relative to ref):
+        //   X_r = A_r + sum_{p<=r} Z_p exp(dg[p][r]),   Z_{r+1} = sx X_r exp(cc_r).
+        // Pass 1 (max-plus): t_0 = 0, G_r = max(log|A_r|, max_{p<=r}(t_p + dg[p][r])), t_{r+1} = G_r + cc_r.
+        // Pass 2 (all threads): M[p][r] = exp(t_p + dg[p][r] - G_r) <= 1, Ahat_r = A_r exp(-G_r).
+        // Pass 3 (linear): Zhat_0 = +-1, acc_r = Ahat_r + sum_p M[p][r] Zhat_p, Zhat_{r+1} = sx acc_r (1 + delta_r),
+        //   delta_r = the rounding error of G_r + cc_r, so that Z_p = Zhat_p exp(t_p) holds to ~1 ulp.
+        // By construction 1 <= |Zhat| <= 33! for xi > 0: no overflow or underflow for any input.
+        double logA = 0.0, sgnA = 1.0, G = 0.0, tnext = 0.0, delta = 0.0;
+        CT(3);
         if (warp == 0) {
             const int r = lane;
             Lse acc = Lse{pm[r], ps[r]};
@@ -421,39 +444,73 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
                 lse_shift(o, dd_diff(ring_g[jrec0 % RB], ref)); // worker reference = g_{jrec0}
                 lse_merge(acc, o);
             }
-            Vec<D> pr;
+            CT(4);
+            logA = acc.m + log(fabs(acc.s)); // -inf when there is no earlier column
+            if constexpr (SGN) sgnA = (acc.s < 0.0) ? -1.0 : 1.0;
+            double tau[32];
 #pragma unroll
-            for (int k = 0; k < D; ++k) pr.v[k] = rho_s[r * D + k];
-            double y = 0.0;
-            double ysg = SGN ? ring_sg[i0 % RB] : 1.0;
-            for (int rp = 0; rp < nrows; ++rp) {
-                Vec<D> pc;
+            for (int p = 0; p < 32; ++p) tau[p] = dg_s[p * 32 + lane];
+            double mx = logA, tcur = 0.0;
 #pragma unroll
-                for (int k = 0; k < D; ++k) pc.v[k] = ring_sig[((i0 + rp) % RB) * D + k];
-                if (r >= rp) lse_add(acc, y - kk * dist2<D>(pr, pc), ysg);
-                const double Rv = acc.m + log(fabs(acc.s));
-                const double nsg = SGN ? ((acc.s < 0.0) ? -a.sx : a.sx) : 1.0;
-                const double ynext_l = Rv + my_cc;
-                if (lane == rp) {
-                    if (!(fabs(acc.s) > 0.0) || !(fabs(Rv) < INFINITY)) atomicOr(a.p.status, (acc.s == 0.0) ? ST_NODE : ST_NONFINITE);
-                    const int jn = i0 + rp + 1;
-                    if (jn < N) {
-                        const double2 gn = dd_add_d(ref, ynext_l);
-                        ring_g[jn % RB] = gn;
-                        ring_sg[jn % RB] = nsg;
-                        g[jn] = gn;
-                        gs[jn] = nsg;
-                    } else {
-                        a.p.rfin[dir] = dd_add_d(ref, Rv);
-                        a.p.rsgn[dir] = (acc.s < 0.0) ? -1.0 : 1.0;
-                    }
+            for (int p = 0; p < 32; ++p) {
+                if (lane == 0) ts_s[p] = tcur;
+                mx = fmax(mx, tcur + tau[p]); // no effect once p > r
+                tcur = __shfl_sync(0xffffffffu, mx + my_cc, p);
+            }
+            G = mx;
+            tnext = G + my_cc; // the value lane r broadcast at step r: t_{r+1}
+            {
+                const double bb = tnext - G;
+                delta = (G - (tnext - bb)) + (my_cc - bb);
+            }
+            mxf_s[lane] = G;
+            CT(5);
+        }
+        __syncthreads();
+        for (int e = tid; e < 32 * 32; e += CH_THREADS) {
+            const int p = e >> 5, r = e & 31;
+            dg_s[e] = (p <= r) ? exp_fast((ts_s[p] + dg_s[e]) - mxf_s[r]) : 0.0;
+        }
+        __syncthreads();
+        CT(6);
+        if (warp == 0) {
+            const int r = lane;
+            double M[32];
+#pragma unroll
+            for (int p = 0; p < 32; ++p) M[p] = dg_s[p * 32 + lane];
+            double accl = sgnA * exp_fast(logA - G);
+            double zcur = SGN ? ring_sg[i0 % RB] : 1.0;
+#pragma unroll
+            for (int p = 0; p < 32; ++p) {
+                accl = fma(M[p], zcur, accl); // M[p] = 0 once p > r
+                double zn = fma(accl, delta, accl);
+                if constexpr (SGN) zn *= a.sx;
+                zcur = __shfl_sync(0xffffffffu, zn, p);
+            }
+            CT(7);
+            // row r: R_r = ref + G_r + log|acc_r| ;  g_{r+1} = ref + t_{r+1} + log|Zhat_{r+1}|
+            const double la = log(fabs(accl));
+            const double lz = log(fabs(fma(accl, delta, accl)));
+            const double nsg = SGN ? ((accl < 0.0) ? -a.sx : a.sx) : 1.0;
+            if (r < nrows) {
+                if (!(fabs(accl) > 0.0) || !(fabs(la) < INFINITY) || !(fabs(G) < INFINITY))
+                    atomicOr(a.p.status, (accl == 0.0) ? ST_NODE : ST_NONFINITE);
+                const int jn = i0 + r + 1;
+                if (jn < N) {
+                    const double2 gn = dd_add_d(dd_add_d(ref, tnext), lz);
+                    ring_g[jn % RB] = gn;
+                    ring_sg[jn % RB] = nsg;
+                    g[jn] = gn;
+                    gs[jn] = nsg;
+                } else {
+                    a.p.rfin[dir] = dd_add_d(dd_add_d(ref, G), la);
+                    a.p.rsgn[dir] = (accl < 0.0) ? -1.0 : 1.0;
                 }
-                y = __shfl_sync(0xffffffffu, ynext_l, rp);
-                if constexpr (SGN) ysg = __shfl_sync(0xffffffffu, nsg, rp);
             }
             __threadfence();
             __syncwarp();
             if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 33));
+            CT(8);
         }
         __syncthreads();
     }
