@@ -213,14 +213,19 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
     return PIMD_OK;
 }
 
-template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
+template <int D> int launch_prep(pimd_t h, cudaStream_t st)
 {
-    const bool sgn = h->xi < 0.0;
     {
         ProfScope ps(h, PIMD_PROF_PREP, st);
         k_prep<D, PREP_TB><<<h->nprep, PREP_TB, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
     }
     CU(cudaGetLastError());
+    return PIMD_OK;
+}
+
+template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
+{
+    const bool sgn = h->xi < 0.0;
     if (h->xi == 0.0) {
         {
             ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
@@ -264,31 +269,38 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
     return PIMD_OK;
 }
 
-// one force evaluation: exchange part on the helper stream, bead (spring/trap/pair) part on the
-// main stream, joined before returning (in stream order)
+// one force evaluation.  The exchange part stays on the main stream (k_prep, then the latency-bound
+// k_chain, which must get its SMs first), the bead part (spring/trap/pair) is forked onto the helper
+// stream after k_prep and fills the remaining SMs; joined before returning (in stream order).
 int eval_forces(pimd_t h, bool scalars, bool est, int nbins, double rmax)
 {
     int rc = ensure_ws(h);
     if (rc) return rc;
-    cudaStream_t se = h->concurrent ? h->s1 : h->s0;
     if (est) {
         CU(cudaMemsetAsync(h->est, 0, sizeof(EstAccum), h->s0));
         if (nbins > 0) CU(cudaMemsetAsync(h->hist, 0, (size_t)nbins * 8, h->s0));
     }
+    cudaStream_t sb = h->concurrent ? h->s1 : h->s0;
+    switch (h->d) {
+    case 1: rc = launch_prep<1>(h, h->s0); break;
+    case 2: rc = launch_prep<2>(h, h->s0); break;
+    default: rc = launch_prep<3>(h, h->s0); break;
+    }
+    if (rc) return rc;
     if (h->concurrent) {
         CU(cudaEventRecord(h->ev_fork, h->s0));
         CU(cudaStreamWaitEvent(h->s1, h->ev_fork, 0));
     }
     switch (h->d) {
-    case 1: rc = launch_exchange<1>(h, se, scalars); break;
-    case 2: rc = launch_exchange<2>(h, se, scalars); break;
-    default: rc = launch_exchange<3>(h, se, scalars); break;
+    case 1: rc = launch_exchange<1>(h, h->s0, scalars); break;
+    case 2: rc = launch_exchange<2>(h, h->s0, scalars); break;
+    default: rc = launch_exchange<3>(h, h->s0, scalars); break;
     }
     if (rc) return rc;
     switch (h->d) {
-    case 1: rc = launch_bead<1>(h, h->s0, est, nbins, rmax); break;
-    case 2: rc = launch_bead<2>(h, h->s0, est, nbins, rmax); break;
-    default: rc = launch_bead<3>(h, h->s0, est, nbins, rmax); break;
+    case 1: rc = launch_bead<1>(h, sb, est, nbins, rmax); break;
+    case 2: rc = launch_bead<2>(h, sb, est, nbins, rmax); break;
+    default: rc = launch_bead<3>(h, sb, est, nbins, rmax); break;
     }
     if (rc) return rc;
     if (h->concurrent) {
@@ -373,7 +385,11 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     h->NB = (N + 31) / 32;
     h->nprep = (N + PREP_TB - 1) / PREP_TB;
     h->nasm = (N + ASM_TB - 1) / ASM_TB;
-    h->look = 1;
+    h->look = 2;
+    if (const char *e = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
+        const int v = std::atoi(e);
+        if (v >= 1 && v <= CH_MAXLOOK) h->look = v;
+    }
     h->concurrent = true;
     h->prof_ev = new std::vector<cudaEvent_t>();
     h->prof_slot = new std::vector<int>();
@@ -386,10 +402,18 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     }
     if (rc) return bail(rc);
     {
+        // Panel workers per direction.  A worker spins while it waits for columns and owns a whole SM,
+        // so only as many as the panel work needs are launched: at ~7e3 cycles per 32-row block of the
+        // chain one SM keeps up with ~16 column tiles per block.
         const int want = h->NB - h->look - 1;
         int cap = h->coop_max_blocks / 2 - 1;
-        if (cap > 64) cap = 64;
-        h->nworkers = want < 0 ? 0 : (want < cap ? want : cap);
+        int need = (h->NB + 11) / 12;
+        if (const char *e = std::getenv("PIMD_WORKERS")) {
+            const int v = std::atoi(e);
+            if (v >= 1) need = v;
+        }
+        if (need > cap) need = cap;
+        h->nworkers = want <= 0 ? 0 : (want < need ? want : need);
         if (want > 0 && h->nworkers < 1) return bail(fail(h, PIMD_ECUDA, "not enough co-resident CTAs for the recursion"));
     }
     if (cudaStreamCreateWithFlags(&h->s1, cudaStreamNonBlocking) != cudaSuccess ||
@@ -562,10 +586,12 @@ int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
     if (vfwd || vbwd) {
         // V^{[1,n]} and V^{[u,N]} from the de-trended tables g: prefix sums of E_int and C(l,l+1)
         // are diagnostics of the evaluation, formed here in long double.
-        std::vector<double> gf(2 * (size_t)(N + 1)), gb(2 * (size_t)(N + 1)), eint(N), cnext(N);
+        std::vector<double> gf(2 * (size_t)(N + 1)), gb(2 * (size_t)(N + 1)), zf(N + 1), zb(N + 1), eint(N), cnext(N);
         double rf[4];
         CU(cudaMemcpyAsync(gf.data(), h->ex.g[0], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
         CU(cudaMemcpyAsync(gb.data(), h->ex.g[1], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(zf.data(), h->ex.gs[0], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(zb.data(), h->ex.gs[1], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
         CU(cudaMemcpyAsync(eint.data(), h->ex.eint, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
         CU(cudaMemcpyAsync(cnext.data(), h->ex.cnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
         CU(cudaMemcpyAsync(rf, h->ex.rfin, 32, cudaMemcpyDeviceToHost, h->s0));
@@ -578,8 +604,9 @@ int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
             T[v] = S[v - 1] + eint[v - 1];
             S[v] = T[v] + (v < N ? (long double)cnext[v - 1] / beta : 0.0L);
         }
-        auto gfv = [&](int j) -> long double { return j < N ? (long double)gf[2 * j] + gf[2 * j + 1] : 0.0L; };
-        auto gbv = [&](int j) -> long double { return (long double)gb[2 * j] + gb[2 * j + 1]; };
+        // g_j = T_j + log|Zhat_j| (the recursion carries the gauge T and the linear factor Zhat)
+        auto gfv = [&](int j) -> long double { return j < N ? (long double)gf[2 * j] + gf[2 * j + 1] + logl(fabsl((long double)zf[j])) : 0.0L; };
+        auto gbv = [&](int j) -> long double { return (long double)gb[2 * j] + gb[2 * j + 1] + logl(fabsl((long double)zb[j])); };
         if (vfwd) {
             vfwd[0] = 0.0;
             for (int n = 1; n <= N; ++n) {

@@ -208,8 +208,8 @@ __global__ void __launch_bounds__(TB) k_bead(const double *__restrict__ x, doubl
 // ==========================================================================================
 struct ExchPtrs {
     double *rho[2], *sig[2], *cc[2];
-    double2 *g[2];
-    double *gs[2];
+    double2 *g[2];        // [N+1] gauge T_j (double-double): g_j = T_j + log|Zhat_j|
+    double *gs[2];        // [N+1] Zhat_j: linear, signed, O(1)-ranged factor of exp(g_j)
     double *pan_m[2], *pan_s[2];
     int *cols_ready;      // [2]
     int *panel_ready[2];  // [NB]
@@ -287,12 +287,13 @@ __global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N
 //   old panel   j < 32 (K - LOOK)          -> a worker CTA, ahead of the chain (log-domain partial)
 //   recent      32 (K - LOOK) <= j < 32 K  -> the chain CTA, all warps
 //   diagonal    32 K <= j <= i             -> the chain CTA, sequential (the dependent part)
-// The chain publishes g_j (double-double) and bumps cols_ready; workers publish (m, s) per row and
-// set panel_ready[K].  All CTAs are co-resident (cooperative launch), so the spins terminate.
+// The chain publishes (T_j, Zhat_j) with exp(g_j) = Zhat_j exp(T_j) and bumps cols_ready; workers
+// publish (m, s) per row and set panel_ready[K].  All CTAs are co-resident (cooperative launch), so
+// the spins terminate.
 // ==========================================================================================
 constexpr int CH_THREADS = 512;
 constexpr int CH_WARPS = CH_THREADS / 32;
-constexpr int CH_MAXLOOK = 8;
+constexpr int CH_MAXLOOK = 6;
 
 struct ChainArgs {
     int N, NB, look, nworkers;
@@ -300,219 +301,404 @@ struct ChainArgs {
     ExchPtrs p;
 };
 
-template <int D> size_t chain_smem_bytes_host(int look)
-{
-    const int RB = (look + 1) * 32;
-    size_t chain = (size_t)RB * 16 + (size_t)RB * 8 + (size_t)RB * D * 8 + 32 * D * 8 + (size_t)look * 32 * 33 * 8 + 64 * 8 +
-                   (size_t)(32 * 32 + 40 + 32) * 8; // + diagonal tile, gauge t[0..32], row gauges
-    size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
-    return chain > worker ? chain : worker;
-}
 
 #ifdef PIMD_CHAIN_TIMING
 __device__ long long g_chain_cyc[16];
-#define CT(k) do { if (tid == 0 && dir == 0) { long long c__ = clock64(); g_chain_cyc[k] += c__ - tprev; tprev = c__; } } while (0)
+__device__ long long g_chain_arr[3][8];
+__device__ unsigned long long g_chain_gt[8];
+PIMD_DEV unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define CT(k) do { if (tid == 0 && dir == 0) { long long c__ = clock64(); g_chain_cyc[k] += c__ - tprev; } tprev = clock64(); } while (0)
+// arrival of warps 0, 1 and 15 at the barrier that ends phase k, measured from the phase start
+#define CTA(k) do { if (lane == 0 && dir == 0 && (warp <= 1 || warp == CH_WARPS - 1)) g_chain_arr[warp == 0 ? 0 : (warp == 1 ? 1 : 2)][k] += clock64() - tprev; } while (0)
 #else
 #define CT(k) do { } while (0)
+#define CTA(k) do { } while (0)
 #endif
 
+// Shared-memory layout of the chain CTA (doubles); L = look.
+template <int D> struct ChainSmem {
+    int RB;                   // ring capacity in columns: 32 (L + 2)
+    size_t ringT, ringZ, ringSig, rho, cc, dg, dgf, ts, dlt, Gs, zeta, partM, partS, apart, sh, total;
+    __host__ __device__ explicit ChainSmem(int L)
+    {
+        RB = 32 * (L + 2);
+        size_t o = 0;
+        ringT = o; o += 2 * (size_t)RB;          // double2 per column: the gauge T_j (double-double)
+        ringZ = o; o += RB;                      // Zhat_j (signed)
+        ringSig = o; o += (size_t)RB * D;
+        rho = o; o += 2 * 32 * D;                // rows of blocks K, K+1 (double buffered)
+        cc = o; o += 2 * 32;
+        dg = o; o += 2 * 32 * 32;                // diagonal tiles of blocks K, K+1: tau, then M
+        dgf = o; o += 2 * 32 * 32 / 2;           // the same tau tiles as float (max-plus pass)
+        ts = o; o += 20;                         // column gauges t_0..t_32 of the block (relative to Tref_K), float
+        dlt = o; o += 40;                        // dlt[p] = t~_p - t_p (rounding remainder of the gauge)
+        Gs = o; o += 32;                         // row gauges G_r
+        zeta = o; o += 2 * 40;                   // Zhat of the block's columns, double buffered
+        partM = o; o += 2 * (size_t)(L + 1) * 32;    // contributions of earlier columns to the NEXT block's rows:
+        partS = o; o += 2 * (size_t)(L + 1) * 32; //   slot 0 panel (workers), 1 previous block, 2..L older blocks
+        apart = o; o += (size_t)(L + 1) * 32;
+        sh = o; o += 8;
+        total = o;
+    }
+};
+
+template <int D> size_t chain_smem_bytes_host(int look)
+{
+    const size_t chain = ChainSmem<D>(look).total * 8;
+    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
+    return chain > worker ? chain : worker;
+}
+
+PIMD_DEV void bar_sync_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// floor(log2|s|) * ln 2 from the exponent field: a lower bound of log|s| within ln 2 (gauge use only)
+PIMD_DEV double approx_log_abs(double s)
+{
+    const int e = (__double2hiint(s) >> 20) & 0x7ff;
+    return (double)(e - 1023) * 0.6931471805599453;
+}
+
+// ==========================================================================================
+// The chain CTA.  Columns carry g_j = T_j + log|Zhat_j| as a
+// double-double gauge T_j and a linear, signed, O(1)-ranged factor Zhat_j; no log or exp sits on
+// the dependent path.  Per block K of 32 rows (rows and columns i0 = 32 K .. i0 + 31):
+//   P1  warp 0: max-plus ("tropical") pass in FP32 -> column gauges t_p, row gauges G_r.
+//       helpers (warps 1..15): diagonal tau tile of block K+1; contributions of the column blocks
+//       K+1-q, q = 2..L, to the rows of block K+1.
+//   P2  all: M[p][r] = exp(t~_p + tau[p][r] - G_r) <= 1;  Ahat parts = s exp(m - G_r).
+//   P3  warp 0: linear pass  acc_r = Ahat_r + sum_p M[p][r] Zhat_p,  Zhat_{r+1} = sx acc_r.
+//       helpers: exp part of the contribution of block K's columns to the rows of block K+1;
+//       one helper warp fetches the workers' panel for block K+1.
+//   P4  all: finish that contribution (needs Zhat), publish T, Zhat (ring + global), load the
+//       coordinates of block K+2.
+// ==========================================================================================
 template <int D, bool SGN>
 __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
 {
-    const int N = a.N, LOOK = a.look, RB = (a.look + 1) * 32;
+    const int N = a.N, L = a.look;
+    const ChainSmem<D> lay(L);
+    const int RB = lay.RB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    double2 *ring_g = reinterpret_cast<double2 *>(smem_raw);
-    double *ring_sg = reinterpret_cast<double *>(ring_g + RB);
-    double *ring_sig = ring_sg + RB;
-    double *rho_s = ring_sig + (size_t)RB * D;
-    double *tau_s = rho_s + 32 * D;
-    double *pm = tau_s + (size_t)LOOK * 32 * 33;
-    double *ps = pm + 32;
-    double *dg_s = ps + 32;        // diagonal tile [p][r]: tau, then M
-    double *ts_s = dg_s + 32 * 32; // column gauges t_0..t_32
-    double *mxf_s = ts_s + 40;     // row gauges G_r
+    double *sm = reinterpret_cast<double *>(smem_raw);
+    double2 *ring_T = reinterpret_cast<double2 *>(sm + lay.ringT);
+    double *ring_Z = sm + lay.ringZ, *ring_sig = sm + lay.ringSig, *rho_s = sm + lay.rho, *cc_s = sm + lay.cc;
+    float *dgf_s = reinterpret_cast<float *>(sm + lay.dgf), *ts_s = reinterpret_cast<float *>(sm + lay.ts);
+    double *dg_s = sm + lay.dg, *dlt_s = sm + lay.dlt, *G_s = sm + lay.Gs, *zeta_s = sm + lay.zeta;
+    double *part_m = sm + lay.partM, *part_s = sm + lay.partS, *apart_s = sm + lay.apart, *sh_s = sm + lay.sh;
 
     const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
     double2 *g = a.p.g[dir];
     double *gs = a.p.gs[dir];
     const double kk = a.kk;
+    // Helper warps: every warp that does not share warp 0's scheduler partition (warp % 4 != 0), so that
+    // the two dependent passes of warp 0 do not queue behind the helpers' FP64 work; the last warp
+    // talks to global memory (publishes columns, fetches the workers' panel and the next coordinates).
+    constexpr int NH = 11, NHT = NH * 32;
+    const bool is_io = (warp == CH_WARPS - 1);
+    const bool is_helper = (warp & 3) != 0 && !is_io;
+    const int hidx = warp - 1 - (warp >> 2), ht = hidx * 32 + lane;
 
-    if (tid == 0) {
-        ring_g[0] = g[0];
-        ring_sg[0] = 1.0;
-    }
-    // prefetch registers: thread t < 32 holds row/column t of the next block
-    Vec<D> pre_rho, pre_sig;
-    double pre_cc = 0.0;
-    auto prefetch = [&](int i0) {
-        const int i = i0 + tid;
-        if (tid < 32) {
+    // coordinates and cc of block B -> shared (rows: rho_s[B&1], columns: ring_sig); zero padding
+    auto load_block = [&](int B, int t, int nt) {
+        for (int e = t; e < 32; e += nt) {
+            const int i = B * 32 + e;
+            Vec<D> pr, pc;
 #pragma unroll
-            for (int c = 0; c < D; ++c) { pre_rho.v[c] = 0.0; pre_sig.v[c] = 0.0; }
-            pre_cc = 0.0;
+            for (int c = 0; c < D; ++c) { pr.v[c] = 0.0; pc.v[c] = 0.0; }
+            double c0 = 0.0;
             if (i < N) {
-                pre_rho = ldvec<D>(rho, i);
-                pre_sig = ldvec<D>(sig, i);
-                if (i < N - 1) pre_cc = cc[i];
+                pr = ldvec<D>(rho, i);
+                pc = ldvec<D>(sig, i);
+                if (i < N - 1) c0 = cc[i];
             }
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                rho_s[((B & 1) * 32 + e) * D + c] = pr.v[c];
+                ring_sig[((i % RB)) * D + c] = pc.v[c];
+            }
+            cc_s[(B & 1) * 32 + e] = c0;
         }
     };
-    prefetch(0);
-    double my_cc = 0.0;
+    // diagonal tile of block B: dg[B&1][p][r] = -kk |rho_r - sig_{32B+p}|^2 for p <= r, -inf above
+    auto diag_tile = [&](int B, int t, int nt) {
+        double *dgB = dg_s + (B & 1) * 1024;
+        for (int e = t; e < 1024; e += nt) {
+            const int p = e >> 5, r = e & 31;
+            const int slot = (B * 32 + p) % RB;
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[((B & 1) * 32 + r) * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
+            const double tv = (p <= r) ? -kk * dist2<D>(pr, pc) : -INFINITY;
+            dgB[e] = tv;
+            dgf_s[(B & 1) * 1024 + e] = (float)tv;
+        }
+    };
 
+#ifdef PIMD_CHAIN_TIMING
+    if (tid == 0) g_chain_gt[dir * 4 + 0] = gtimer();
+#endif
+    // ---- prologue: blocks 0 and 1, first column, empty parts
+    load_block(0, tid, CH_THREADS);
+    load_block(1, tid, CH_THREADS);
+    if (tid == 0) {
+        ring_T[0] = g[0];
+        ring_Z[0] = 1.0;
+        zeta_s[0] = 1.0;
+        sh_s[0] = 0.0;
+    }
+    for (int e = tid; e < (L + 1) * 32; e += CH_THREADS) { part_m[e] = -INFINITY; part_s[e] = 0.0; }
+    __syncthreads();
+    diag_tile(0, tid, CH_THREADS);
+    __syncthreads();
 #ifdef PIMD_CHAIN_TIMING
     long long tprev = clock64();
 #endif
+    double2 pend_T = make_double2(0.0, 0.0); // warp 15: columns computed in the previous block, to publish
+    double pend_Z = 0.0;
+    int pend_j = -1, pend_ready = 0;
+    Vec<D> pre_rho, pre_sig; // warp 15: coordinates of block K+2 in flight
+    double pre_cc = 0.0;
+
     for (int K = 0; K < a.NB; ++K) {
-        CT(0);
-        const int i0 = K * 32;
+        const int i0 = K * 32, cur = K & 1, nxt = cur ^ 1;
         const int nrows = min(32, N - i0);
-        const int jrec0 = max(0, 32 * (K - LOOK));
-        const int nrec = i0 - jrec0;
-        if (tid < 32) {
-#pragma unroll
-            for (int c = 0; c < D; ++c) {
-                rho_s[tid * D + c] = pre_rho.v[c];
-                ring_sig[((i0 + tid) % RB) * D + c] = pre_sig.v[c];
-            }
-            my_cc = pre_cc;
-        }
-        prefetch(i0 + 32);
-        __syncthreads();
-        CT(1);
-        const double2 ref = ring_g[i0 % RB];
+        const bool has_next = (K + 1 < a.NB);
+        const double2 Tref = ring_T[i0 % RB];
+        double *dgK = dg_s + cur * 1024;
+        double *zK = zeta_s + cur * 40, *zN = zeta_s + nxt * 40;
+        const double *pmK = part_m + cur * (L + 1) * 32, *psK = part_s + cur * (L + 1) * 32;
+        double *pmN = part_m + nxt * (L + 1) * 32, *psN = part_s + nxt * (L + 1) * 32;
+        double G = 0.0, accr = 0.0; // warp 0: row gauge and row sum of lane r
+        double uE[3], uM[3];        // helpers: exp part and maximum of the rows they own in the next block
+        CT(0);
 
-        // ---- recent tiles: tau[c][r] = (g_j - ref) - kk |rho_r - sig_j|^2, and the diagonal
-        // tile dg[p][r] = -kk |rho_r - sig_{i0+p}|^2 (p <= r; -inf above the diagonal)
-        for (int e = tid; e < nrec * 32; e += CH_THREADS) {
-            const int c = e >> 5, r = e & 31;
-            const int slot = (jrec0 + c) % RB;
-            Vec<D> pr, pc;
-#pragma unroll
-            for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[r * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
-            tau_s[c * 33 + r] = dd_diff(ring_g[slot], ref) - kk * dist2<D>(pr, pc);
-        }
-        for (int e = tid; e < 32 * 32; e += CH_THREADS) {
-            const int p = e >> 5, r = e & 31;
-            const int slot = (i0 + p) % RB;
-            Vec<D> pr, pc;
-#pragma unroll
-            for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[r * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
-            dg_s[e] = (p <= r) ? -kk * dist2<D>(pr, pc) : -INFINITY;
-        }
-        __syncthreads();
-        CT(2);
-        for (int r = warp; r < 32; r += CH_WARPS) {
-            double m = -INFINITY;
-            for (int c = lane; c < nrec; c += 32) m = fmax(m, tau_s[c * 33 + r]);
-            m = warp_max(m);
-            double s = 0.0;
-            for (int c = lane; c < nrec; c += 32) {
-                double e = exp_fast(tau_s[c * 33 + r] - m);
-                if constexpr (SGN) e *= ring_sg[(jrec0 + c) % RB];
-                s += e;
-            }
-            s = warp_sum(s);
-            if (lane == 0) { pm[r] = m; ps[r] = s; }
-        }
-        __syncthreads();
-
-        // ---- the dependent 32 x 32 diagonal part, warp 0, lane = row r.
-        // With Z_p = exp(g_{i0+p} - ref) and A_r = the sum over all earlier columns (relative to ref):
-        //   X_r = A_r + sum_{p<=r} Z_p exp(dg[p][r]),   Z_{r+1} = sx X_r exp(cc_r).
-        // Pass 1 (max-plus): t_0 = 0, G_r = max(log|A_r|, max_{p<=r}(t_p + dg[p][r])), t_{r+1} = G_r + cc_r.
-        // Pass 2 (all threads): M[p][r] = exp(t_p + dg[p][r] - G_r) <= 1, Ahat_r = A_r exp(-G_r).
-        // Pass 3 (linear): Zhat_0 = +-1, acc_r = Ahat_r + sum_p M[p][r] Zhat_p, Zhat_{r+1} = sx acc_r (1 + delta_r),
-        //   delta_r = the rounding error of G_r + cc_r, so that Z_p = Zhat_p exp(t_p) holds to ~1 ulp.
-        // By construction 1 <= |Zhat| <= 33! for xi > 0: no overflow or underflow for any input.
-        double logA = 0.0, sgnA = 1.0, G = 0.0, tnext = 0.0, delta = 0.0;
-        CT(3);
+        // ================= P1
         if (warp == 0) {
             const int r = lane;
-            Lse acc = Lse{pm[r], ps[r]};
-            if (nrec == 0) acc = lse_empty();
-            if (jrec0 > 0) {
-                if (lane == 0) {
-                    while (ld_acquire(&a.p.panel_ready[dir][K]) == 0) { }
-                }
-                __syncwarp();
-                Lse o = lse_empty();
-                if (i0 + r < N) {
-                    o.m = ldcg1(&a.p.pan_m[dir][i0 + r]);
-                    o.s = ldcg1(&a.p.pan_s[dir][i0 + r]);
-                }
-                lse_shift(o, dd_diff(ring_g[jrec0 % RB], ref)); // worker reference = g_{jrec0}
-                lse_merge(acc, o);
-            }
-            CT(4);
-            logA = acc.m + log(fabs(acc.s)); // -inf when there is no earlier column
-            if constexpr (SGN) sgnA = (acc.s < 0.0) ? -1.0 : 1.0;
-            double tau[32];
+            const double my_cc = cc_s[cur * 32 + r];
+            const double sh = sh_s[0];
+            float mx = -INFINITY; // log of the earlier-column sum, to within ln 2 per part
+            for (int k = 0; k <= L; ++k) mx = fmaxf(mx, (float)((pmK[k * 32 + r] + sh) + approx_log_abs(psK[k * 32 + r])));
+            float tau[32];
 #pragma unroll
-            for (int p = 0; p < 32; ++p) tau[p] = dg_s[p * 32 + lane];
-            double mx = logA, tcur = 0.0;
+            for (int p = 0; p < 32; ++p) tau[p] = dgf_s[cur * 1024 + p * 32 + lane];
+            float tcur = 0.f;
+            const float ccf = (float)my_cc;
 #pragma unroll
             for (int p = 0; p < 32; ++p) {
                 if (lane == 0) ts_s[p] = tcur;
-                mx = fmax(mx, tcur + tau[p]); // no effect once p > r
-                tcur = __shfl_sync(0xffffffffu, mx + my_cc, p);
+                mx = fmaxf(mx, tcur + tau[p]); // no effect once p > r
+                tcur = __shfl_sync(0xffffffffu, mx + ccf, p);
             }
-            G = mx;
-            tnext = G + my_cc; // the value lane r broadcast at step r: t_{r+1}
-            {
-                const double bb = tnext - G;
-                delta = (G - (tnext - bb)) + (my_cc - bb);
+            G = (double)mx;
+            const double tn = (double)(mx + ccf); // t_{r+1}, the value lane r broadcast at step r
+            G_s[r] = G;
+            dlt_s[r + 1] = (G - tn) + my_cc;      // t~_{r+1} - t_{r+1}, t~ = G + cc exactly
+            if (lane == 0) { ts_s[32] = tcur; dlt_s[0] = 0.0; }
+        } else if (is_io) {
+            // publish the previous block's columns to the workers (off the dependent path)
+            if (pend_ready) {
+                if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
+                pend_ready = 0;
             }
-            mxf_s[lane] = G;
-            CT(5);
-        }
-        __syncthreads();
-        for (int e = tid; e < 32 * 32; e += CH_THREADS) {
-            const int p = e >> 5, r = e & 31;
-            dg_s[e] = (p <= r) ? exp_fast((ts_s[p] + dg_s[e]) - mxf_s[r]) : 0.0;
-        }
-        __syncthreads();
-        CT(6);
-        if (warp == 0) {
-            const int r = lane;
-            double M[32];
+        } else if (is_helper && has_next) {
+            diag_tile(K + 1, ht, NHT);
+            // older column blocks C = K+1-q, q = 2..L -> rows of block K+1 (relative to Tref of block K);
+            // lane = column, a helper warp owns rows hidx, hidx + 11, hidx + 22
+            for (int q = 2; q <= L; ++q) {
+                const int C = K + 1 - q;
+                if (C < 0) {
+                    for (int rr = hidx; rr < 32; rr += NH)
+                        if (lane == 0) { pmN[q * 32 + rr] = -INFINITY; psN[q * 32 + rr] = 0.0; }
+                    continue;
+                }
+                const int slot = (C * 32 + lane) % RB;
+                Vec<D> pc;
 #pragma unroll
-            for (int p = 0; p < 32; ++p) M[p] = dg_s[p * 32 + lane];
-            double accl = sgnA * exp_fast(logA - G);
-            double zcur = SGN ? ring_sg[i0 % RB] : 1.0;
+                for (int k = 0; k < D; ++k) pc.v[k] = ring_sig[slot * D + k];
+                const double tc = dd_diff(ring_T[slot], Tref), zc = ring_Z[slot];
+                double t[3];
+                float mf[3];
 #pragma unroll
-            for (int p = 0; p < 32; ++p) {
-                accl = fma(M[p], zcur, accl); // M[p] = 0 once p > r
-                double zn = fma(accl, delta, accl);
-                if constexpr (SGN) zn *= a.sx;
-                zcur = __shfl_sync(0xffffffffu, zn, p);
-            }
-            CT(7);
-            // row r: R_r = ref + G_r + log|acc_r| ;  g_{r+1} = ref + t_{r+1} + log|Zhat_{r+1}|
-            const double la = log(fabs(accl));
-            const double lz = log(fabs(fma(accl, delta, accl)));
-            const double nsg = SGN ? ((accl < 0.0) ? -a.sx : a.sx) : 1.0;
-            if (r < nrows) {
-                if (!(fabs(accl) > 0.0) || !(fabs(la) < INFINITY) || !(fabs(G) < INFINITY))
-                    atomicOr(a.p.status, (accl == 0.0) ? ST_NODE : ST_NONFINITE);
-                const int jn = i0 + r + 1;
-                if (jn < N) {
-                    const double2 gn = dd_add_d(dd_add_d(ref, tnext), lz);
-                    ring_g[jn % RB] = gn;
-                    ring_sg[jn % RB] = nsg;
-                    g[jn] = gn;
-                    gs[jn] = nsg;
-                } else {
-                    a.p.rfin[dir] = dd_add_d(dd_add_d(ref, G), la);
-                    a.p.rsgn[dir] = (accl < 0.0) ? -1.0 : 1.0;
+                for (int k = 0; k < 3; ++k) {
+                    const int rr = min(hidx + NH * k, 31);
+                    Vec<D> pr;
+#pragma unroll
+                    for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + rr) * D + c];
+                    t[k] = tc - kk * dist2<D>(pr, pc);
+                    mf[k] = (float)t[k];
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) mf[k] = fmaxf(mf[k], __shfl_xor_sync(0xffffffffu, mf[k], o));
+                }
+                double sv[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) sv[k] = zc * exp_fast(t[k] - (double)mf[k]);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) sv[k] += __shfl_xor_sync(0xffffffffu, sv[k], o);
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int rr = hidx + NH * k;
+                    if (lane == 0 && rr < 32) { pmN[q * 32 + rr] = (double)mf[k]; psN[q * 32 + rr] = sv[k]; }
                 }
             }
-            __threadfence();
-            __syncwarp();
-            if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 33));
-            CT(8);
         }
+        CTA(1);
         __syncthreads();
+        CT(1);
+
+        // ================= P2
+        for (int e = tid; e < 1024; e += CH_THREADS) {
+            const int p = e >> 5, r = e & 31;
+            double m = (p <= r) ? exp_fast((((double)ts_s[p] - G_s[r]) + dgK[e]) + dlt_s[p]) : 0.0;
+            if constexpr (SGN) { if (p >= 1) m *= a.sx; }
+            dgK[e] = m;
+        }
+        if (tid < (L + 1) * 32) apart_s[tid] = psK[tid] * exp_fast((pmK[tid] + sh_s[0]) - G_s[tid & 31]);
+        CTA(2);
+        __syncthreads();
+        CT(2);
+
+        // ================= P3
+        if (warp == 0) {
+            double M[32];
+#pragma unroll
+            for (int p = 0; p < 32; ++p) M[p] = dgK[p * 32 + lane];
+            double acc = 0.0;
+            for (int k = 0; k <= L; ++k) acc += apart_s[k * 32 + lane];
+            double zc = zK[0];
+#pragma unroll
+            for (int p = 0; p < 32; ++p) {
+                acc = fma(M[p], zc, acc);              // M[p] = 0 once p > r
+                zc = __shfl_sync(0xffffffffu, acc, p); // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M)
+                if (lane == 0) zK[p + 1] = SGN ? a.sx * zc : zc;
+            }
+            accr = acc;
+            if (lane == 0) zN[0] = SGN ? a.sx * zc : zc;
+        } else if (has_next && (is_io || is_helper)) {
+            if (is_io) {
+                // the workers' panel for block K+1: columns < 32 (K+1-L), published relative to T_{32(K+1-L)}
+                const int jrec0n = 32 * (K + 1 - L);
+                double m = -INFINITY, s = 0.0;
+                if (jrec0n > 0) {
+                    if (lane == 0) {
+                        while (ld_acquire(&a.p.panel_ready[dir][K + 1]) == 0) { }
+                    }
+                    __syncwarp();
+                    const int i = i0 + 32 + lane;
+                    if (i < N) {
+                        m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n % RB], Tref);
+                        s = ldcg1(&a.p.pan_s[dir][i]);
+                    }
+                }
+                pmN[lane] = m;
+                psN[lane] = s;
+                // coordinates of block K+2: issue the loads now, store them in P4
+                const int i = i0 + 64 + lane;
+#pragma unroll
+                for (int c = 0; c < D; ++c) { pre_rho.v[c] = 0.0; pre_sig.v[c] = 0.0; }
+                pre_cc = 0.0;
+                if (i < N) {
+                    pre_rho = ldvec<D>(rho, i);
+                    pre_sig = ldvec<D>(sig, i);
+                    if (i < N - 1) pre_cc = cc[i];
+                }
+            } else {
+                // block K's columns -> rows of block K+1: everything but the factor Zhat
+                Vec<D> pc;
+#pragma unroll
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + lane) % RB) * D + c];
+                const double tc = (double)ts_s[lane], dc = dlt_s[lane];
+                float mf[3];
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    const int rr = min(hidx + NH * k, 31);
+                    Vec<D> pr;
+#pragma unroll
+                    for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + rr) * D + c];
+                    uE[k] = (tc - kk * dist2<D>(pr, pc)) + dc;
+                    mf[k] = (float)uE[k];
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) mf[k] = fmaxf(mf[k], __shfl_xor_sync(0xffffffffu, mf[k], o));
+                }
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    uM[k] = (double)mf[k];
+                    uE[k] = exp_fast(uE[k] - uM[k]);
+                }
+            }
+        }
+        CTA(3);
+        __syncthreads();
+        CT(3);
+
+        // ================= P4
+        if (warp == 0) {
+            const int r = lane, jn = i0 + r + 1;
+            if (r < nrows) {
+                if (!(fabs(accr) > 0.0) || !(fabs(accr) < INFINITY)) atomicOr(a.p.status, (accr == 0.0) ? ST_NODE : ST_NONFINITE);
+                if (jn < N) {
+                    ring_T[jn % RB] = dd_add_d(dd_add_d(Tref, (double)ts_s[r + 1]), dlt_s[r + 1]);
+                    ring_Z[jn % RB] = zK[r + 1];
+                } else {
+                    a.p.rfin[dir] = dd_add_d(dd_add_d(Tref, G), log(fabs(accr)));
+                    a.p.rsgn[dir] = (accr < 0.0) ? -1.0 : 1.0;
+                }
+            }
+            if (lane == 0) sh_s[0] = -((double)ts_s[32] + dlt_s[32]);
+        } else if (is_io) {
+            const int jn = i0 + lane + 1;
+            pend_j = (jn < N) ? jn : -1;
+            pend_T = dd_add_d(dd_add_d(Tref, (double)ts_s[lane + 1]), dlt_s[lane + 1]);
+            pend_Z = zK[lane + 1];
+            pend_ready = 1;
+            if (has_next) { // block K+2 (zeros beyond N)
+#pragma unroll
+                for (int c = 0; c < D; ++c) {
+                    rho_s[(cur * 32 + lane) * D + c] = pre_rho.v[c];
+                    ring_sig[((i0 + 64 + lane) % RB) * D + c] = pre_sig.v[c];
+                }
+                cc_s[cur * 32 + lane] = pre_cc;
+            }
+        } else if (is_helper && has_next) {
+            const double zl = zK[lane];
+            double sv[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) sv[k] = uE[k] * zl;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) sv[k] += __shfl_xor_sync(0xffffffffu, sv[k], o);
+            }
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const int rr = hidx + NH * k;
+                if (lane == 0 && rr < 32) { pmN[32 + rr] = uM[k]; psN[32 + rr] = sv[k]; }
+            }
+        }
+        CTA(4);
+        __syncthreads();
+        CT(4);
+    }
+#ifdef PIMD_CHAIN_TIMING
+    if (tid == 0) g_chain_gt[dir * 4 + 1] = gtimer();
+#endif
+    if (warp == CH_WARPS - 1 && pend_ready) {
+        if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) st_release(&a.p.cols_ready[dir], N);
     }
 }
 
@@ -558,7 +744,7 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             {
                 const int j = 32 * J + lane;
                 st_g[lane] = ldcg2(&g[j]);
-                if constexpr (SGN) st_sg[lane] = ldcg1(&gs[j]);
+                st_sg[lane] = ldcg1(&gs[j]);
                 Vec<D> pc = ldvec<D>(sig, j);
 #pragma unroll
                 for (int c = 0; c < D; ++c) st_sig[lane * D + c] = pc.v[c];
@@ -585,9 +771,7 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 }
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    double e = exp_fast(tau[k] - acc.m);
-                    if constexpr (SGN) e *= st_sg[c0 + k];
-                    acc.s += e;
+                    acc.s = fma(exp_fast(tau[k] - acc.m), st_sg[c0 + k], acc.s);
                 }
             }
             __syncwarp();
@@ -666,7 +850,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) sc.v[c] = 0.0;
         if (j < N) {
             gj = gd[j];
-            if constexpr (SGN) sj = p.gs[dir][j];
+            sj = p.gs[dir][j];
             sc = ldvec<D>(p.sig[dir], j);
         }
         sg_g[threadIdx.x] = gj;
@@ -679,8 +863,8 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
     const Vec<D> pr = ldvec<D>(p.rho[dir], i);
     // A = g^{other}[N-1-i] - R_N as dd, rounded once per element after adding g^{dir}[j]
     const double2 A = dd_sub(go[N - 1 - i], p.rfin[0]);
-    double osg = 1.0;
-    if constexpr (SGN) osg = p.gs[1 - dir][N - 1 - i] * p.rsgn[0];
+    double osg = p.gs[1 - dir][N - 1 - i];
+    if constexpr (SGN) osg *= p.rsgn[0];
     const int ncol = min(FP_TB, i - j0 + 1); // columns j0 .. min(j0+127, i)
     double sw = 0.0, swc = 0.0;
     Vec<D> sws;
@@ -693,8 +877,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
         const double2 gj = sg_g[k];
         const double kr2 = kk * dist2<D>(pr, pc);
-        double w = exp_fast(((A.x + gj.x) + (A.y + gj.y)) - kr2);
-        if constexpr (SGN) w *= sg_s[k];
+        const double w = exp_fast(((A.x + gj.x) + (A.y + gj.y)) - kr2) * sg_s[k];
         sw += w;
         swc = fma(w, kr2, swc);
 #pragma unroll
@@ -727,8 +910,7 @@ __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, double xi, Ex
         auto pn = [&](int m) -> double { // Pr[m -> m+1], 0 <= m <= N-2
             const double2 A = dd_sub(p.g[1][N - 1 - m], R);
             const double2 B = p.g[0][m + 1];
-            double w = exp_fast(((A.x + B.x) + (A.y + B.y)) - p.cnext[m]);
-            if constexpr (SGN) w *= p.gs[1][N - 1 - m] * p.gs[0][m + 1] * rs;
+            const double w = exp_fast(((A.x + B.x) + (A.y + B.y)) - p.cnext[m]) * (p.gs[1][N - 1 - m] * p.gs[0][m + 1] * rs);
             return 1.0 - xi * (double)(m + 1) * w;
         };
         const double pl = (l < N - 1) ? pn(l) : 0.0;
