@@ -249,10 +249,10 @@ def run_ours(args, w):
     fp64_peak = binding.probe_fp64_peak()
     pairs = w.P * w.N * (w.N - 1) / 2.0 if w.g != 0.0 else 0.0
     kern = {k: {"ms_avg": (ms / n if n else None), "launches": n} for k, (ms, n) in prof.items() if n}
-    bead_ms = kern.get("bead", {}).get("ms_avg")
+    bead_ms = kern.get("pair", {}).get("ms_avg")
     if pairs and bead_ms:
         ach = pairs * FLOP_PER_PAIR / (bead_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "k_bead (spring + trap + pair forces)", "achieved": ach, "peak": fp64_peak,
+        roofline = {"bound": "alu", "kernel": "k_pair (pair forces, Newton's third law)", "achieved": ach, "peak": fp64_peak,
                     "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": None,
                     "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
                                    "1.965 GHz x 2 = 37.2 TFLOP/s)",

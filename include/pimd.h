@@ -126,7 +126,7 @@ uint64_t pimd_launch_count(pimd_t h);
  * events on the stream it is launched on.  pimd_get_profile() synchronises, adds up the elapsed
  * times per slot since the previous call (milliseconds, and launch counts), returns them in the
  * HOST arrays ms_host / count_host (PIMD_PROF_NSLOTS entries each; either may be NULL) and resets. */
-#define PIMD_PROF_BEAD 0      /* spring + trap + pair forces (steps 1, 2) */
+#define PIMD_PROF_BEAD 0      /* spring + trap forces (step 1) */
 #define PIMD_PROF_PREP 1      /* closing springs, E_int, recursion inputs (step 3) */
 #define PIMD_PROF_CHAIN 2     /* forward + backward recursions (steps 4, 5) */
 #define PIMD_PROF_FORCEPASS 3 /* connection probabilities and their sums (step 6) */
@@ -134,7 +134,8 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_FINALIZE 5  /* V_B, sign, <E_c> */
 #define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
 #define PIMD_PROF_COMBINE 7   /* force output */
-#define PIMD_PROF_NSLOTS 8
+#define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
+#define PIMD_PROF_NSLOTS 9
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 

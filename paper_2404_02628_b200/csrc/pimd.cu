@@ -197,18 +197,25 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
 {
     const dim3 grid((h->N + BEAD_TB - 1) / BEAD_TB, h->P), block(BEAD_TB);
     const double om2P = h->omega * h->omega / h->P, is2 = 1.0 / (h->s * h->s);
-    const double coef = 2.0 * h->g * is2 / h->P;
-    const bool pair = h->g != 0.0;
-#define LB(PAIR, EST) \
-    k_bead<D, PAIR, EST, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, coef, h->g, h->est, h->hist, nbins, rmax)
     {
+        // spring + trap forces (and the trap energy / histogram on estimator calls): F is written here
         ProfScope ps(h, PIMD_PROF_BEAD, st);
-        if (pair && est) LB(true, true);
-        else if (pair) LB(true, false);
-        else if (est) LB(false, true);
-        else LB(false, false);
+        if (est) k_bead<D, false, true, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, 0.0, h->g, h->est, h->hist, nbins, rmax);
+        else k_bead<D, false, false, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, 0.0, h->g, h->est, h->hist, nbins, rmax);
     }
-#undef LB
+    CU(cudaGetLastError());
+    if (h->g != 0.0) {
+        // pair forces, added to F (Newton's third law, one Gaussian per unordered pair)
+        const int NT = (h->N + 31) / 32;
+        const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
+        const int nchunk = (hmax + PAIR_CH - 1) / PAIR_CH;
+        const long long tasks = (long long)NT * (nchunk + 1);
+        const dim3 pgrid((unsigned)((tasks + PAIR_WARPS - 1) / PAIR_WARPS), h->P);
+        const double coef = 2.0 * h->g / (h->s * h->P);
+        ProfScope ps(h, PIMD_PROF_PAIR, st);
+        if (est) k_pair<D, true><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, 1.0 / h->s, coef, h->g, h->est);
+        else k_pair<D, false><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, 1.0 / h->s, coef, h->g, h->est);
+    }
     CU(cudaGetLastError());
     return PIMD_OK;
 }

@@ -1091,6 +1091,158 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
     out[idx] = f;
 }
 
+// ==========================================================================================
+// Step 2 of the hot path: pair forces of one bead slice with Newton's third law,
+//   F_l^j += (1/P) sum_{i != l} (2g/s^2) e^{-|r_l^j - r_i^j|^2/s^2} (r_l^j - r_i^j)      (Eq. 18)
+// Particles are cut into tiles of 32.  Every unordered pair of tiles (I, J) is visited once through
+// the cyclic scheme J = (I + m) mod NT, m = 1..H (H = (NT-1)/2; for even NT the last offset NT/2 is
+// taken by I < NT/2 only).  A warp task owns row tile I and PAIR_CH consecutive offsets m; lane t
+// keeps particle i = 32 I + t and its force in registers.  Two column tiles are in flight at a time
+// (two independent exp chains per lane).  At step k lane t meets column (t + k) mod 32 of each:
+// positions come from shared memory (conflict free), the column's force accumulator travels from
+// lane to lane (one shuffle rotation per step), so each Gaussian is evaluated once and used for both
+// partners.  Tile results are added to F with FP64 atomics (F already holds the spring/trap forces).
+// The last task of a row does the 32 x 32 diagonal tile the plain way.
+// Coordinates are pre-scaled by 1/s so that the exponent is -|dx'|^2; padding particles sit at
+// +-1e150 and give exactly 0.
+// grid (ceil(tasks/PAIR_WARPS), P), block PAIR_WARPS * 32; tasks = NT (nchunk + 1).
+// ==========================================================================================
+constexpr int PAIR_WARPS = 8;
+constexpr int PAIR_CH = 8;
+
+template <int D> PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, Vec<D> &fi, Vec<D> &fj, double &se, double &sea,
+                                         bool est)
+{
+    Vec<D> dl;
+#pragma unroll
+    for (int c = 0; c < D; ++c) dl.v[c] = ri.v[c] - sj[c];
+    double r2 = dl.v[0] * dl.v[0];
+#pragma unroll
+    for (int c = 1; c < D; ++c) r2 = fma(dl.v[c], dl.v[c], r2);
+    const double e = exp_fast(-r2);
+#pragma unroll
+    for (int c = 0; c < D; ++c) {
+        fi.v[c] = fma(e, dl.v[c], fi.v[c]);
+        fj.v[c] = fma(-e, dl.v[c], fj.v[c]);
+    }
+    if (est) {
+        se += e;
+        sea = fma(-e, r2, sea);
+    }
+}
+
+template <int D, bool EST>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restrict__ x, double *__restrict__ F, int N, int NT,
+                                                         int nchunk, double inv_s, double coef /* 2 g / (s P) */, double g,
+                                                         EstAccum *est)
+{
+    __shared__ double tiles[PAIR_WARPS][2][32 * D];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int task = blockIdx.x * PAIR_WARPS + warp;
+    if (task >= NT * (nchunk + 1)) return; // warp-uniform; no block-wide barrier below
+    const int I = task / (nchunk + 1), c = task - I * (nchunk + 1);
+    const size_t sl = (size_t)blockIdx.y * N * D;
+    const double *xs = x + sl;
+    double *Fs = F + sl;
+    double *tA = tiles[warp][0], *tB = tiles[warp][1];
+
+    const int i = I * 32 + lane;
+    const bool vi = i < N;
+    Vec<D> ri, fi;
+#pragma unroll
+    for (int k = 0; k < D; ++k) { ri.v[k] = 1e150; fi.v[k] = 0.0; }
+    if (vi) {
+        ri = ldvec<D>(xs, i);
+#pragma unroll
+        for (int k = 0; k < D; ++k) ri.v[k] *= inv_s;
+    }
+    double se = 0.0, sea = 0.0;
+
+    auto stage = [&](double *dst, int J) { // J < 0: an all-padding tile
+        const int jx = J * 32 + lane;
+        Vec<D> p;
+#pragma unroll
+        for (int k = 0; k < D; ++k) p.v[k] = -1e150;
+        if (J >= 0 && jx < N) {
+            p = ldvec<D>(xs, jx);
+#pragma unroll
+            for (int k = 0; k < D; ++k) p.v[k] *= inv_s;
+        }
+#pragma unroll
+        for (int k = 0; k < D; ++k) dst[lane * D + k] = p.v[k];
+    };
+    auto flush = [&](int J, int col, const Vec<D> &f) {
+        const int jx = J * 32 + col;
+        if (J >= 0 && jx < N) {
+#pragma unroll
+            for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)jx * D + k], coef * f.v[k]);
+        }
+    };
+
+    if (c == nchunk) {
+        // diagonal tile: ordered pairs, the self term has dl = 0
+        __syncwarp();
+        stage(tA, I);
+        __syncwarp();
+        Vec<D> dummy;
+#pragma unroll
+        for (int k = 0; k < D; ++k) dummy.v[k] = 0.0;
+#pragma unroll 4
+        for (int k = 0; k < 32; ++k) {
+            const int col = (lane + k) & 31;
+            pair_term<D>(ri, tA + col * D, fi, dummy, se, sea, EST);
+        }
+        if (EST) {
+            se = vi ? 0.5 * (se - 1.0) : 0.0;
+            sea = vi ? 0.5 * sea : 0.0;
+        }
+    } else {
+        const int H = (NT & 1) ? (NT - 1) / 2 : (NT / 2 - 1 + (I < NT / 2 ? 1 : 0));
+        const int m0 = 1 + c * PAIR_CH, m1 = min(m0 + PAIR_CH - 1, H);
+        for (int m = m0; m <= m1; m += 2) {
+            int JA = I + m, JB = (m + 1 <= m1) ? I + m + 1 : -1;
+            if (JA >= NT) JA -= NT;
+            if (JB >= NT) JB -= NT;
+            __syncwarp();
+            stage(tA, JA);
+            stage(tB, JB);
+            __syncwarp();
+            Vec<D> fA, fB;
+#pragma unroll
+            for (int k = 0; k < D; ++k) { fA.v[k] = 0.0; fB.v[k] = 0.0; }
+            const int nxt = (lane + 1) & 31;
+#pragma unroll 2
+            for (int k = 0; k < 32; ++k) {
+                const int col = (lane + k) & 31;
+                pair_term<D>(ri, tA + col * D, fi, fA, se, sea, EST);
+                pair_term<D>(ri, tB + col * D, fi, fB, se, sea, EST);
+                if (k < 31) {
+#pragma unroll
+                    for (int q = 0; q < D; ++q) {
+                        fA.v[q] = __shfl_sync(0xffffffffu, fA.v[q], nxt);
+                        fB.v[q] = __shfl_sync(0xffffffffu, fB.v[q], nxt);
+                    }
+                }
+            }
+            const int col = (lane + 31) & 31;
+            flush(JA, col, fA);
+            flush(JB, col, fB);
+        }
+    }
+    if (vi) {
+#pragma unroll
+        for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)i * D + k], coef * fi.v[k]);
+    }
+    if (EST) {
+        se = warp_sum(se);
+        sea = warp_sum(sea);
+        if (lane == 0) {
+            atomicAdd(&est->upair, g * se);
+            atomicAdd(&est->virpair, g * (se + sea));
+        }
+    }
+}
+
 __global__ void k_zero(double *p, size_t n)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
