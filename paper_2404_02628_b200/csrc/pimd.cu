@@ -208,13 +208,14 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         // pair forces, added to F (Newton's third law, one Gaussian per unordered pair)
         const int NT = (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
-        const int nchunk = (hmax + PAIR_CH - 1) / PAIR_CH;
+        const int nchunk = hmax > 0 ? (hmax + PAIR_CH / 2) / PAIR_CH + ((hmax + PAIR_CH / 2) / PAIR_CH == 0) : 0; // ~PAIR_CH offsets per task
+        const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
         const long long tasks = (long long)NT * (nchunk + 1);
         const dim3 pgrid((unsigned)((tasks + PAIR_WARPS - 1) / PAIR_WARPS), h->P);
         const double coef = 2.0 * h->g / (h->s * h->P);
         ProfScope ps(h, PIMD_PROF_PAIR, st);
-        if (est) k_pair<D, true><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, 1.0 / h->s, coef, h->g, h->est);
-        else k_pair<D, false><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, 1.0 / h->s, coef, h->g, h->est);
+        if (est) k_pair<D, true><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, h->g, h->est);
+        else k_pair<D, false><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, h->g, h->est);
     }
     CU(cudaGetLastError());
     return PIMD_OK;

@@ -1096,7 +1096,7 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
 //   F_l^j += (1/P) sum_{i != l} (2g/s^2) e^{-|r_l^j - r_i^j|^2/s^2} (r_l^j - r_i^j)      (Eq. 18)
 // Particles are cut into tiles of 32.  Every unordered pair of tiles (I, J) is visited once through
 // the cyclic scheme J = (I + m) mod NT, m = 1..H (H = (NT-1)/2; for even NT the last offset NT/2 is
-// taken by I < NT/2 only).  A warp task owns row tile I and PAIR_CH consecutive offsets m; lane t
+// taken by I < NT/2 only).  A warp task owns row tile I and `ch` consecutive offsets m; lane t
 // keeps particle i = 32 I + t and its force in registers.  Two column tiles are in flight at a time
 // (two independent exp chains per lane).  At step k lane t meets column (t + k) mod 32 of each:
 // positions come from shared memory (conflict free), the column's force accumulator travels from
@@ -1110,8 +1110,8 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
 constexpr int PAIR_WARPS = 8;
 constexpr int PAIR_CH = 8;
 
-template <int D> PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, Vec<D> &fi, Vec<D> &fj, double &se, double &sea,
-                                         bool est)
+template <int D, bool EST>
+PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, Vec<D> &fi, Vec<D> &fj, double &se, double &sea)
 {
     Vec<D> dl;
 #pragma unroll
@@ -1119,25 +1119,48 @@ template <int D> PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, Vec
     double r2 = dl.v[0] * dl.v[0];
 #pragma unroll
     for (int c = 1; c < D; ++c) r2 = fma(dl.v[c], dl.v[c], r2);
-    const double e = exp_fast(-r2);
+    const double e = exp_tab(-r2, tab);
 #pragma unroll
     for (int c = 0; c < D; ++c) {
         fi.v[c] = fma(e, dl.v[c], fi.v[c]);
         fj.v[c] = fma(-e, dl.v[c], fj.v[c]);
     }
-    if (est) {
+    if constexpr (EST) {
         se += e;
         sea = fma(-e, r2, sea);
     }
 }
 
+// 32 steps of lane t against NJ column tiles held twice over in shared memory (tl = tile + t*D, so
+// that column (t + k) mod 32 is at the compile-time offset k*D); the column accumulators rotate.
+template <int D, int NJ, bool EST>
+PIMD_DEV void pair_sweep(const Vec<D> &ri, const double *tlA, const double *tlB, const double *tab, Vec<D> &fi, Vec<D> &fA,
+                         Vec<D> &fB, double &se, double &sea, int nxt)
+{
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        pair_term<D, EST>(ri, tlA + k * D, tab, fi, fA, se, sea);
+        if constexpr (NJ == 2) pair_term<D, EST>(ri, tlB + k * D, tab, fi, fB, se, sea);
+        if (k < 31) {
+#pragma unroll
+            for (int q = 0; q < D; ++q) {
+                fA.v[q] = __shfl_sync(0xffffffffu, fA.v[q], nxt);
+                if constexpr (NJ == 2) fB.v[q] = __shfl_sync(0xffffffffu, fB.v[q], nxt);
+            }
+        }
+    }
+}
+
 template <int D, bool EST>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restrict__ x, double *__restrict__ F, int N, int NT,
-                                                         int nchunk, double inv_s, double coef /* 2 g / (s P) */, double g,
-                                                         EstAccum *est)
+                                                         int nchunk, int ch, double inv_s, double coef /* 2 g / (s P) */,
+                                                         double g, EstAccum *est)
 {
-    __shared__ double tiles[PAIR_WARPS][2][32 * D];
+    __shared__ double tiles[PAIR_WARPS][2][64 * D];
+    __shared__ double tab[32];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x < 32) tab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    __syncthreads();
     const int task = blockIdx.x * PAIR_WARPS + warp;
     if (task >= NT * (nchunk + 1)) return; // warp-uniform; no block-wide barrier below
     const int I = task / (nchunk + 1), c = task - I * (nchunk + 1);
@@ -1145,6 +1168,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
     const double *xs = x + sl;
     double *Fs = F + sl;
     double *tA = tiles[warp][0], *tB = tiles[warp][1];
+    const double *tlA = tA + lane * D, *tlB = tB + lane * D;
 
     const int i = I * 32 + lane;
     const bool vi = i < N;
@@ -1158,49 +1182,47 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
     }
     double se = 0.0, sea = 0.0;
 
-    auto stage = [&](double *dst, int J) { // J < 0: an all-padding tile
+    auto stage = [&](double *dst, int J) {
         const int jx = J * 32 + lane;
         Vec<D> p;
 #pragma unroll
         for (int k = 0; k < D; ++k) p.v[k] = -1e150;
-        if (J >= 0 && jx < N) {
+        if (jx < N) {
             p = ldvec<D>(xs, jx);
 #pragma unroll
             for (int k = 0; k < D; ++k) p.v[k] *= inv_s;
         }
 #pragma unroll
-        for (int k = 0; k < D; ++k) dst[lane * D + k] = p.v[k];
+        for (int k = 0; k < D; ++k) { dst[lane * D + k] = p.v[k]; dst[(lane + 32) * D + k] = p.v[k]; }
     };
     auto flush = [&](int J, int col, const Vec<D> &f) {
         const int jx = J * 32 + col;
-        if (J >= 0 && jx < N) {
+        if (jx < N) {
 #pragma unroll
             for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)jx * D + k], coef * f.v[k]);
         }
     };
+    const int nxt = (lane + 1) & 31, lastcol = (lane + 31) & 31;
 
     if (c == nchunk) {
         // diagonal tile: ordered pairs, the self term has dl = 0
-        __syncwarp();
         stage(tA, I);
         __syncwarp();
         Vec<D> dummy;
 #pragma unroll
         for (int k = 0; k < D; ++k) dummy.v[k] = 0.0;
-#pragma unroll 4
-        for (int k = 0; k < 32; ++k) {
-            const int col = (lane + k) & 31;
-            pair_term<D>(ri, tA + col * D, fi, dummy, se, sea, EST);
-        }
-        if (EST) {
+#pragma unroll 8
+        for (int k = 0; k < 32; ++k) pair_term<D, EST>(ri, tlA + k * D, tab, fi, dummy, se, sea);
+        if constexpr (EST) {
             se = vi ? 0.5 * (se - 1.0) : 0.0;
             sea = vi ? 0.5 * sea : 0.0;
         }
     } else {
         const int H = (NT & 1) ? (NT - 1) / 2 : (NT / 2 - 1 + (I < NT / 2 ? 1 : 0));
-        const int m0 = 1 + c * PAIR_CH, m1 = min(m0 + PAIR_CH - 1, H);
-        for (int m = m0; m <= m1; m += 2) {
-            int JA = I + m, JB = (m + 1 <= m1) ? I + m + 1 : -1;
+        const int m0 = 1 + c * ch, m1 = min(m0 + ch - 1, H);
+        int m = m0;
+        for (; m + 1 <= m1; m += 2) {
+            int JA = I + m, JB = I + m + 1;
             if (JA >= NT) JA -= NT;
             if (JB >= NT) JB -= NT;
             __syncwarp();
@@ -1210,30 +1232,28 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
             Vec<D> fA, fB;
 #pragma unroll
             for (int k = 0; k < D; ++k) { fA.v[k] = 0.0; fB.v[k] = 0.0; }
-            const int nxt = (lane + 1) & 31;
-#pragma unroll 2
-            for (int k = 0; k < 32; ++k) {
-                const int col = (lane + k) & 31;
-                pair_term<D>(ri, tA + col * D, fi, fA, se, sea, EST);
-                pair_term<D>(ri, tB + col * D, fi, fB, se, sea, EST);
-                if (k < 31) {
+            pair_sweep<D, 2, EST>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
+            flush(JA, lastcol, fA);
+            flush(JB, lastcol, fB);
+        }
+        if (m <= m1) {
+            int JA = I + m;
+            if (JA >= NT) JA -= NT;
+            __syncwarp();
+            stage(tA, JA);
+            __syncwarp();
+            Vec<D> fA, fB;
 #pragma unroll
-                    for (int q = 0; q < D; ++q) {
-                        fA.v[q] = __shfl_sync(0xffffffffu, fA.v[q], nxt);
-                        fB.v[q] = __shfl_sync(0xffffffffu, fB.v[q], nxt);
-                    }
-                }
-            }
-            const int col = (lane + 31) & 31;
-            flush(JA, col, fA);
-            flush(JB, col, fB);
+            for (int k = 0; k < D; ++k) { fA.v[k] = 0.0; fB.v[k] = 0.0; }
+            pair_sweep<D, 1, EST>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
+            flush(JA, lastcol, fA);
         }
     }
     if (vi) {
 #pragma unroll
         for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)i * D + k], coef * fi.v[k]);
     }
-    if (EST) {
+    if constexpr (EST) {
         se = warp_sum(se);
         sea = warp_sum(sea);
         if (lane == 0) {

@@ -44,6 +44,43 @@ PIMD_DEV double exp_fast(double x)
 }
 
 // ---------------------------------------------------------------------------------------------
+// exp(x) for x <= 0 (the Gaussian pair factor), table driven: x = j ln2/32 + r, |r| <= ln2/64,
+// exp(x) = 2^(j>>5) * 2^((j&31)/32) * P6(r); degree-6 Taylor remainder 3.5e-18.  11 FP64
+// instructions + one shared-memory lookup; max relative error ~3e-16.  0 for x < -708.
+// `tab` points to the 32 doubles 2^(i/32) in shared memory (copied from c_exp2_32).
+// ---------------------------------------------------------------------------------------------
+__constant__ double c_exp2_32[32] = {
+    1.0, 1.0218971486541166, 1.0442737824274138, 1.0671404006768237,
+    1.0905077326652577, 1.1143867425958924, 1.1387886347566916, 1.1637248587775775,
+    1.189207115002721, 1.215247359980469, 1.241857812073484, 1.2690509571917332,
+    1.2968395546510096, 1.3252366431597413, 1.3542555469368927, 1.383909881963832,
+    1.4142135623730951, 1.4451808069770467, 1.4768261459394993, 1.5091644275934228,
+    1.5422108254079407, 1.5759808451078865, 1.6104903319492543, 1.645755478153965,
+    1.681792830507429, 1.718619298122478, 1.7562521603732995, 1.7947090750031072,
+    1.8340080864093424, 1.8741676341103, 1.9152065613971474, 1.9571441241754002};
+
+PIMD_DEV double exp_tab(double x, const double *tab)
+{
+    const double MAGIC = 6755399441055744.0; // 1.5 * 2^52
+    const double t = fma(x, 46.16624130844683, MAGIC); // 32 / ln 2
+    const int j = __double2loint(t);
+    const double kd = t - MAGIC;
+    double r = fma(kd, -0.02166084938653512, x);       // ln2/32, upper 33 bits (kd * hi is exact)
+    r = fma(kd, -5.9631716539705866e-12, r);
+    double p = 1.0 / 720.0;
+    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    const double v = tab[j & 31] * p;
+    const bool uf = (unsigned)__double2hiint(x) > 0xC0862000u; // x < -708 (or NaN): integer compare, off the FP64 pipe
+    const int hi = __double2hiint(v) + ((j >> 5) << 20);
+    return __hiloint2double(uf ? 0 : hi, uf ? 0 : __double2loint(v));
+}
+
+// ---------------------------------------------------------------------------------------------
 // double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
 // tables a[u], q[l] reach 1e5..1e7 in magnitude while only their DIFFERENCES enter an exp, so
 // they are carried as dd and differenced before rounding to double.
