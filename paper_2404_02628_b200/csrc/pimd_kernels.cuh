@@ -373,7 +373,7 @@ PIMD_DEV double approx_log_abs(double s)
 //       coordinates of block K+2.
 // ==========================================================================================
 template <int D, bool SGN>
-__device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
+__device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, const double *etab)
 {
     const int N = a.N, L = a.look;
     const ChainSmem<D> lay(L);
@@ -538,7 +538,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
                 }
                 double sv[3];
 #pragma unroll
-                for (int k = 0; k < 3; ++k) sv[k] = zc * exp_fast(t[k] - (double)mf[k]);
+                for (int k = 0; k < 3; ++k) sv[k] = zc * exp_tab(t[k] - (double)mf[k], etab);
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
@@ -558,11 +558,11 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
         // ================= P2
         for (int e = tid; e < 1024; e += CH_THREADS) {
             const int p = e >> 5, r = e & 31;
-            double m = (p <= r) ? exp_fast((((double)ts_s[p] - G_s[r]) + dgK[e]) + dlt_s[p]) : 0.0;
+            double m = (p <= r) ? exp_tab((((double)ts_s[p] - G_s[r]) + dgK[e]) + dlt_s[p], etab) : 0.0;
             if constexpr (SGN) { if (p >= 1) m *= a.sx; }
             dgK[e] = m;
         }
-        if (tid < (L + 1) * 32) apart_s[tid] = psK[tid] * exp_fast((pmK[tid] + sh_s[0]) - G_s[tid & 31]);
+        if (tid < (L + 1) * 32) apart_s[tid] = psK[tid] * exp_tab((pmK[tid] + sh_s[0]) - G_s[tid & 31], etab);
         CTA(2);
         __syncthreads();
         CT(2);
@@ -635,7 +635,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
 #pragma unroll
                 for (int k = 0; k < 3; ++k) {
                     uM[k] = (double)mf[k];
-                    uE[k] = exp_fast(uE[k] - uM[k]);
+                    uE[k] = exp_tab(uE[k] - uM[k], etab);
                 }
             }
         }
@@ -703,7 +703,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw)
 }
 
 template <int D, bool SGN>
-__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw)
+__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw, const double *etab)
 {
     const int N = a.N, LOOK = a.look;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -766,12 +766,12 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                     cm = fmax(cm, tau[k]);
                 }
                 if (cm > acc.m) {
-                    acc.s *= exp_fast(acc.m - cm);
+                    acc.s *= exp_tab(acc.m - cm, etab);
                     acc.m = cm;
                 }
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    acc.s = fma(exp_fast(tau[k] - acc.m), st_sg[c0 + k], acc.s);
+                    acc.s = fma(exp_tab(tau[k] - acc.m, etab), st_sg[c0 + k], acc.s);
                 }
             }
             __syncwarp();
@@ -813,9 +813,12 @@ template <int D, bool SGN>
 __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double etab[32]; // 2^(i/32) for exp_tab
+    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    __syncthreads();
     const int dir = blockIdx.y;
-    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw);
+    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw, etab);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab);
 }
 
 // ==========================================================================================
@@ -835,6 +838,8 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 {
     const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
     if (ct > rt) return;
+    __shared__ double etab[32];
+    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
     __shared__ double2 sg_g[FP_TB];
     __shared__ double sg_s[FP_TB];
     __shared__ double sg_sig[FP_TB * D];
@@ -877,7 +882,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
         const double2 gj = sg_g[k];
         const double kr2 = kk * dist2<D>(pr, pc);
-        const double w = exp_fast(((A.x + gj.x) + (A.y + gj.y)) - kr2) * sg_s[k];
+        const double w = exp_tab(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab) * sg_s[k];
         sw += w;
         swc = fma(w, kr2, swc);
 #pragma unroll
