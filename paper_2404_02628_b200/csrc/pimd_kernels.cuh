@@ -318,10 +318,10 @@ PIMD_DEV unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u
 // Shared-memory layout of the chain CTA (doubles); L = look.
 template <int D> struct ChainSmem {
     int RB;                   // ring capacity in columns: 32 (L + 2)
-    size_t ringT, ringZ, ringSig, rho, cc, dg, dgf, ts, dlt, Gs, zeta, partM, partS, apart, sh, total;
+    size_t ringT, ringZ, ringSig, rho, cc, dg, dgf, ts, dlt, Gs, zeta, partM, partS, partG, apart, sh, total;
     __host__ __device__ explicit ChainSmem(int L)
     {
-        RB = 32 * (L + 2);
+        RB = (L <= 2) ? 128 : 256;               // >= 32 (L + 2), a power of two
         size_t o = 0;
         ringT = o; o += 2 * (size_t)RB;          // double2 per column: the gauge T_j (double-double)
         ringZ = o; o += RB;                      // Zhat_j (signed)
@@ -336,6 +336,7 @@ template <int D> struct ChainSmem {
         zeta = o; o += 2 * 40;                   // Zhat of the block's columns, double buffered
         partM = o; o += 2 * (size_t)(L + 1) * 32;    // contributions of earlier columns to the NEXT block's rows:
         partS = o; o += 2 * (size_t)(L + 1) * 32; //   slot 0 panel (workers), 1 previous block, 2..L older blocks
+        partG = o; o += (size_t)(L + 1) * 32;    // float [2][(L+1)*32]: log|part| to within ln 2 (gauge start)
         apart = o; o += (size_t)(L + 1) * 32;
         sh = o; o += 8;
         total = o;
@@ -384,6 +385,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     double *ring_Z = sm + lay.ringZ, *ring_sig = sm + lay.ringSig, *rho_s = sm + lay.rho, *cc_s = sm + lay.cc;
     float *dgf_s = reinterpret_cast<float *>(sm + lay.dgf), *ts_s = reinterpret_cast<float *>(sm + lay.ts);
     double *dg_s = sm + lay.dg, *dlt_s = sm + lay.dlt, *G_s = sm + lay.Gs, *zeta_s = sm + lay.zeta;
+    float *part_g = reinterpret_cast<float *>(sm + lay.partG);
     double *part_m = sm + lay.partM, *part_s = sm + lay.partS, *apart_s = sm + lay.apart, *sh_s = sm + lay.sh;
 
     const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
@@ -414,7 +416,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
             for (int c = 0; c < D; ++c) {
                 rho_s[((B & 1) * 32 + e) * D + c] = pr.v[c];
-                ring_sig[((i % RB)) * D + c] = pc.v[c];
+                ring_sig[(i & (RB - 1)) * D + c] = pc.v[c];
             }
             cc_s[(B & 1) * 32 + e] = c0;
         }
@@ -424,7 +426,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         double *dgB = dg_s + (B & 1) * 1024;
         for (int e = t; e < 1024; e += nt) {
             const int p = e >> 5, r = e & 31;
-            const int slot = (B * 32 + p) % RB;
+            const int slot = (B * 32 + p) & (RB - 1);
             Vec<D> pr, pc;
 #pragma unroll
             for (int k = 0; k < D; ++k) { pr.v[k] = rho_s[((B & 1) * 32 + r) * D + k]; pc.v[k] = ring_sig[slot * D + k]; }
@@ -446,7 +448,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         zeta_s[0] = 1.0;
         sh_s[0] = 0.0;
     }
-    for (int e = tid; e < (L + 1) * 32; e += CH_THREADS) { part_m[e] = -INFINITY; part_s[e] = 0.0; }
+    for (int e = tid; e < (L + 1) * 32; e += CH_THREADS) { part_m[e] = -INFINITY; part_s[e] = 0.0; part_g[e] = -INFINITY; }
     __syncthreads();
     diag_tile(0, tid, CH_THREADS);
     __syncthreads();
@@ -463,11 +465,13 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         const int i0 = K * 32, cur = K & 1, nxt = cur ^ 1;
         const int nrows = min(32, N - i0);
         const bool has_next = (K + 1 < a.NB);
-        const double2 Tref = ring_T[i0 % RB];
+        const double2 Tref = ring_T[i0 & (RB - 1)];
         double *dgK = dg_s + cur * 1024;
         double *zK = zeta_s + cur * 40, *zN = zeta_s + nxt * 40;
         const double *pmK = part_m + cur * (L + 1) * 32, *psK = part_s + cur * (L + 1) * 32;
         double *pmN = part_m + nxt * (L + 1) * 32, *psN = part_s + nxt * (L + 1) * 32;
+        const float *pgK = part_g + cur * (L + 1) * 32;
+        float *pgN = part_g + nxt * (L + 1) * 32;
         double G = 0.0, accr = 0.0; // warp 0: row gauge and row sum of lane r
         double uE[3], uM[3];        // helpers: exp part and maximum of the rows they own in the next block
         CT(0);
@@ -478,7 +482,8 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             const double my_cc = cc_s[cur * 32 + r];
             const double sh = sh_s[0];
             float mx = -INFINITY; // log of the earlier-column sum, to within ln 2 per part
-            for (int k = 0; k <= L; ++k) mx = fmaxf(mx, (float)((pmK[k * 32 + r] + sh) + approx_log_abs(psK[k * 32 + r])));
+            for (int k = 0; k <= L; ++k) mx = fmaxf(mx, pgK[k * 32 + r]);
+            mx += (float)sh;
             float tau[32];
 #pragma unroll
             for (int p = 0; p < 32; ++p) tau[p] = dgf_s[cur * 1024 + p * 32 + lane];
@@ -512,10 +517,10 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 const int C = K + 1 - q;
                 if (C < 0) {
                     for (int rr = hidx; rr < 32; rr += NH)
-                        if (lane == 0) { pmN[q * 32 + rr] = -INFINITY; psN[q * 32 + rr] = 0.0; }
+                        if (lane == 0) { pmN[q * 32 + rr] = -INFINITY; psN[q * 32 + rr] = 0.0; pgN[q * 32 + rr] = -INFINITY; }
                     continue;
                 }
-                const int slot = (C * 32 + lane) % RB;
+                const int slot = (C * 32 + lane) & (RB - 1);
                 Vec<D> pc;
 #pragma unroll
                 for (int k = 0; k < D; ++k) pc.v[k] = ring_sig[slot * D + k];
@@ -547,7 +552,11 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
                 for (int k = 0; k < 3; ++k) {
                     const int rr = hidx + NH * k;
-                    if (lane == 0 && rr < 32) { pmN[q * 32 + rr] = (double)mf[k]; psN[q * 32 + rr] = sv[k]; }
+                    if (lane == 0 && rr < 32) {
+                        pmN[q * 32 + rr] = (double)mf[k];
+                        psN[q * 32 + rr] = sv[k];
+                        pgN[q * 32 + rr] = mf[k] + (float)approx_log_abs(sv[k]);
+                    }
                 }
             }
         }
@@ -556,13 +565,19 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         CT(1);
 
         // ================= P2
-        for (int e = tid; e < 1024; e += CH_THREADS) {
-            const int p = e >> 5, r = e & 31;
-            double m = (p <= r) ? exp_tab((((double)ts_s[p] - G_s[r]) + dgK[e]) + dlt_s[p], etab) : 0.0;
-            if constexpr (SGN) { if (p >= 1) m *= a.sx; }
-            dgK[e] = m;
+        {
+            // two independent exps per thread; tau = -inf above the diagonal gives exactly 0
+            const int r = tid & 31, p0 = tid >> 5, p1 = p0 + 16;
+            const double Gr = G_s[r];
+            const double a0 = (((double)ts_s[p0] - Gr) + dgK[tid]) + dlt_s[p0];
+            const double a1 = (((double)ts_s[p1] - Gr) + dgK[tid + 512]) + dlt_s[p1];
+            double m0 = exp_tab(a0, etab), m1 = exp_tab(a1, etab);
+            if constexpr (SGN) { if (p0 >= 1) m0 *= a.sx; m1 *= a.sx; }
+            dgK[tid] = m0;
+            dgK[tid + 512] = m1;
+            const int ai = tid - (CH_THREADS - (L + 1) * 32); // the last warps also scale the earlier-column parts
+            if (ai >= 0) apart_s[ai] = psK[ai] * exp_tab((pmK[ai] + sh_s[0]) - G_s[ai & 31], etab);
         }
-        if (tid < (L + 1) * 32) apart_s[tid] = psK[tid] * exp_tab((pmK[tid] + sh_s[0]) - G_s[tid & 31], etab);
         CTA(2);
         __syncthreads();
         CT(2);
@@ -595,12 +610,13 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                     __syncwarp();
                     const int i = i0 + 32 + lane;
                     if (i < N) {
-                        m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n % RB], Tref);
+                        m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n & (RB - 1)], Tref);
                         s = ldcg1(&a.p.pan_s[dir][i]);
                     }
                 }
                 pmN[lane] = m;
                 psN[lane] = s;
+                pgN[lane] = (float)(m + approx_log_abs(s));
                 // coordinates of block K+2: issue the loads now, store them in P4
                 const int i = i0 + 64 + lane;
 #pragma unroll
@@ -615,7 +631,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 // block K's columns -> rows of block K+1: everything but the factor Zhat
                 Vec<D> pc;
 #pragma unroll
-                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + lane) % RB) * D + c];
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + lane) & (RB - 1)) * D + c];
                 const double tc = (double)ts_s[lane], dc = dlt_s[lane];
                 float mf[3];
 #pragma unroll
@@ -649,8 +665,8 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             if (r < nrows) {
                 if (!(fabs(accr) > 0.0) || !(fabs(accr) < INFINITY)) atomicOr(a.p.status, (accr == 0.0) ? ST_NODE : ST_NONFINITE);
                 if (jn < N) {
-                    ring_T[jn % RB] = dd_add_d(dd_add_d(Tref, (double)ts_s[r + 1]), dlt_s[r + 1]);
-                    ring_Z[jn % RB] = zK[r + 1];
+                    ring_T[jn & (RB - 1)] = dd_add_d(dd_add_d(Tref, (double)ts_s[r + 1]), dlt_s[r + 1]);
+                    ring_Z[jn & (RB - 1)] = zK[r + 1];
                 } else {
                     a.p.rfin[dir] = dd_add_d(dd_add_d(Tref, G), log(fabs(accr)));
                     a.p.rsgn[dir] = (accr < 0.0) ? -1.0 : 1.0;
@@ -667,7 +683,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
                 for (int c = 0; c < D; ++c) {
                     rho_s[(cur * 32 + lane) * D + c] = pre_rho.v[c];
-                    ring_sig[((i0 + 64 + lane) % RB) * D + c] = pre_sig.v[c];
+                    ring_sig[((i0 + 64 + lane) & (RB - 1)) * D + c] = pre_sig.v[c];
                 }
                 cc_s[cur * 32 + lane] = pre_cc;
             }
@@ -684,7 +700,11 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
                 const int rr = hidx + NH * k;
-                if (lane == 0 && rr < 32) { pmN[32 + rr] = uM[k]; psN[32 + rr] = sv[k]; }
+                if (lane == 0 && rr < 32) {
+                    pmN[32 + rr] = uM[k];
+                    psN[32 + rr] = sv[k];
+                    pgN[32 + rr] = (float)(uM[k] + approx_log_abs(sv[k]));
+                }
             }
         }
         CTA(4);
