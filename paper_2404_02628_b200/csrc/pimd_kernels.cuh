@@ -437,7 +437,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     };
 
 #ifdef PIMD_CHAIN_TIMING
-    if (tid == 0) g_chain_gt[dir * 4 + 0] = gtimer();
+    if (tid == 0) { g_chain_gt[dir * 4 + 0] = gtimer(); g_chain_gt[dir * 4 + 2] = clock64(); }
 #endif
     // ---- prologue: blocks 0 and 1, first column, empty parts
     load_block(0, tid, CH_THREADS);
@@ -510,7 +510,6 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 pend_ready = 0;
             }
         } else if (is_helper && has_next) {
-            diag_tile(K + 1, ht, NHT);
             // older column blocks C = K+1-q, q = 2..L -> rows of block K+1 (relative to Tref of block K);
             // lane = column, a helper warp owns rows hidx, hidx + 11, hidx + 22
             for (int q = 2; q <= L; ++q) {
@@ -653,6 +652,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                     uM[k] = (double)mf[k];
                     uE[k] = exp_tab(uE[k] - uM[k], etab);
                 }
+                diag_tile(K + 1, ht, NHT); // tau tile of the next block (needs coordinates only)
             }
         }
         CTA(3);
@@ -712,7 +712,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         CT(4);
     }
 #ifdef PIMD_CHAIN_TIMING
-    if (tid == 0) g_chain_gt[dir * 4 + 1] = gtimer();
+    if (tid == 0) { g_chain_gt[dir * 4 + 1] = gtimer(); g_chain_gt[dir * 4 + 3] = clock64(); }
 #endif
     if (warp == CH_WARPS - 1 && pend_ready) {
         if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
