@@ -546,7 +546,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
-                    for (int k = 0; k < 3; ++k) sv[k] += __shfl_xor_sync(0xffffffffu, sv[k], o);
+                    for (int k = 0; k < 3; ++k) sv[k] += shfl_xor_d(sv[k], o);
                 }
 #pragma unroll
                 for (int k = 0; k < 3; ++k) {
@@ -592,7 +592,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
             for (int p = 0; p < 32; ++p) {
                 acc = fma(M[p], zc, acc);              // M[p] = 0 once p > r
-                zc = __shfl_sync(0xffffffffu, acc, p); // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M)
+                zc = shfl_bcast(acc, p);               // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M)
                 if (lane == 0) zK[p + 1] = SGN ? a.sx * zc : zc;
             }
             accr = acc;
@@ -695,7 +695,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
-                for (int k = 0; k < 3; ++k) sv[k] += __shfl_xor_sync(0xffffffffu, sv[k], o);
+                for (int k = 0; k < 3; ++k) sv[k] += shfl_xor_d(sv[k], o);
             }
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
@@ -1129,7 +1129,7 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
 // partners.  Tile results are added to F with FP64 atomics (F already holds the spring/trap forces).
 // The last task of a row does the 32 x 32 diagonal tile the plain way.
 // Coordinates are pre-scaled by 1/s so that the exponent is -|dx'|^2; padding particles sit at
-// +-1e150 and give exactly 0.
+// +-1e150 and give e^-708 ~ 3e-308 (their forces are never written).
 // grid (ceil(tasks/PAIR_WARPS), P), block PAIR_WARPS * 32; tasks = NT (nchunk + 1).
 // ==========================================================================================
 constexpr int PAIR_WARPS = 8;
@@ -1144,7 +1144,7 @@ PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, V
     double r2 = dl.v[0] * dl.v[0];
 #pragma unroll
     for (int c = 1; c < D; ++c) r2 = fma(dl.v[c], dl.v[c], r2);
-    const double e = exp_tab(-r2, tab);
+    const double e = exp_neg_tab64(r2, tab);
 #pragma unroll
     for (int c = 0; c < D; ++c) {
         fi.v[c] = fma(e, dl.v[c], fi.v[c]);
@@ -1152,7 +1152,7 @@ PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, V
     }
     if constexpr (EST) {
         se += e;
-        sea = fma(-e, r2, sea);
+        sea = fma(-e, fmin(r2, 708.0), sea); // padding pairs have r2 ~ 1e300 and e = e^-708, not 0
     }
 }
 
@@ -1169,8 +1169,8 @@ PIMD_DEV void pair_sweep(const Vec<D> &ri, const double *tlA, const double *tlB,
         if (k < 31) {
 #pragma unroll
             for (int q = 0; q < D; ++q) {
-                fA.v[q] = __shfl_sync(0xffffffffu, fA.v[q], nxt);
-                if constexpr (NJ == 2) fB.v[q] = __shfl_sync(0xffffffffu, fB.v[q], nxt);
+                fA.v[q] = shfl_bcast(fA.v[q], nxt);
+                if constexpr (NJ == 2) fB.v[q] = shfl_bcast(fB.v[q], nxt);
             }
         }
     }
@@ -1182,9 +1182,9 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
                                                          double g, EstAccum *est)
 {
     __shared__ double tiles[PAIR_WARPS][2][64 * D];
-    __shared__ double tab[32];
+    __shared__ double tab[64];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x < 32) tab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) tab[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int task = blockIdx.x * PAIR_WARPS + warp;
     if (task >= NT * (nchunk + 1)) return; // warp-uniform; no block-wide barrier below

@@ -81,6 +81,50 @@ PIMD_DEV double exp_tab(double x, const double *tab)
 }
 
 // ---------------------------------------------------------------------------------------------
+// exp(-r2) for r2 >= 0 (the Gaussian pair factor), 64-entry table: -r2 = j ln2/64 + r, |r| <= ln2/128,
+// exp(-r2) = 2^(j>>6) * 2^((j&63)/64) * P5(r); degree-5 Taylor remainder 3.5e-17.  9 FP64
+// instructions, no FP64 compare: r2 is clamped to 708 through its high word (integer min), so the
+// smallest value returned is e^-708 = 3e-308 instead of 0.  One FMA reduction: the rounding of ln2/64
+// costs a relative error r2 * 1.1e-16, i.e. at most 4e-17 of the largest term.
+// `tab` points to the 64 doubles 2^(i/64) in shared memory (copied from c_exp2_64).
+// ---------------------------------------------------------------------------------------------
+__constant__ double c_exp2_64[64] = {
+    1.0, 1.0108892860517005, 1.0218971486541166, 1.0330248790212284,
+    1.0442737824274138, 1.0556451783605572, 1.0671404006768237, 1.0787607977571199,
+    1.0905077326652577, 1.102382583307841, 1.1143867425958924, 1.1265216186082418,
+    1.1387886347566916, 1.1511892299529827, 1.1637248587775775, 1.1763969916502812,
+    1.189207115002721, 1.202156731452703, 1.215247359980469, 1.22848053610687,
+    1.241857812073484, 1.255380757024691, 1.2690509571917332, 1.2828700160787783,
+    1.2968395546510096, 1.3109612115247644, 1.3252366431597413, 1.339667524053303,
+    1.3542555469368927, 1.3690024229745905, 1.383909881963832, 1.3989796725383112,
+    1.4142135623730951, 1.42961333839197, 1.4451808069770467, 1.460917794180647,
+    1.4768261459394993, 1.4929077282912648, 1.5091644275934228, 1.5255981507445384,
+    1.5422108254079407, 1.559004400237837, 1.5759808451078865, 1.593142151342267,
+    1.6104903319492543, 1.6280274218573478, 1.645755478153965, 1.6636765803267364,
+    1.681792830507429, 1.7001063537185235, 1.718619298122478, 1.7373338352737062,
+    1.7562521603732995, 1.7753764925265212, 1.7947090750031072, 1.8142521755003989,
+    1.8340080864093424, 1.8539791250833855, 1.8741676341103, 1.8945759815869656,
+    1.9152065613971474, 1.9360617934922943, 1.9571441241754002, 1.978456026387951};
+
+PIMD_DEV double exp_neg_tab64(double r2, const double *tab)
+{
+    const double MAGIC = 6755399441055744.0; // 1.5 * 2^52
+    r2 = __hiloint2double(min(__double2hiint(r2), 0x40862000), __double2loint(r2)); // r2 <= 708 (r2 >= 0)
+    const double t = fma(r2, -92.33248261689366, MAGIC); // -64 / ln 2
+    const int j = __double2loint(t);
+    const double kd = t - MAGIC;
+    const double r = fma(kd, -0.010830424696249145, -r2); // ln2 / 64
+    double p = 1.0 / 120.0;
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    const double v = tab[j & 63] * p;
+    return __hiloint2double(__double2hiint(v) + (j >> 6) * 1048576, __double2loint(v));
+}
+
+// ---------------------------------------------------------------------------------------------
 // double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
 // tables a[u], q[l] reach 1e5..1e7 in magnitude while only their DIFFERENCES enter an exp, so
 // they are carried as dd and differenced before rounding to double.
@@ -146,17 +190,33 @@ PIMD_DEV void lse_shift(Lse &a, double delta) // re-reference: all t_i -> t_i + 
     if (a.m != -INFINITY) a.m += delta;
 }
 
+// broadcast of a double from lane `src`: the two halves are shuffled separately and reassembled in
+// place (a plain 64-bit __shfl_sync made ptxas swap the halves with three dependent XORs per use)
+PIMD_DEV double shfl_bcast(double v, int src)
+{
+    const int lo = __shfl_sync(0xffffffffu, __double2loint(v), src);
+    const int hi = __shfl_sync(0xffffffffu, __double2hiint(v), src);
+    return __hiloint2double(hi, lo);
+}
+
+PIMD_DEV double shfl_xor_d(double v, int mask)
+{
+    const int lo = __shfl_xor_sync(0xffffffffu, __double2loint(v), mask);
+    const int hi = __shfl_xor_sync(0xffffffffu, __double2hiint(v), mask);
+    return __hiloint2double(hi, lo);
+}
+
 // warp reductions (all 32 lanes participate)
 PIMD_DEV double warp_max(double v)
 {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, shfl_xor_d(v, o));
     return v;
 }
 PIMD_DEV double warp_sum(double v)
 {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    for (int o = 16; o > 0; o >>= 1) v += shfl_xor_d(v, o);
     return v;
 }
 
