@@ -138,6 +138,11 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_NSLOTS 9
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
+/* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM
+ * cycles per phase of its 32-row blocks: cycles_host[0] loop overhead; [2k-1] the dependent warp's own time
+ * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish); [2k] its wait at the
+ * barrier that ends phase k.  HOST out, 16 entries, accumulated since the previous call (then reset). */
+int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host);
 
 /* Measured FP64 FMA issue rate of the device (a register-resident DFMA loop over all SMs; used
  * as the ALU roofline denominator).  tflops is HOST out (2 flop per DFMA). */

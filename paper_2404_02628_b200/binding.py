@@ -44,6 +44,7 @@ _SYMBOLS = {
     "pimd_launch_count": (C.c_uint64, [C.c_void_p]),
     "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_get_profile": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_get_chain_phases": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_probe_fp64_peak": (C.c_int, [C.c_void_p, _dp]),
     "pimd_last_error": (C.c_char_p, [C.c_void_p]),
     "pimd_version": (C.c_char_p, []),
@@ -219,6 +220,12 @@ class Pimd:
         cnt = (C.c_uint64 * len(PROF_SLOTS))()
         self._check(self._lib.pimd_get_profile(self._h, ms, cnt))
         return {name: (float(ms[i]), int(cnt[i])) for i, name in enumerate(PROF_SLOTS)}
+
+    def get_chain_phases(self):
+        """16 cycle counters of the forward chain CTA (see pimd_get_chain_phases); reset on read."""
+        out = (C.c_uint64 * 16)()
+        self._check(self._lib.pimd_get_chain_phases(self._h, out))
+        return [int(v) for v in out]
 
     def launch_count(self):
         return int(self._lib.pimd_launch_count(self._h))

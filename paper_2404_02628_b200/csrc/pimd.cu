@@ -47,6 +47,7 @@ struct pimd_s {
     Scalars *scal;
     EstAccum *est;
     int *status;
+    unsigned long long *phase; // chain phase clock (profiling)
     // pinned host mirrors
     Scalars *h_scal;
     EstAccum *h_est;
@@ -149,6 +150,7 @@ size_t carve(pimd_t h, unsigned char *base)
     h->ex.tpart = (double *)take((size_t)h->nprep * 2 * 8);
     h->ex.rfin = (double2 *)take(2 * 16);
     h->ex.rsgn = (double *)take(2 * 8);
+    h->phase = (unsigned long long *)take(16 * 8);
     h->status = (int *)take(4 * 4);
     h->ex.status = h->status;
     h->ecpart = (double *)take((size_t)h->nasm * 8);
@@ -244,6 +246,7 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         ChainArgs a;
         a.N = h->N; a.NB = h->NB; a.look = h->look; a.nworkers = h->nworkers;
         a.kk = h->kk; a.sx = sgn ? -1.0 : 1.0; a.p = h->ex;
+        a.phase = h->profiling ? h->phase : nullptr;
         void *args[] = {&a};
         const dim3 grid(1 + h->nworkers, 2), block(CH_THREADS);
         const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
@@ -719,6 +722,17 @@ int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host)
         h->prof_ms[k] = 0.0;
         h->prof_n[k] = 0;
     }
+    return PIMD_OK;
+}
+
+int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host)
+{
+    if (!h || !cycles_host) return PIMD_EINVAL;
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(cycles_host, h->phase, 16 * 8, cudaMemcpyDeviceToHost, h->s0));
+    CU(cudaMemsetAsync(h->phase, 0, 16 * 8, h->s0));
+    CU(cudaStreamSynchronize(h->s0));
     return PIMD_OK;
 }
 

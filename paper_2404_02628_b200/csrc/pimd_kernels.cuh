@@ -293,32 +293,20 @@ __global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N
 // ==========================================================================================
 constexpr int CH_THREADS = 512;
 constexpr int CH_WARPS = CH_THREADS / 32;
-constexpr int CH_MAXLOOK = 6;
+constexpr int CH_MAXLOOK = 3; // (4 L + 1) * 32 part entries are scaled by one pass of 512 threads
 
 struct ChainArgs {
     int N, NB, look, nworkers;
     double kk, sx;
     ExchPtrs p;
+    unsigned long long *phase; // optional [16]: cycles of the forward chain CTA per phase (profiling), or NULL
 };
 
-
-#ifdef PIMD_CHAIN_TIMING
-__device__ long long g_chain_cyc[16];
-__device__ long long g_chain_arr[3][8];
-__device__ unsigned long long g_chain_gt[8];
-PIMD_DEV unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define CT(k) do { if (tid == 0 && dir == 0) { long long c__ = clock64(); g_chain_cyc[k] += c__ - tprev; } tprev = clock64(); } while (0)
-// arrival of warps 0, 1 and 15 at the barrier that ends phase k, measured from the phase start
-#define CTA(k) do { if (lane == 0 && dir == 0 && (warp <= 1 || warp == CH_WARPS - 1)) g_chain_arr[warp == 0 ? 0 : (warp == 1 ? 1 : 2)][k] += clock64() - tprev; } while (0)
-#else
-#define CT(k) do { } while (0)
-#define CTA(k) do { } while (0)
-#endif
 
 // Shared-memory layout of the chain CTA (doubles); L = look.
 template <int D> struct ChainSmem {
     int RB;                   // ring capacity in columns: 32 (L + 2)
-    size_t ringT, ringZ, ringSig, rho, cc, dg, dgf, ts, dlt, Gs, zeta, partM, partS, partG, apart, sh, total;
+    size_t ringT, ringZ, ringSig, rho, cc, dg, dgf, ue, ts, dlt, Gs, zeta, partM, partS, partG, apart, sh, total;
     __host__ __device__ explicit ChainSmem(int L)
     {
         RB = (L <= 2) ? 128 : 256;               // >= 32 (L + 2), a power of two
@@ -329,15 +317,16 @@ template <int D> struct ChainSmem {
         rho = o; o += 2 * 32 * D;                // rows of blocks K, K+1 (double buffered)
         cc = o; o += 2 * 32;
         dg = o; o += 2 * 32 * 32;                // diagonal tiles of blocks K, K+1: tau, then M
+        ue = o; o += 32 * 32;                    // exp part of block K's columns against the rows of block K+1
         dgf = o; o += 2 * 32 * 32 / 2;           // the same tau tiles as float (max-plus pass)
         ts = o; o += 20;                         // column gauges t_0..t_32 of the block (relative to Tref_K), float
         dlt = o; o += 40;                        // dlt[p] = t~_p - t_p (rounding remainder of the gauge)
         Gs = o; o += 32;                         // row gauges G_r
         zeta = o; o += 2 * 40;                   // Zhat of the block's columns, double buffered
-        partM = o; o += 2 * (size_t)(L + 1) * 32;    // contributions of earlier columns to the NEXT block's rows:
-        partS = o; o += 2 * (size_t)(L + 1) * 32; //   slot 0 panel (workers), 1 previous block, 2..L older blocks
-        partG = o; o += (size_t)(L + 1) * 32;    // float [2][(L+1)*32]: log|part| to within ln 2 (gauge start)
-        apart = o; o += (size_t)(L + 1) * 32;
+        partM = o; o += 2 * (size_t)(4 * L + 1) * 32;    // contributions of earlier columns to the NEXT block's rows:
+        partS = o; o += 2 * (size_t)(4 * L + 1) * 32; //   slot 0 panel (workers), then two half tiles per column block
+        partG = o; o += (size_t)(4 * L + 1) * 32;    // float [2][(L+1)*32]: log|part| to within ln 2 (gauge start)
+        apart = o; o += (size_t)(4 * L + 1) * 32;
         sh = o; o += 8;
         total = o;
     }
@@ -363,20 +352,24 @@ PIMD_DEV double approx_log_abs(double s)
 // The chain CTA.  Columns carry g_j = T_j + log|Zhat_j| as a
 // double-double gauge T_j and a linear, signed, O(1)-ranged factor Zhat_j; no log or exp sits on
 // the dependent path.  Per block K of 32 rows (rows and columns i0 = 32 K .. i0 + 31):
-//   P1  warp 0: max-plus ("tropical") pass in FP32 -> column gauges t_p, row gauges G_r.
-//       helpers (warps 1..15): diagonal tau tile of block K+1; contributions of the column blocks
-//       K+1-q, q = 2..L, to the rows of block K+1.
-//   P2  all: M[p][r] = exp(t~_p + tau[p][r] - G_r) <= 1;  Ahat parts = s exp(m - G_r).
+//   P1  warp 0: max-plus ("tropical") pass in FP32 -> column gauges t_p, row gauges G_r.  The io warp
+//       publishes the previous block's columns to the workers and fetches their panel for block K+1.
+//   P2  all: M[p][r] = exp(t~_p + tau[p][r] - G_r) <= 1;  Ahat parts = s exp(m - G_r); the exp part of
+//       the contribution of block K's columns to the rows of block K+1 (T known, Zhat not yet), and the
+//       complete contributions of the column blocks K+1-q, q = 2..L.
 //   P3  warp 0: linear pass  acc_r = Ahat_r + sum_p M[p][r] Zhat_p,  Zhat_{r+1} = sx acc_r.
-//       helpers: exp part of the contribution of block K's columns to the rows of block K+1;
-//       one helper warp fetches the workers' panel for block K+1.
-//   P4  all: finish that contribution (needs Zhat), publish T, Zhat (ring + global), load the
-//       coordinates of block K+2.
+//   P4  all: finish block K's contribution (needs Zhat), publish T, Zhat to the ring, tau tile of
+//       block K+1, coordinates of block K+2.
+// Nothing but warp 0 (and a few global accesses of the io warp) runs during P1 and P3: shuffles share
+// the SM's load/store pipe, and helper traffic placed beside the passes delayed them one for one.
 // ==========================================================================================
 template <int D, bool SGN>
 __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, const double *etab)
 {
-    const int N = a.N, L = a.look;
+    int N = a.N, L = a.look;
+    // keep the two in registers: re-reading kernel parameters from the constant bank inside the block loop
+    // was measured to stall the dependent warp for hundreds of cycles
+    asm volatile("" : "+r"(N), "+r"(L));
     const ChainSmem<D> lay(L);
     const int RB = lay.RB;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -384,6 +377,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     double2 *ring_T = reinterpret_cast<double2 *>(sm + lay.ringT);
     double *ring_Z = sm + lay.ringZ, *ring_sig = sm + lay.ringSig, *rho_s = sm + lay.rho, *cc_s = sm + lay.cc;
     float *dgf_s = reinterpret_cast<float *>(sm + lay.dgf), *ts_s = reinterpret_cast<float *>(sm + lay.ts);
+    double *ue_s = sm + lay.ue;
     double *dg_s = sm + lay.dg, *dlt_s = sm + lay.dlt, *G_s = sm + lay.Gs, *zeta_s = sm + lay.zeta;
     float *part_g = reinterpret_cast<float *>(sm + lay.partG);
     double *part_m = sm + lay.partM, *part_s = sm + lay.partS, *apart_s = sm + lay.apart, *sh_s = sm + lay.sh;
@@ -392,13 +386,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     double2 *g = a.p.g[dir];
     double *gs = a.p.gs[dir];
     const double kk = a.kk;
-    // Helper warps: every warp that does not share warp 0's scheduler partition (warp % 4 != 0), so that
-    // the two dependent passes of warp 0 do not queue behind the helpers' FP64 work; the last warp
-    // talks to global memory (publishes columns, fetches the workers' panel and the next coordinates).
-    constexpr int NH = 11, NHT = NH * 32;
-    const bool is_io = (warp == CH_WARPS - 1);
-    const bool is_helper = (warp & 3) != 0 && !is_io;
-    const int hidx = warp - 1 - (warp >> 2), ht = hidx * 32 + lane;
+    const bool is_io = (warp == CH_WARPS - 1); // the warp that talks to global memory
 
     // coordinates and cc of block B -> shared (rows: rho_s[B&1], columns: ring_sig); zero padding
     auto load_block = [&](int B, int t, int nt) {
@@ -436,9 +424,6 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         }
     };
 
-#ifdef PIMD_CHAIN_TIMING
-    if (tid == 0) { g_chain_gt[dir * 4 + 0] = gtimer(); g_chain_gt[dir * 4 + 2] = clock64(); }
-#endif
     // ---- prologue: blocks 0 and 1, first column, empty parts
     load_block(0, tid, CH_THREADS);
     load_block(1, tid, CH_THREADS);
@@ -448,60 +433,134 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         zeta_s[0] = 1.0;
         sh_s[0] = 0.0;
     }
-    for (int e = tid; e < (L + 1) * 32; e += CH_THREADS) { part_m[e] = -INFINITY; part_s[e] = 0.0; part_g[e] = -INFINITY; }
+    for (int e = tid; e < (4 * L + 1) * 32; e += CH_THREADS) { part_m[e] = -INFINITY; part_s[e] = 0.0; part_g[e] = -INFINITY; }
     __syncthreads();
     diag_tile(0, tid, CH_THREADS);
     __syncthreads();
-#ifdef PIMD_CHAIN_TIMING
-    long long tprev = clock64();
-#endif
-    double2 pend_T = make_double2(0.0, 0.0); // warp 15: columns computed in the previous block, to publish
+    double2 pend_T = make_double2(0.0, 0.0); // io warp: columns computed in the previous block, to publish
     double pend_Z = 0.0;
     int pend_j = -1, pend_ready = 0;
-    Vec<D> pre_rho, pre_sig; // warp 15: coordinates of block K+2 in flight
+    Vec<D> pre_rho, pre_sig; // io warp: coordinates of block K+2 in flight
     double pre_cc = 0.0;
+    int panel_done = 0;      // io warp: the workers' panel of block K+1 has been fetched
+    int bad = 0;             // warp 0: status bits of its rows
+    double2 fin_T = make_double2(0.0, 0.0);
+    double fin_G = 0.0, fin_acc = 1.0;
+    const int NP = 4 * L + 1; // parts of the earlier-column sum of a row: panel, then four quarter tiles per block
 
-    for (int K = 0; K < a.NB; ++K) {
+    // Shuffles, shared-memory loads and stores all go through one pipe per SM (measured: 16 warps doing
+    // warp reductions at once take ~4 cycles per shuffle).  The two dependent passes of warp 0 are chains of
+    // shuffles, so whatever runs beside them must be register arithmetic with very few shared accesses:
+    // tiles are computed with lane = row and a column loop (broadcast loads, no shuffles), two warps
+    // per tile, each leaving a partial (max, sum) per row.
+
+    // 8 columns [colbase, colbase+8) of a complete column block against row `pr`: partial log-domain sum
+    auto part_tile = [&](const Vec<D> &pr, int colbase, const double2 &Tref_, float &mf, double &sv) {
+        double t[8];
+        mf = -INFINITY;
+#pragma unroll
+        for (int p = 0; p < 8; ++p) {
+            const int slot = (colbase + p) & (RB - 1);
+            Vec<D> pc;
+#pragma unroll
+            for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
+            t[p] = dd_diff(ring_T[slot], Tref_) - kk * dist2<D>(pr, pc);
+            mf = fmaxf(mf, (float)t[p]);
+        }
+        const double m = (double)mf;
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int p = 0; p < 8; p += 2) {
+            s0 = fma(ring_Z[(colbase + p) & (RB - 1)], exp_tab(t[p] - m, etab), s0);
+            s1 = fma(ring_Z[(colbase + p + 1) & (RB - 1)], exp_tab(t[p + 1] - m, etab), s1);
+        }
+        sv = s0 + s1;
+    };
+
+    // optional phase clock of the forward chain CTA: slot 2k-1 = warp 0's own time in phase k, slot 2k = its
+    // wait at the barrier that ends phase k, slot 0 = loop overhead
+    __shared__ long long ph_s[16];
+    const bool tim = a.phase != nullptr && dir == 0 && tid == 0;
+    if (tid < 16) ph_s[tid] = 0;
+    long long tprev = clock64();
+#define PH(k) do { if (tim) { const long long c__ = clock64(); ph_s[k] += c__ - tprev; tprev = c__; } } while (0)
+    int NBk = a.NB;
+    asm volatile("" : "+r"(NBk));
+    for (int K = 0; K < NBk; ++K) {
+        PH(0);
         const int i0 = K * 32, cur = K & 1, nxt = cur ^ 1;
-        const int nrows = min(32, N - i0);
-        const bool has_next = (K + 1 < a.NB);
+        int nrows = min(32, N - i0);
+        asm volatile("" : "+r"(nrows)); // no re-derivation from the constant bank later on
+        const bool has_next = (K + 1 < NBk);
         const double2 Tref = ring_T[i0 & (RB - 1)];
         double *dgK = dg_s + cur * 1024;
         double *zK = zeta_s + cur * 40, *zN = zeta_s + nxt * 40;
-        const double *pmK = part_m + cur * (L + 1) * 32, *psK = part_s + cur * (L + 1) * 32;
-        double *pmN = part_m + nxt * (L + 1) * 32, *psN = part_s + nxt * (L + 1) * 32;
-        const float *pgK = part_g + cur * (L + 1) * 32;
-        float *pgN = part_g + nxt * (L + 1) * 32;
+        const double *pmK = part_m + cur * NP * 32, *psK = part_s + cur * NP * 32;
+        double *pmN = part_m + nxt * NP * 32, *psN = part_s + nxt * NP * 32;
+        const float *pgK = part_g + cur * NP * 32;
+        float *pgN = part_g + nxt * NP * 32;
         double G = 0.0, accr = 0.0; // warp 0: row gauge and row sum of lane r
-        double uE[3], uM[3];        // helpers: exp part and maximum of the rows they own in the next block
-        CT(0);
+        float uMf = -INFINITY;
 
-        // ================= P1
+        // fetch the workers' panel of block K+1 (columns < 32 (K+1-L), relative to T_{32(K+1-L)})
+        auto fetch_panel = [&](bool wait) {
+            const int jrec0n = 32 * (K + 1 - L);
+            double m = -INFINITY, s = 0.0;
+            if (jrec0n > 0) {
+                int ready = 0;
+                if (lane == 0) {
+                    ready = ld_acquire(&a.p.panel_ready[dir][K + 1]);
+                    while (wait && ready == 0) ready = ld_acquire(&a.p.panel_ready[dir][K + 1]);
+                }
+                ready = __shfl_sync(0xffffffffu, ready, 0);
+                if (!ready) return;
+                const int i = i0 + 32 + lane;
+                if (i < N) {
+                    m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n & (RB - 1)], Tref);
+                    s = ldcg1(&a.p.pan_s[dir][i]);
+                }
+            }
+            pmN[lane] = m;
+            psN[lane] = s;
+            pgN[lane] = (float)(m + approx_log_abs(s));
+            panel_done = 1;
+        };
+
+        // ================= P1: warp 0 max-plus pass.  Beside it: io warp publishes block K-1 and tries the
+        // panel; warps 1, 2 the older column blocks against the rows of block K+1; warps 3..6 the tau
+        // tile of block K+1
         if (warp == 0) {
             const int r = lane;
             const double my_cc = cc_s[cur * 32 + r];
             const double sh = sh_s[0];
             float mx = -INFINITY; // log of the earlier-column sum, to within ln 2 per part
-            for (int k = 0; k <= L; ++k) mx = fmaxf(mx, pgK[k * 32 + r]);
+            {
+                float v[9];
+#pragma unroll
+                for (int k = 0; k < 9; ++k) v[k] = (k < NP) ? pgK[k * 32 + r] : -INFINITY;
+                mx = fmaxf(fmaxf(fmaxf(fmaxf(v[0], v[1]), fmaxf(v[2], v[3])), fmaxf(fmaxf(v[4], v[5]), fmaxf(v[6], v[7]))), v[8]);
+                for (int k = 9; k < NP; ++k) mx = fmaxf(mx, pgK[k * 32 + r]);
+            }
             mx += (float)sh;
+            // fully unrolled: a rolled loop costs ~20 more cycles per step (branch + divergence check)
             float tau[32];
 #pragma unroll
             for (int p = 0; p < 32; ++p) tau[p] = dgf_s[cur * 1024 + p * 32 + lane];
-            float tcur = 0.f;
+            float tcur = 0.f, tmine = 0.f; // tmine: t_lane, kept in a register (no store inside the chain)
             const float ccf = (float)my_cc;
 #pragma unroll
             for (int p = 0; p < 32; ++p) {
-                if (lane == 0) ts_s[p] = tcur;
                 mx = fmaxf(mx, tcur + tau[p]); // no effect once p > r
                 tcur = __shfl_sync(0xffffffffu, mx + ccf, p);
+                if (lane == p + 1) tmine = tcur;
             }
             G = (double)mx;
             const double tn = (double)(mx + ccf); // t_{r+1}, the value lane r broadcast at step r
             G_s[r] = G;
             dlt_s[r + 1] = (G - tn) + my_cc;      // t~_{r+1} - t_{r+1}, t~ = G + cc exactly
+            ts_s[lane] = tmine;
             if (lane == 0) { ts_s[32] = tcur; dlt_s[0] = 0.0; }
         } else if (is_io) {
-            // publish the previous block's columns to the workers (off the dependent path)
             if (pend_ready) {
                 if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
                 __threadfence();
@@ -509,61 +568,43 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
                 pend_ready = 0;
             }
-        } else if (is_helper && has_next) {
-            // older column blocks C = K+1-q, q = 2..L -> rows of block K+1 (relative to Tref of block K);
-            // lane = column, a helper warp owns rows hidx, hidx + 11, hidx + 22
+            panel_done = 0;
+            if (has_next) fetch_panel(false);
+        } else if (has_next && warp <= 4) {
+            Vec<D> pr;
+#pragma unroll
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + lane) * D + c];
             for (int q = 2; q <= L; ++q) {
-                const int C = K + 1 - q;
-                if (C < 0) {
-                    for (int rr = hidx; rr < 32; rr += NH)
-                        if (lane == 0) { pmN[q * 32 + rr] = -INFINITY; psN[q * 32 + rr] = 0.0; pgN[q * 32 + rr] = -INFINITY; }
-                    continue;
-                }
-                const int slot = (C * 32 + lane) & (RB - 1);
+                const int C = K + 1 - q, slotp = (4 * q - 4 + warp) * 32 + lane; // parts 5..8 for q = 2, ...
+                float mf = -INFINITY;
+                double sv = 0.0;
+                if (C >= 0) part_tile(pr, C * 32 + (warp - 1) * 8, Tref, mf, sv);
+                pmN[slotp] = (double)mf;
+                psN[slotp] = sv;
+                pgN[slotp] = mf + (float)approx_log_abs(sv);
+            }
+        } else if (has_next && warp <= 8) {
+            // tau tile of block K+1, lane = row, 8 columns per warp
+            double *dgB = dg_s + nxt * 1024;
+            Vec<D> pr;
+#pragma unroll
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + lane) * D + c];
+#pragma unroll
+            for (int pp = 0; pp < 8; ++pp) {
+                const int p = (warp - 5) * 8 + pp;
                 Vec<D> pc;
 #pragma unroll
-                for (int k = 0; k < D; ++k) pc.v[k] = ring_sig[slot * D + k];
-                const double tc = dd_diff(ring_T[slot], Tref), zc = ring_Z[slot];
-                double t[3];
-                float mf[3];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const int rr = min(hidx + NH * k, 31);
-                    Vec<D> pr;
-#pragma unroll
-                    for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + rr) * D + c];
-                    t[k] = tc - kk * dist2<D>(pr, pc);
-                    mf[k] = (float)t[k];
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) mf[k] = fmaxf(mf[k], __shfl_xor_sync(0xffffffffu, mf[k], o));
-                }
-                double sv[3];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) sv[k] = zc * exp_tab(t[k] - (double)mf[k], etab);
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) sv[k] += shfl_xor_d(sv[k], o);
-                }
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const int rr = hidx + NH * k;
-                    if (lane == 0 && rr < 32) {
-                        pmN[q * 32 + rr] = (double)mf[k];
-                        psN[q * 32 + rr] = sv[k];
-                        pgN[q * 32 + rr] = mf[k] + (float)approx_log_abs(sv[k]);
-                    }
-                }
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + 32 + p) & (RB - 1)) * D + c];
+                const double tv = (p <= lane) ? -kk * dist2<D>(pr, pc) : -INFINITY;
+                dgB[p * 32 + lane] = tv;
+                dgf_s[nxt * 1024 + p * 32 + lane] = (float)tv;
             }
         }
-        CTA(1);
+        PH(1);
         __syncthreads();
-        CT(1);
+        PH(2);
 
-        // ================= P2
+        // ================= P2 (all threads): M pass and the earlier-column parts under the row gauges
         {
             // two independent exps per thread; tau = -inf above the diagonal gives exactly 0
             const int r = tid & 31, p0 = tid >> 5, p1 = p0 + 16;
@@ -574,49 +615,40 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             if constexpr (SGN) { if (p0 >= 1) m0 *= a.sx; m1 *= a.sx; }
             dgK[tid] = m0;
             dgK[tid + 512] = m1;
-            const int ai = tid - (CH_THREADS - (L + 1) * 32); // the last warps also scale the earlier-column parts
+            const int ai = tid - (CH_THREADS - NP * 32); // the last warps also scale the earlier-column parts
             if (ai >= 0) apart_s[ai] = psK[ai] * exp_tab((pmK[ai] + sh_s[0]) - G_s[ai & 31], etab);
         }
-        CTA(2);
+        PH(3);
         __syncthreads();
-        CT(2);
+        PH(4);
 
-        // ================= P3
+        // ================= P3: warp 0 linear pass.  Beside it: io warp (panel if not ready in P1, loads of
+        // block K+2's coordinates); warps 1, 2 the exp part of block K's columns against the rows of block K+1
         if (warp == 0) {
             double M[32];
 #pragma unroll
             for (int p = 0; p < 32; ++p) M[p] = dgK[p * 32 + lane];
             double acc = 0.0;
-            for (int k = 0; k <= L; ++k) acc += apart_s[k * 32 + lane];
-            double zc = zK[0];
+            {
+                double v[9]; // independent loads first (a runtime-count loop serialises on the load latency)
+#pragma unroll
+                for (int k = 0; k < 9; ++k) v[k] = (k < NP) ? apart_s[k * 32 + lane] : 0.0;
+                acc = (((v[0] + v[1]) + (v[2] + v[3])) + ((v[4] + v[5]) + (v[6] + v[7]))) + v[8];
+                for (int k = 9; k < NP; ++k) acc += apart_s[k * 32 + lane];
+            }
+            double zc = zK[0], zmine = zc; // zmine: X^_{lane-1}, kept in a register
 #pragma unroll
             for (int p = 0; p < 32; ++p) {
-                acc = fma(M[p], zc, acc);              // M[p] = 0 once p > r
-                zc = shfl_bcast(acc, p);               // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M)
-                if (lane == 0) zK[p + 1] = SGN ? a.sx * zc : zc;
+                acc = fma(M[p], zc, acc);  // M[p][r] = 0 once p > r
+                zc = shfl_bcast(acc, p);   // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M)
+                if (lane == p + 1) zmine = zc;
             }
             accr = acc;
-            if (lane == 0) zN[0] = SGN ? a.sx * zc : zc;
-        } else if (has_next && (is_io || is_helper)) {
-            if (is_io) {
-                // the workers' panel for block K+1: columns < 32 (K+1-L), published relative to T_{32(K+1-L)}
-                const int jrec0n = 32 * (K + 1 - L);
-                double m = -INFINITY, s = 0.0;
-                if (jrec0n > 0) {
-                    if (lane == 0) {
-                        while (ld_acquire(&a.p.panel_ready[dir][K + 1]) == 0) { }
-                    }
-                    __syncwarp();
-                    const int i = i0 + 32 + lane;
-                    if (i < N) {
-                        m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n & (RB - 1)], Tref);
-                        s = ldcg1(&a.p.pan_s[dir][i]);
-                    }
-                }
-                pmN[lane] = m;
-                psN[lane] = s;
-                pgN[lane] = (float)(m + approx_log_abs(s));
-                // coordinates of block K+2: issue the loads now, store them in P4
+            if (lane >= 1) zK[lane] = SGN ? a.sx * zmine : zmine;
+            if (lane == 0) { zK[32] = SGN ? a.sx * zc : zc; zN[0] = SGN ? a.sx * zc : zc; }
+        } else if (is_io) {
+            if (has_next) {
+                if (!panel_done) fetch_panel(true);
                 const int i = i0 + 64 + lane;
 #pragma unroll
                 for (int c = 0; c < D; ++c) { pre_rho.v[c] = 0.0; pre_sig.v[c] = 0.0; }
@@ -626,51 +658,43 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                     pre_sig = ldvec<D>(sig, i);
                     if (i < N - 1) pre_cc = cc[i];
                 }
-            } else {
-                // block K's columns -> rows of block K+1: everything but the factor Zhat
+            }
+        } else if (has_next && warp <= 4) {
+            Vec<D> pr;
+#pragma unroll
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + lane) * D + c];
+            const int c0 = (warp - 1) * 8;
+            double u[8];
+#pragma unroll
+            for (int p = 0; p < 8; ++p) {
                 Vec<D> pc;
 #pragma unroll
-                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + lane) & (RB - 1)) * D + c];
-                const double tc = (double)ts_s[lane], dc = dlt_s[lane];
-                float mf[3];
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const int rr = min(hidx + NH * k, 31);
-                    Vec<D> pr;
-#pragma unroll
-                    for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(nxt * 32 + rr) * D + c];
-                    uE[k] = (tc - kk * dist2<D>(pr, pc)) + dc;
-                    mf[k] = (float)uE[k];
-                }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) mf[k] = fmaxf(mf[k], __shfl_xor_sync(0xffffffffu, mf[k], o));
-                }
-#pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    uM[k] = (double)mf[k];
-                    uE[k] = exp_tab(uE[k] - uM[k], etab);
-                }
-                diag_tile(K + 1, ht, NHT); // tau tile of the next block (needs coordinates only)
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((i0 + c0 + p) & (RB - 1)) * D + c];
+                u[p] = ((double)ts_s[c0 + p] - kk * dist2<D>(pr, pc)) + dlt_s[c0 + p];
+                uMf = fmaxf(uMf, (float)u[p]);
             }
+            const double m = (double)uMf;
+#pragma unroll
+            for (int p = 0; p < 8; ++p) ue_s[(c0 + p) * 32 + lane] = exp_tab(u[p] - m, etab);
         }
-        CTA(3);
+        PH(5);
         __syncthreads();
-        CT(3);
+        PH(6);
 
-        // ================= P4
+        // ================= P4: warps 1, 2 finish block K's contribution (needs Zhat); warp 0 publishes T and
+        // Zhat to the ring; io warp takes its copy for the workers and stores block K+2's coordinates
         if (warp == 0) {
-            const int r = lane, jn = i0 + r + 1;
-            if (r < nrows) {
-                if (!(fabs(accr) > 0.0) || !(fabs(accr) < INFINITY)) atomicOr(a.p.status, (accr == 0.0) ? ST_NODE : ST_NONFINITE);
-                if (jn < N) {
-                    ring_T[jn & (RB - 1)] = dd_add_d(dd_add_d(Tref, (double)ts_s[r + 1]), dlt_s[r + 1]);
-                    ring_Z[jn & (RB - 1)] = zK[r + 1];
-                } else {
-                    a.p.rfin[dir] = dd_add_d(dd_add_d(Tref, G), log(fabs(accr)));
-                    a.p.rsgn[dir] = (accr < 0.0) ? -1.0 : 1.0;
-                }
+            if (lane < nrows) { // status and the final row are dealt with once, after the loop
+                if (accr == 0.0) bad |= ST_NODE;
+                else if (!(fabs(accr) < INFINITY)) bad |= ST_NONFINITE;
+            }
+            if (!has_next) { fin_T = Tref; fin_G = G; fin_acc = accr; }
+        } else if (warp == 9) {
+            // T and Zhat of the columns this block produced -> ring
+            const int jn = i0 + lane + 1;
+            if (jn < N) {
+                ring_T[jn & (RB - 1)] = dd_add_d(dd_add_d(Tref, (double)ts_s[lane + 1]), dlt_s[lane + 1]);
+                ring_Z[jn & (RB - 1)] = zK[lane + 1];
             }
             if (lane == 0) sh_s[0] = -((double)ts_s[32] + dlt_s[32]);
         } else if (is_io) {
@@ -679,7 +703,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             pend_T = dd_add_d(dd_add_d(Tref, (double)ts_s[lane + 1]), dlt_s[lane + 1]);
             pend_Z = zK[lane + 1];
             pend_ready = 1;
-            if (has_next) { // block K+2 (zeros beyond N)
+            if (has_next) { // block K+2 (zeros beyond N): free buffers, first read in P1 of block K+1
 #pragma unroll
                 for (int c = 0; c < D; ++c) {
                     rho_s[(cur * 32 + lane) * D + c] = pre_rho.v[c];
@@ -687,34 +711,36 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 }
                 cc_s[cur * 32 + lane] = pre_cc;
             }
-        } else if (is_helper && has_next) {
-            const double zl = zK[lane];
-            double sv[3];
+        } else if (has_next && warp <= 4) {
+            const int c0 = (warp - 1) * 8;
+            double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) sv[k] = uE[k] * zl;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-                for (int k = 0; k < 3; ++k) sv[k] += shfl_xor_d(sv[k], o);
+            for (int p = 0; p < 8; p += 2) {
+                s0 = fma(ue_s[(c0 + p) * 32 + lane], zK[c0 + p], s0);
+                s1 = fma(ue_s[(c0 + p + 1) * 32 + lane], zK[c0 + p + 1], s1);
             }
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const int rr = hidx + NH * k;
-                if (lane == 0 && rr < 32) {
-                    pmN[32 + rr] = uM[k];
-                    psN[32 + rr] = sv[k];
-                    pgN[32 + rr] = (float)(uM[k] + approx_log_abs(sv[k]));
-                }
-            }
+            const double sv = s0 + s1, m = (double)uMf;
+            pmN[warp * 32 + lane] = m; // parts 1..4
+            psN[warp * 32 + lane] = sv;
+            pgN[warp * 32 + lane] = (float)(m + approx_log_abs(sv));
         }
-        CTA(4);
+        PH(7);
         __syncthreads();
-        CT(4);
+        PH(8);
     }
-#ifdef PIMD_CHAIN_TIMING
-    if (tid == 0) { g_chain_gt[dir * 4 + 1] = gtimer(); g_chain_gt[dir * 4 + 3] = clock64(); }
-#endif
-    if (warp == CH_WARPS - 1 && pend_ready) {
+#undef PH
+    if (tim) {
+        for (int k = 0; k < 16; ++k) a.phase[k] += (unsigned long long)ph_s[k];
+    }
+    if (warp == 0) {
+        // R_{N-1} = T + G + log|X^| of the last row, its sign, and the status of all rows
+        if (lane == (N - 1) % 32) {
+            a.p.rfin[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
+            a.p.rsgn[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
+        }
+        if (bad) atomicOr(a.p.status, bad);
+    }
+    if (is_io && pend_ready) {
         if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
         __threadfence();
         __syncwarp();
