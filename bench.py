@@ -27,6 +27,10 @@ UNIT = "steps/s"
 # algorithmic FP64 work of the pair kernel: 25 FP64 instructions per unordered bead pair at d = 2
 # (SURVEY.md 8(d)), counted as FMA-equivalents = 2 flop each
 FLOP_PER_PAIR = 50.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+# (profiles/r1_b_cfg3.md, profiles/r1_b_cfg5b.md); None where no capture of that workload exists
+NCU_TRAFFIC = {("cfg3", "pair"): 1704448 + 0, ("cfg3", "forcepass"): 290560 + 0,
+               ("cfg5b", "pair"): 5186048 + 0, ("cfg5b", "forcepass"): 1768960 + 0}
 
 
 def describe(w):
@@ -71,6 +75,40 @@ class ClockSampler:
         reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
         return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons, "samples": len(rows),
                 "power_w_max": max(float(r[2]) for r in rows)}
+
+
+def max_over_ranks(value, world, device="cuda"):
+    """MAX of a per-rank scalar over all ranks (the timing rule for every multi-GPU number) and the
+    whole-job rate helper: works with any initialised torch.distributed backend (NCCL on GPUs; gloo
+    in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank, seconds_per_rank, world, device="cuda"):
+    """Replicas: every rank does `units_per_rank`; value = all units / slowest rank's time."""
+    return world * units_per_rank / max_over_ranks(seconds_per_rank, world, device)
+
+
+def recursion_report(w, kern, phases, steps, clocks):
+    """Latency figures of the N-long chain (neither roofline binds it)."""
+    ch = kern.get("chain", {}).get("ms_avg")
+    nb = (w.N + 31) // 32
+    out = {"kernel": "k_chain (forward + backward recursion, one cooperative launch)", "bound": "latency",
+           "ms": ch, "ns_per_row": (ch * 1e6 / w.N if ch else None), "rows_per_block": 32}
+    if ch and sum(phases[:9]) > 0:
+        per = [c / float(steps * nb) for c in phases[:9]]
+        out["cycles_per_block"] = {"loop_overhead": per[0], "P1_maxplus_pass": per[1] + per[2], "P2_exponentials": per[3] + per[4],
+                                   "P3_linear_pass": per[5] + per[6], "P4_publish": per[7] + per[8], "sum": sum(per)}
+        out["floor_cycles_per_block"] = 32 * (41 + 38)
+        out["note"] = ("SM cycles of the forward chain CTA per 32-row block (clock64 inside the kernel, own time + barrier wait "
+                       "per phase); floor = 32 x (SHFL + FADD + FMNMX + FADD) + 32 x (SHFL + DFMA) from measured latencies")
+    return out
 
 
 def load_peaks():
@@ -203,10 +241,8 @@ def run_ours(args, w):
     launches = sim.launch_count() - l0
     prof = sim.get_profile()
     sim.set_profiling(False)
-    tmax = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    t_dev = float(tmax.item())
+    phases = sim.get_chain_phases()
+    t_dev = max_over_ranks(t_dev, world)
     value = world * args.steps / t_dev
 
     # the same K steps back to back with the state left in L2 (how an MD run actually executes)
@@ -234,10 +270,7 @@ def run_ours(args, w):
         sim.get_state_host(xh, vh)  # synchronises
     barrier()
     te = time.perf_counter() - te
-    temax = torch.tensor([te], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(temax, op=dist.ReduceOp.MAX)
-    e2e = world * ne2e / float(temax.item())
+    e2e = whole_job_rate(ne2e, te, world)
     nbytes = int(x0.nbytes + v0.nbytes)
 
     if rank != 0:
@@ -247,16 +280,29 @@ def run_ours(args, w):
 
     peaks, peak_src = load_peaks()
     fp64_peak = binding.probe_fp64_peak()
+    # the same kernels timed alone (exchange and bead parts serialised on one stream): the burst figure
+    sim.set_concurrency(False)
+    sim.set_profiling(True)
+    sim.get_profile()
+    sim.step(max(5, min(args.steps, 20)))
+    iso = {k: ms / n for k, (ms, n) in sim.get_profile().items() if n}
+    sim.set_profiling(False)
+    sim.set_concurrency(True)
     pairs = w.P * w.N * (w.N - 1) / 2.0 if w.g != 0.0 else 0.0
     kern = {k: {"ms_avg": (ms / n if n else None), "launches": n} for k, (ms, n) in prof.items() if n}
     bead_ms = kern.get("pair", {}).get("ms_avg")
     if pairs and bead_ms:
         ach = pairs * FLOP_PER_PAIR / (bead_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": "k_pair (pair forces, Newton's third law)", "achieved": ach, "peak": fp64_peak,
-                    "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": None,
+                    "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": NCU_TRAFFIC.get((w.name, "pair")),
+                    "traffic_note": "DRAM bytes per launch (ncu); the algorithmic inputs are L2-resident: %d B of positions" % (w.P * w.N * w.d * 8),
                     "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
                                    "1.965 GHz x 2 = 37.2 TFLOP/s)",
-                    "convention": "50 flop (25 FP64 instructions) per unordered bead pair, %d pairs per launch" % int(pairs)}
+                    "convention": "50 flop (25 FP64 instructions, SURVEY.md 8(d)) per unordered bead pair, %d pairs per launch; "
+                                  "the shipped kernel spends 17 FP64 instructions per pair (table-driven exp), so frac can "
+                                  "exceed the FP64 pipe utilisation ncu reports" % int(pairs),
+                    "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
+                    "alone": {"ms": iso.get("pair"), "frac": pairs * FLOP_PER_PAIR / (iso["pair"] * 1e-3) / 1e12 / fp64_peak}}
     else:
         # non-interacting workloads: the exchange passes dominate; they recompute the closing springs
         # instead of streaming an N x N matrix, so they are ALU bound too
@@ -264,9 +310,11 @@ def run_ours(args, w):
         elems = float(w.N) * (w.N + 1)  # two sweeps over the lower triangle
         ach = elems * 54.0 / (fp_ms * 1e-3) / 1e12 if fp_ms else None
         roofline = {"bound": "alu", "kernel": "k_forcepass (connection probabilities)", "achieved": ach, "peak": fp64_peak,
-                    "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": None,
+                    "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": NCU_TRAFFIC.get((w.name, "forcepass")),
                     "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak",
-                    "convention": "54 flop (27 FP64 instructions) per matrix element, N(N+1) elements per launch"}
+                    "convention": "54 flop (27 FP64 instructions) per matrix element, N(N+1) elements per launch",
+                    "alone": {"ms": iso.get("forcepass"),
+                              "frac": (elems * 54.0 / (iso["forcepass"] * 1e-3) / 1e12 / fp64_peak) if iso.get("forcepass") else None}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -282,6 +330,8 @@ def run_ours(args, w):
         "pair_forces_per_s": pairs * value,
         "steps_per_s_l2_resident": resident_sps * world,
         "kernels": kern,
+        "kernels_alone_ms": iso,
+        "recursion": recursion_report(w, kern, phases, args.steps, clocks),
         "roofline": roofline,
         "peaks": {"fp64_tflops_probe": fp64_peak, "hbm_gbs": peaks.get("hbm_gbs"), "source": peak_src},
     }

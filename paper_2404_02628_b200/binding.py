@@ -45,6 +45,7 @@ _SYMBOLS = {
     "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_get_profile": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_get_chain_phases": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_selftest_exp": (C.c_int, [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_size_t]),
     "pimd_probe_fp64_peak": (C.c_int, [C.c_void_p, _dp]),
     "pimd_last_error": (C.c_char_p, [C.c_void_p]),
     "pimd_version": (C.c_char_p, []),
@@ -239,6 +240,18 @@ def probe_fp64_peak(stream=None):
     if rc != OK:
         raise PimdError(rc, lib.pimd_last_error(None).decode())
     return out.value
+
+
+def selftest_exp(which, x_dev, stream=None):
+    """y = the device exponential `which` (see pimd_selftest_exp) applied to the CUDA float64 tensor x_dev."""
+    import torch
+
+    lib = load()
+    y = torch.empty_like(x_dev)
+    rc = lib.pimd_selftest_exp(C.c_void_p(stream or 0), int(which), _ptr(x_dev), _ptr(y), x_dev.numel())
+    if rc != OK:
+        raise PimdError(rc, lib.pimd_last_error(None).decode())
+    return y
 
 
 def version():

@@ -1320,6 +1320,20 @@ __global__ void k_zero(double *p, size_t n)
     if (i < n) p[i] = 0.0;
 }
 
+// the device exponentials evaluated element-wise (parity tests): which = 0 exp_fast(x), 1 exp_tab(x),
+// 2 exp_neg_tab64(x) = exp(-x), x >= 0
+__global__ void __launch_bounds__(256) k_exp_selftest(const double *__restrict__ x, double *__restrict__ y, size_t n, int which)
+{
+    __shared__ double t32[32], t64[64];
+    if (threadIdx.x < 32) t32[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) t64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __syncthreads();
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = x[i];
+    y[i] = which == 0 ? exp_fast(v) : (which == 1 ? exp_tab(v, t32) : exp_neg_tab64(v, t64));
+}
+
 // FP64 FMA issue-rate probe: 8 independent chains per thread, register resident.
 __global__ void __launch_bounds__(256) k_dfma_probe(double *out, int iters, double a, double b)
 {

@@ -167,3 +167,42 @@ def test_ten_steps_match_oracle(binding, oracle, thermostat):
     sim.close()
     assert relerr(xg.cpu().numpy(), xo) <= 1e-9
     assert relerr(vg.cpu().numpy(), vo) <= 1e-8
+
+
+def test_device_exponentials_match_libm(binding):
+    """The three hand-written exponentials of the hot kernels against numpy's exp (<= 4 ulp), incl. the tails."""
+    rng = np.random.default_rng(11)
+    x = np.concatenate([rng.uniform(-40.0, 0.0, 200000), rng.uniform(-700.0, -40.0, 50000), rng.uniform(0.0, 5.0, 20000),
+                        np.array([0.0, -1e-300, -0.5 * np.log(2.0), -707.9, -709.5, -1e5, -np.inf])])
+    xd = torch.from_numpy(x).cuda()
+    ref = np.exp(x)
+    for which in (0, 1):
+        y = binding.selftest_exp(which, xd).cpu().numpy()
+        live = x >= -708.0
+        assert np.max(np.abs(y[live] - ref[live]) / ref[live]) <= 1e-15
+        assert np.all(y[~live] == 0.0)
+    r2 = -x[x <= 0.0]
+    r2 = r2[np.isfinite(r2)]
+    y = binding.selftest_exp(2, torch.from_numpy(r2).cuda()).cpu().numpy()
+    ref2 = np.exp(-r2)
+    live = r2 <= 700.0
+    # one-FMA argument reduction: relative error grows like r2 * 1.1e-16 (DESIGN.md 5.2)
+    assert np.max(np.abs(y[live] - ref2[live]) / ref2[live] / (1.0 + r2[live])) <= 3e-16
+    assert np.all(y[~live] <= 1e-300) and np.all(y >= 0.0)
+
+
+def test_chain_phase_clock(binding):
+    w = wl.custom(300, 4, d=2, beta=3.0, g=0.0, xi=1.0, init="ring", sigma=2.0)
+    x, v = wl.make_state(w, 0)
+    sim = make(binding, w, thermostat=1)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    sim.step(2)
+    assert sum(sim.get_chain_phases()) == 0  # profiling off: the clock is not running
+    sim.set_profiling(True)
+    sim.step(3)
+    ph = sim.get_chain_phases()
+    sim.close()
+    assert len(ph) == 16 and all(c > 0 for c in ph[:9])
+    nb = (w.N + 31) // 32
+    per_block = sum(ph[:9]) / (3 * nb)
+    assert 1e3 < per_block < 1e5  # a 32-row block costs a few thousand SM cycles
