@@ -374,7 +374,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
-    ap.add_argument("--sweep", default="cfg2,cfg5_N2500,cfg5_N10000,cfg5b")
+    ap.add_argument("--sweep", default="cfg1,cfg2,cfg4,cfg5_N2500,cfg5_N10000,cfg5_N20000,cfg5_N40000,cfg5b")
     ap.add_argument("--sweep-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

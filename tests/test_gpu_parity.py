@@ -206,3 +206,97 @@ def test_chain_phase_clock(binding):
     nb = (w.N + 31) // 32
     per_block = sum(ph[:9]) / (3 * nb)
     assert 1e3 < per_block < 1e5  # a 32-row block costs a few thousand SM cycles
+
+
+# ------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (default look-ahead, workers, streams)
+# ------------------------------------------------------------------------------------------------------------
+def _forces_and_tables(binding, w, x):
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda())
+    f, vb, sg = sim.forces()
+    vf, vbw, pn = sim.get_tables()
+    F = f.cpu().numpy()
+    sim.close()
+    return F, vb, sg, vf, vbw, pn
+
+
+def test_full_size_n10000_against_oracle(binding, oracle):
+    """config 5 at N = 10000 (non-interacting): V_B and every force against the oracle, element by element."""
+    w = wl.WORKLOADS["cfg5_N10000"]
+    x, _ = wl.make_state(w, 0)
+    Fo, vbo, sgo = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
+    F, vb, sg = gpu_forces(binding, w, x)
+    assert sg == sgo == 1
+    assert abs(vb - vbo) <= RTOL * abs(vbo)
+    check_forces(F, Fo, RTOL)
+
+
+def test_full_size_identical_rings_closed_form(binding):
+    """All particles on the same ring: W_N = e^{-beta N E_ring} prod_{j<N}(1 + j xi) / N!  (DESIGN.md pins; exact
+    for any N and xi), so V_B = N E_ring - (1/beta) sum_j [log(1 + j xi) - log(j + 1)].  N = 10000 and 40000."""
+    for N, xi in ((10000, 1.0), (10000, 0.5), (40000, 1.0)):
+        P, d, beta = 16, 2, 3.0
+        rng = np.random.default_rng(5)
+        ring = rng.normal(0.0, 0.3, size=(P, 1, d))
+        x = np.ascontiguousarray(np.repeat(ring, N, axis=1))
+        w = wl.custom(N, P, d=d, beta=beta, g=0.0, xi=xi, init="iid")
+        ks = P / beta ** 2
+        diffs = np.diff(np.concatenate([ring[:, 0, :], ring[:1, 0, :]]), axis=0)
+        e_ring = 0.5 * ks * float(np.sum(diffs ** 2))
+        j = np.arange(N, dtype=np.float64)
+        vb_exact = N * e_ring - float(np.sum(np.log1p(j * xi) - np.log(j + 1.0))) / beta
+        F, vb, sg = gpu_forces(binding, w, x)
+        assert sg == 1
+        assert abs(vb - vb_exact) <= RTOL * abs(vb_exact)
+        # by symmetry every particle feels the force of one closed ring of its own beads plus the trap
+        xr = ring[:, 0, :]
+        f_ring = -ks * (2 * xr - np.roll(xr, 1, axis=0) - np.roll(xr, -1, axis=0)) - (w.omega ** 2 / P) * xr
+        ref = np.repeat(f_ring[:, None, :], N, axis=1)
+        assert relerr(F, ref) <= 1e-9
+
+
+@pytest.mark.parametrize("name", ["cfg5b", "cfg5_N40000"])
+def test_full_size_invariants(binding, name):
+    """Properties that hold at any size (no oracle run needed): forward = backward (Eq. 6 at n = N equals Eq. 11 at
+    u = 1), Pr[l -> l+1] in [0, 1] with Pr[N -> N+1] = 0, the exchange + spring forces sum to zero over all beads
+    (translation invariance), Newton's third law for the pair part, and Euler's theorem for the degree-2
+    homogeneous V_B."""
+    w = wl.WORKLOADS[name]
+    x, _ = wl.make_state(w, 0)
+    F, vb, sg, vf, vbw, pn = _forces_and_tables(binding, w, x)
+    assert sg == 1 and np.isfinite(vb)
+    assert abs(vf[w.N] - vb) <= 1e-9 * abs(vb)
+    assert abs(vbw[1] - vb) <= 1e-9 * abs(vb)          # V^{[1,N]} from the backward recursion
+    # Eq. 13 is 1 - (a ratio close to 1): its absolute rounding error is that of an exponent of size ~1e4 (R13)
+    assert pn[-1] == 0.0 and pn.min() >= -1e-10 and pn.max() <= 1.0 + 1e-10
+    # remove the trap force; what is left is translation invariant
+    Fint = F + (w.omega ** 2 / w.P) * x
+    scale = np.abs(Fint).sum()
+    assert np.all(np.abs(Fint.sum(axis=(0, 1))) <= 1e-11 * scale)
+    if w.g == 0.0:
+        # Euler: sum r . grad V_B = 2 V_spring-part; with g = 0, -sum r.F_int = 2 (V_B - (1/beta) log-term) is not closed
+        # form, but the virial identity -sum r . F_int = 2 <E_c> links it to the primitive estimator
+        sim = make(binding, w)
+        sim.set_state(torch.from_numpy(x).cuda())
+        ep, ev, _ = sim.estimators()
+        sim.close()
+        ec = w.P * w.d * w.N / (2.0 * w.beta) + 0.5 * (w.omega ** 2 / w.P) * float(np.sum(x * x)) - ep
+        assert abs(-float(np.sum(x * Fint)) - 2.0 * ec) <= 1e-9 * abs(2.0 * ec)
+
+
+def test_full_size_sampled_pair_forces(binding, oracle):
+    """cfg5b (N = 10000, g = 0.2): the external (trap + pair) force on sampled beads against the oracle's
+    one-bead routine, and the sampled total force minus it against a g = 0 evaluation."""
+    w = wl.WORKLOADS["cfg5b"]
+    x, _ = wl.make_state(w, 0)
+    F, vb, sg = gpu_forces(binding, w, x)
+    F0, vb0, _ = gpu_forces(binding, w.with_(g=0.0), x)
+    assert abs(vb - vb0) <= 1e-12 * abs(vb)  # V_B does not depend on the pair interaction
+    rng = np.random.default_rng(3)
+    fmax = np.max(np.abs(F - F0))
+    for _ in range(40):
+        j, l = int(rng.integers(w.P)), int(rng.integers(w.N))
+        fe = oracle.external_force_on(x, w.omega, w.g, w.s, j, l)
+        fe0 = oracle.external_force_on(x, w.omega, 0.0, w.s, j, l)
+        assert np.max(np.abs((F[j, l] - F0[j, l]) - (fe - fe0))) <= 1e-9 * fmax
