@@ -135,7 +135,8 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
 #define PIMD_PROF_COMBINE 7   /* force output */
 #define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
-#define PIMD_PROF_NSLOTS 9
+#define PIMD_PROF_CHAIN_FALLBACK 9 /* the max-plus recursion queued behind the stale-gauge one (returns at once if unused) */
+#define PIMD_PROF_NSLOTS 10
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM

@@ -33,7 +33,7 @@ struct pimd_s {
     // derived
     double ks, kk, lambda;
     size_t ndof, slice;
-    int NB, nprep, nasm, look, nworkers;
+    int NB, nprep, nasm, look, look_spec, nworkers;
     // streams
     cudaStream_t s0, s1;
     cudaEvent_t ev_fork, ev_join;
@@ -53,6 +53,9 @@ struct pimd_s {
     EstAccum *h_est;
     int *h_status;
     bool forces_valid;
+    bool gauge_valid; // g/gs hold the (T, Zhat) of a completed evaluation of nearby positions
+    bool use_spec;    // PIMD_NOSPEC=1 turns the stale-gauge kernel off
+    size_t spec_smem;
     int coop_max_blocks; // co-resident CTA limit of k_chain
     size_t chain_smem;
     uint64_t launches;
@@ -186,6 +189,9 @@ template <int D> int setup_chain_attr(pimd_t h)
     h->chain_smem = smem;
     CU(cudaFuncSetAttribute(k_chain<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CU(cudaFuncSetAttribute(k_chain<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    h->spec_smem = chain_spec_smem_bytes_host<D>();
+    CU(cudaFuncSetAttribute(k_chain_spec<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->spec_smem));
+    CU(cudaFuncSetAttribute(k_chain_spec<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->spec_smem));
     int nb = 0, dev = 0, sms = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_chain<D, true>, CH_THREADS, smem));
     CU(cudaGetDevice(&dev));
@@ -247,13 +253,32 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         a.N = h->N; a.NB = h->NB; a.look = h->look; a.nworkers = h->nworkers;
         a.kk = h->kk; a.sx = sgn ? -1.0 : 1.0; a.p = h->ex;
         a.phase = h->profiling ? h->phase : nullptr;
+        a.cond = 0;
+        const int look_spec = h->look_spec;
         void *args[] = {&a};
         const dim3 grid(1 + h->nworkers, 2), block(CH_THREADS);
         const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
-        {
+        if (h->gauge_valid && h->use_spec) {
+            // the previous evaluation's gauge is at hand: linear pass only; the max-plus kernel is queued
+            // behind it and returns at once unless the gauge turned out not to fit
+            const void *fs = sgn ? (const void *)k_chain_spec<D, true> : (const void *)k_chain_spec<D, false>;
+            a.look = look_spec; // the workers need one more block of head start when the chain runs this fast
+            {
+                ProfScope ps(h, PIMD_PROF_CHAIN, st);
+                CU(cudaLaunchCooperativeKernel(fs, grid, block, args, h->spec_smem, st));
+            }
+            a.look = h->look;
+            a.cond = 1;
+            a.phase = nullptr;
+            {
+                ProfScope ps(h, PIMD_PROF_CHAIN_FALLBACK, st);
+                CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
+            }
+        } else {
             ProfScope ps(h, PIMD_PROF_CHAIN, st);
             CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
         }
+        h->gauge_valid = true;
         const int NT = (h->N + FP_TB - 1) / FP_TB;
         const dim3 fgrid(NT, NT, 2);
         {
@@ -397,11 +422,14 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     h->nprep = (N + PREP_TB - 1) / PREP_TB;
     h->nasm = (N + ASM_TB - 1) / ASM_TB;
     h->look = 2;
+    h->look_spec = 2;
     if (const char *e = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
         const int v = std::atoi(e);
-        if (v >= 1 && v <= CH_MAXLOOK) h->look = v;
+        if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;
     }
     h->concurrent = true;
+    h->gauge_valid = false;
+    h->use_spec = !(std::getenv("PIMD_NOSPEC") && std::atoi(std::getenv("PIMD_NOSPEC")) != 0);
     h->prof_ev = new std::vector<cudaEvent_t>();
     h->prof_slot = new std::vector<int>();
     int rc = PIMD_OK;
@@ -418,7 +446,7 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
         // chain one SM keeps up with ~16 column tiles per block.
         const int want = h->NB - h->look - 1;
         int cap = h->coop_max_blocks / 2 - 1;
-        int need = (h->NB + 11) / 12;
+        int need = (h->NB + 7) / 8;
         if (const char *e = std::getenv("PIMD_WORKERS")) {
             const int v = std::atoi(e);
             if (v >= 1) need = v;
@@ -511,6 +539,7 @@ static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpy
     if (h->thermostat == PIMD_THERMOSTAT_NHC) CU(cudaMemsetAsync(h->nhc, 0, h->ndof * 8 * PIMD_NHC_LENGTH, h->s0));
     CU(cudaMemsetAsync(h->status, 0, 4 * sizeof(int), h->s0));
     h->forces_valid = false;
+    h->gauge_valid = false;
     return PIMD_OK;
 }
 

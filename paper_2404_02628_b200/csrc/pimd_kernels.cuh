@@ -9,6 +9,7 @@
 //   backward: rho_i = r_u^1, sig_j = r_l^P with u = N-1-i, l = N-1-j, g_j = q[l] - q[N]
 //   cc = beta C(l,l+1) - lambda - ln(l+1)   (the same array, read in opposite order).
 #pragma once
+#include <cooperative_groups.h>
 #include "pimd_math.cuh"
 
 namespace pimd {
@@ -260,6 +261,18 @@ __global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N
             p.acc[1][(size_t)l * (D + 2) + c] = 0.0;
         }
         if (l < NB) { p.panel_ready[0][l] = 0; p.panel_ready[1][l] = 0; }
+        // refresh the gauge the previous evaluation left behind: (T, Zhat) -> (T + k ln2, Zhat 2^-k) with
+        // |Zhat 2^-k| in [1, 2), so that T tracks the solution from step to step (k_chain_spec)
+#pragma unroll
+        for (int dir = 0; dir < 2; ++dir) {
+            const double z = p.gs[dir][l + 1];
+            const int ex = (__double2hiint(z) >> 20) & 0x7ff;
+            if (ex != 0 && ex != 0x7ff) {
+                const int k = ex - 1023;
+                p.g[dir][l + 1] = dd_add_d(p.g[dir][l + 1], (double)k * 0.6931471805599453);
+                p.gs[dir][l + 1] = scalbn(z, -k);
+            }
+        }
         if (l == 0) {
             p.g[0][0] = make_double2(-lambda, 0.0);
             p.g[1][0] = make_double2(0.0, 0.0);
@@ -268,6 +281,7 @@ __global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N
             p.cols_ready[0] = 1;
             p.cols_ready[1] = 1;
             *p.status = 0;
+            p.status[2] = 0;
         }
     }
     double s1 = block_sum<TB>(e_int, red);
@@ -299,6 +313,7 @@ struct ChainArgs {
     int N, NB, look, nworkers;
     double kk, sx;
     ExchPtrs p;
+    int cond;                  // 1: run only if status[2] is set (fallback behind k_chain_spec)
     unsigned long long *phase; // optional [16]: cycles of the forward chain CTA per phase (profiling), or NULL
 };
 
@@ -563,7 +578,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
         } else if (is_io) {
             if (pend_ready) {
                 if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
-                __threadfence();
+                // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
                 __syncwarp();
                 if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
                 pend_ready = 0;
@@ -699,7 +714,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             if (lane == 0) sh_s[0] = -((double)ts_s[32] + dlt_s[32]);
         } else if (is_io) {
             const int jn = i0 + lane + 1;
-            pend_j = (jn < N) ? jn : -1;
+            pend_j = (jn <= N) ? jn : -1; // column N too: its T is the last row's gauge for k_chain_spec
             pend_T = dd_add_d(dd_add_d(Tref, (double)ts_s[lane + 1]), dlt_s[lane + 1]);
             pend_Z = zK[lane + 1];
             pend_ready = 1;
@@ -742,7 +757,406 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     }
     if (is_io && pend_ready) {
         if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
-        __threadfence();
+        // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
+        __syncwarp();
+        if (lane == 0) st_release(&a.p.cols_ready[dir], N);
+    }
+}
+
+// ==========================================================================================
+// The chain CTA with a STALE GAUGE.  Between two MD steps the
+// solution moves by a factor e^{O(1)} per column, so the gauge T_j the previous evaluation left in
+// g[dir] (refreshed by k_prep so that |Zhat| is in [1,2)) is as good as a fresh max-plus pass: with it
+// the column gauges t_p, the row gauges G_r = t_{r+1} - cc_r, the tile M = exp(t_p + tau - G_r), the
+// scaled contributions of all earlier columns and even the NEW T_j are known before the block is
+// reached.  What remains dependent is one linear pass per 32-row block (DFMA + SHFL per row), and
+// everything it needs is prepared by the other warps one or two blocks ahead:
+//   window K (while warp 0 solves block K):
+//     warp 15   publishes block K-1 (T, Zhat) to the workers, prefetches coordinates / cc / old T of block K+3
+//     warp 14   fetches and scales the workers' panel of block K+1
+//     warp 1    gauges of block K+2 (and the new T of its columns -> ring)
+//     warps 2-9   M tile of block K+1
+//     warps 10-13 contributions of the column blocks K+1-q, q = 2..L, to the rows of block K+1
+//     then warps 1-13: E'(K+2) = exp part of block K+1's columns against the rows of block K+2
+//   At the end of a block the exponent of Zhat of its last column is taken out of the following blocks'
+//   frame (exact powers of two), so a systematic drift of the solution along the chain cannot overflow.
+//   warp 0 folds E'(K+1) Zhat into the next block's start value inside its own loop (one more DFMA per
+//   step, off the dependent path), so one block-wide barrier per block is all the synchronisation.
+// A row sum outside [1e-270, 1e270] (the gauge no longer fits: first evaluation, state replaced, a jump)
+// raises status[2]; the host always queues the max-plus kernel behind this one, and that kernel returns at
+// once unless the flag is set.
+// ==========================================================================================
+template <int D> struct SpecSmem {
+    int RB;
+    size_t ringT, ringZ, ringSig, rho, cc, traw, ts, dlt, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, total;
+    __host__ __device__ SpecSmem()
+    {
+        RB = 256;
+        size_t o = 0;
+        ringT = o; o += 2 * (size_t)RB;
+        ringZ = o; o += RB;
+        ringSig = o; o += (size_t)RB * D;
+        rho = o; o += 4 * 32 * D;     // rows of blocks B & 3
+        cc = o; o += 4 * 32;
+        traw = o; o += 4 * 2 * 34;    // old T (double-double) of columns 32B .. 32B+32
+        ts = o; o += 4 * 20;          // float[4][40]
+        dlt = o; o += 4 * 40;
+        Gs = o; o += 4 * 32;
+        trefn = o; o += 4 * 2;        // new T of column 32B (double-double)
+        mt = o; o += 2 * 1024;        // M tiles of blocks B & 1
+        ue = o; o += 2 * 1024;        // E'(B & 1)
+        baseT = o; o += 2 * 2 * 4 * 32; // [B & 1][q - 2][quarter][row] partial sums of the older column blocks
+        baseP = o; o += 2 * 32;       // scaled panel for block B & 1
+        zmail = o; o += 2 * 32;       // Zhat of the columns block B & 1 produced, for the io warp
+        kacc = o; o += 4;             // int[8]: power of two taken out of Zhat up to the start of block B & 7
+        total = o;
+    }
+};
+
+template <int D, bool SGN>
+__device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_raw, const double *etab64)
+{
+    int N = a.N, L = a.look, NBk = a.NB;
+    asm volatile("" : "+r"(N), "+r"(L), "+r"(NBk));
+    const SpecSmem<D> lay;
+    constexpr int RB = 256;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    double *sm = reinterpret_cast<double *>(smem_raw);
+    double2 *ring_T = reinterpret_cast<double2 *>(sm + lay.ringT);
+    double *ring_Z = sm + lay.ringZ, *ring_sig = sm + lay.ringSig, *rho_s = sm + lay.rho, *cc_s = sm + lay.cc;
+    double2 *traw_s = reinterpret_cast<double2 *>(sm + lay.traw);
+    float *ts_s = reinterpret_cast<float *>(sm + lay.ts);
+    double *dlt_s = sm + lay.dlt, *G_s = sm + lay.Gs;
+    double2 *trefn_s = reinterpret_cast<double2 *>(sm + lay.trefn);
+    double *mt_s = sm + lay.mt, *ue_s = sm + lay.ue, *baseT_s = sm + lay.baseT, *baseP_s = sm + lay.baseP, *zmail_s = sm + lay.zmail;
+    int *kacc_s = reinterpret_cast<int *>(sm + lay.kacc);
+
+    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
+    double2 *g = a.p.g[dir];
+    double *gs = a.p.gs[dir];
+    const double kk = a.kk;
+    const bool is_io = (warp == CH_WARPS - 1);
+
+    // ---- pieces of the preparation, written for a group of `nt` threads with index `t`
+    // coordinates, cc and the old gauge of block B -> shared (32 threads are enough); zeros beyond N
+    auto load_raw = [&](int B, int t, int nt) {
+        const int b3 = B & 3;
+        for (int e = t; e < 33; e += nt) {
+            const int i = B * 32 + e;
+            // beyond the last column the gauge continues flat: padded rows must stay finite (0 * inf = NaN would
+            // leak into the real rows through their zero matrix entries)
+            const double2 told = ldcg2(&g[min(i, N)]);
+            traw_s[b3 * 34 + e] = told;
+            if (e < 32) {
+                Vec<D> pr, pc;
+#pragma unroll
+                for (int c = 0; c < D; ++c) { pr.v[c] = 0.0; pc.v[c] = 0.0; }
+                double c0 = 0.0;
+                if (i < N) {
+                    pr = ldvec<D>(rho, i);
+                    pc = ldvec<D>(sig, i);
+                    if (i < N - 1) c0 = cc[i];
+                }
+#pragma unroll
+                for (int c = 0; c < D; ++c) {
+                    rho_s[(b3 * 32 + e) * D + c] = pr.v[c];
+                    ring_sig[(i & (RB - 1)) * D + c] = pc.v[c];
+                }
+                cc_s[b3 * 32 + e] = c0;
+            }
+        }
+    };
+    // gauges of block B (one warp, lane = row r): t_{r+1} from the old T, G_r = t_{r+1} - cc_r, the new
+    // gauge t~_{r+1} = G_r + cc_r exactly (float t + remainder dlt), the new T of column 32B+r+1
+    auto gauges = [&](int B) {
+        const int b3 = B & 3, r = lane;
+        const double told = dd_diff(traw_s[b3 * 34 + r + 1], traw_s[b3 * 34]);
+        const double my_cc = cc_s[b3 * 32 + r];
+        const float Gf = (float)(told - my_cc);
+        const float tn = Gf + (float)my_cc;
+        const double dl = ((double)Gf - (double)tn) + my_cc;
+        G_s[b3 * 32 + r] = (double)Gf;
+        ts_s[b3 * 40 + r + 1] = tn;
+        dlt_s[b3 * 40 + r + 1] = dl;
+        if (r == 0) { ts_s[b3 * 40] = 0.f; dlt_s[b3 * 40] = 0.0; }
+        const double2 Tn = dd_add_d(dd_add_d(trefn_s[b3], (double)tn), dl);
+        ring_T[(B * 32 + r + 1) & (RB - 1)] = Tn;
+        if (r == 31) trefn_s[(B + 1) & 3] = Tn;
+    };
+    // M tile of block B: M[p][r] = exp(t~_p + tau[p][r] - G_r), p <= r (sx folded in for p >= 1)
+    auto build_M = [&](int B, int t, int nt) {
+        // only p <= r is needed: columns pp and 31-pp share one pass of 32 lanes (33 entries; the odd one,
+        // row 31 of column 31-pp, goes to a 17th pass); everything above the diagonal stays 0 from the start
+        const int b3 = B & 3;
+        double *mB = mt_s + (B & 1) * 1024;
+#pragma unroll 3
+        for (int e = t; e < 17 * 32; e += nt) {
+            const int pass = e >> 5, l = e & 31;
+            int p, r;
+            if (pass < 16) {
+                if (l >= pass) { p = pass; r = l; } else { p = 31 - pass; r = 31 - pass + l; }
+            } else {
+                p = 31 - (l & 15); r = 31; // 16 leftovers (each written twice, same value)
+            }
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
+            double m = exp_neg_tab64(-((((double)ts_s[b3 * 40 + p] - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + dlt_s[b3 * 40 + p]), etab64);
+            if constexpr (SGN) { if (p >= 1) m *= a.sx; }
+            mB[p * 32 + r] = m;
+        }
+    };
+    // E'(B)[p][r]: column p of block B-1 against row r of block B, relative to the new T of column 32B,
+    // scaled by exp(-G_r(B)); everything but the factor Zhat_p (sx folded in for p >= 1)
+    auto build_ue = [&](int B, int t, int nt) {
+        const int b3 = B & 3, c3 = (B - 1) & 3;
+        double *uB = ue_s + (B & 1) * 1024;
+        const double t32 = (double)ts_s[c3 * 40 + 32], d32 = dlt_s[c3 * 40 + 32];
+#pragma unroll 4
+        for (int e = t; e < 1024; e += nt) {
+            const int p = e >> 5, r = e & 31;
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c]; }
+            double u = ((((double)ts_s[c3 * 40 + p] - t32) - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + (dlt_s[c3 * 40 + p] - d32);
+            u = exp_neg_tab64(-(u), etab64);
+            if constexpr (SGN) { if (p >= 1) u *= a.sx; }
+            uB[e] = u;
+        }
+    };
+    // contributions of the complete column block B-q (q = 2..L) to the rows of block B, scaled by exp(-G_r(B)),
+    // in the gauge as the gauges() chain wrote it: quarter `qt` (8 columns), lane = row.  One partial sum per
+    // (q, quarter, row); warp 0 rescales it by the power of two that separates the two blocks' frames.
+    auto build_base = [&](int B, int qt) {
+        const int b3 = B & 3, r = lane;
+        Vec<D> pr;
+#pragma unroll
+        for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b3 * 32 + r) * D + c];
+        const double2 TrefB = trefn_s[b3];
+        const double Gr = G_s[b3 * 32 + r];
+        for (int q = 2; q <= L; ++q) {
+            const int C = B - q;
+            double s0 = 0.0, s1 = 0.0;
+            if (C >= 0) {
+                double u[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int slot = (C * 32 + qt * 8 + k) & (RB - 1);
+                    Vec<D> pc;
+#pragma unroll
+                    for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
+                    u[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) u[k] = exp_neg_tab64(-(u[k]), etab64);
+#pragma unroll
+                for (int k = 0; k < 8; k += 2) {
+                    s0 = fma(ring_Z[(C * 32 + qt * 8 + k) & (RB - 1)], u[k], s0);
+                    s1 = fma(ring_Z[(C * 32 + qt * 8 + k + 1) & (RB - 1)], u[k + 1], s1);
+                }
+            }
+            baseT_s[(((B & 1) * 2 + (q - 2)) * 4 + qt) * 32 + r] = s0 + s1;
+        }
+    };
+    // the workers' panel of block B (columns < 32 (B-L), published relative to the T of column 32 (B-L)),
+    // scaled like the rest; one warp, lane = row; waits for the workers
+    auto fetch_panel = [&](int B) {
+        const int b3 = B & 3, jrec0 = 32 * (B - L);
+        double v = 0.0;
+        if (jrec0 > 0 && B < NBk) {
+            if (lane == 0) {
+                while (ld_acquire(&a.p.panel_ready[dir][B]) == 0) { }
+            }
+            __syncwarp();
+            const int i = B * 32 + lane;
+            if (i < N) {
+                const double m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0 & (RB - 1)], trefn_s[b3]);
+                v = ldcg1(&a.p.pan_s[dir][i]) * exp_neg_tab64(-(m - G_s[b3 * 32 + lane]), etab64);
+            }
+        }
+        baseP_s[(B & 1) * 32 + lane] = v;
+    };
+    // 2^e as a double, 0 for e < -1000 (a contribution that far down is nothing), e <= 1000 assumed
+    auto pow2i = [](int e) { return e < -1000 ? 0.0 : __hiloint2double((1023 + min(e, 1000)) << 20, 0); };
+
+    // ---- prologue: raw data of blocks 0..2, gauges of blocks 0 and 1, then the helpers' window "-1"
+    for (int B = 0; B < 3; ++B) load_raw(B, tid, CH_THREADS);
+    if (tid == 0) {
+        const double2 T0 = ldcg2(&g[0]);
+        trefn_s[0] = T0;
+        ring_T[0] = T0;
+        ring_Z[0] = 1.0;
+    }
+    __syncthreads();
+    if (warp == 0) gauges(0);
+    __syncthreads();
+    if (warp == 0) gauges(1);
+    for (int e = tid; e < 2 * 2 * 4 * 32; e += CH_THREADS) baseT_s[e] = 0.0;
+    for (int e = tid; e < 2 * 1024; e += CH_THREADS) mt_s[e] = 0.0;
+    if (tid < 64) baseP_s[tid] = 0.0;
+    if (tid < 8) kacc_s[tid] = 0;
+    build_M(0, tid, CH_THREADS);
+    __syncthreads();
+    build_ue(1, tid, CH_THREADS);
+
+    int bad = 0;                     // warp 0: status of its rows
+    int kacc = 0;                    // warp 0: power of two taken out of Zhat up to the start of block K
+    int kh1 = 0, kh2 = 0, kh3 = 0, kh4 = 0; // warp 0: the same for blocks K-1 .. K-4
+    double z0 = 1.0, acc_next = 0.0; // warp 0: Zhat of the block's first column; start value of the next block
+    double2 fin_T = make_double2(0.0, 0.0);
+    double fin_G = 0.0, fin_acc = 1.0;
+    const double2 LN2 = make_double2(0.6931471805599453, 2.3190468138462996e-17);
+
+    __shared__ long long ph_s[16];
+    const bool tim = a.phase != nullptr && dir == 0 && tid == 0;
+    if (tid < 16) ph_s[tid] = 0;
+    long long tprev = clock64();
+#define PH(k) do { if (tim) { const long long c__ = clock64(); ph_s[k] += c__ - tprev; tprev = c__; } } while (0)
+
+    for (int K = 0; K < NBk; ++K) {
+        __syncthreads(); // everything block K needs is ready; everything of block K-1 has been consumed
+        PH(0);
+        const int i0 = K * 32, cur = K & 1, k3 = K & 3;
+        const int nrows = min(32, N - i0);
+        if (warp == 0) {
+            const double *mK = mt_s + cur * 1024 + lane, *uN = ue_s + (cur ^ 1) * 1024 + lane;
+            // earlier columns, each group brought from its own frame to this block's (exact powers of two);
+            // all loads first, the frames of the last blocks are kept in registers (kh[q] = frame of block K-q)
+            const double *bq = baseT_s + (cur * 2 * 4) * 32 + lane;
+            const double b20 = bq[0], b21 = bq[32], b22 = bq[64], b23 = bq[96];
+            const double b30 = bq[128], b31 = bq[160], b32 = bq[192], b33 = bq[224];
+            const double bp = baseP_s[cur * 32 + lane];
+            double m_n = mK[0], u_n = uN[32];
+            const double u0 = uN[0];
+            double acc = acc_next * pow2i(kh1 - kacc);
+            if (K >= 2) acc = fma((b20 + b21) + (b22 + b23), pow2i(kh2 - kacc), acc);
+            if (L >= 3 && K >= 3) acc = fma((b30 + b31) + (b32 + b33), pow2i(kh3 - kacc), acc);
+            if (K - L - 1 >= 0) acc = fma(bp, pow2i((L == 1 ? kh2 : (L == 2 ? kh3 : kh4)) - kacc), acc);
+            double zc = z0;
+            acc_next = u0 * z0;
+            PH(1);
+#pragma unroll
+            for (int p = 0; p < 32; ++p) {
+                const double m_p = m_n, u_p = u_n; // operands of this step were loaded one step ahead
+                if (p < 31) m_n = mK[(p + 1) * 32];
+                if (p < 30) u_n = uN[(p + 2) * 32];
+                acc = fma(m_p, zc, acc);          // M[p][r] = 0 once p > r
+                zc = shfl_bcast(acc, p);          // X^_p; Zhat_{p+1} = sx X^_p (sx is folded into M and E')
+                if (p < 31) acc_next = fma(u_p, zc, acc_next);
+            }
+            PH(2);
+            // Zhat of the columns this block produced (frame of block K); the next block's frame takes the
+            // exponent of its first column out, so that Zhat stays O(1) however far the solution has drifted
+            const double zmine = SGN ? a.sx * acc : acc;
+            const double z32 = SGN ? a.sx * zc : zc;
+            const int ex = (__double2hiint(z32) >> 20) & 0x7ff;
+            const int kstep = (ex != 0 && ex != 0x7ff) ? ex - 1023 : 0;
+            z0 = z32 * pow2i(-kstep);
+            zmail_s[cur * 32 + lane] = zmine;
+            const int jn = i0 + lane + 1;
+            if (jn < N) ring_Z[jn & (RB - 1)] = (lane == 31) ? z0 : zmine;
+            if (lane == 0) kacc_s[K & 7] = kacc;
+            if (lane < nrows) {
+                if (acc == 0.0) bad |= ST_NODE;
+                else if (!(fabs(acc) > 1e-270 && fabs(acc) < 1e270)) {
+#ifdef PIMD_DEBUG_GAUGE
+                    if (!(bad & 4) && a.phase) { a.phase[8 + 4 * dir] = i0 + lane; a.phase[9 + 4 * dir] = (unsigned long long)__double_as_longlong(acc);
+                        a.phase[10 + 4 * dir] = (unsigned long long)__double_as_longlong(z0); a.phase[11 + 4 * dir] = (unsigned long long)(long long)kacc; }
+#endif
+                    bad |= 4;
+                }
+            }
+            if (K + 1 == NBk) {
+                fin_T = dd_add_d(dd_add_d(trefn_s[k3], (double)kacc * LN2.x), (double)kacc * LN2.y);
+                fin_G = G_s[k3 * 32 + lane];
+                fin_acc = acc;
+            }
+            kh4 = kh3; kh3 = kh2; kh2 = kh1; kh1 = kacc;
+            kacc += kstep;
+            PH(3);
+        } else if (warp == CH_WARPS - 1) {
+            if (K > 0) { // publish the columns block K-1 produced, in its frame (column N is kept too: its T is
+                         // the last row's gauge next time)
+                const int jn = i0 - 32 + lane + 1;
+                if (jn <= N) {
+                    const double kf = (double)kacc_s[(K - 1) & 7];
+                    g[jn] = dd_add_d(dd_add_d(ring_T[jn & (RB - 1)], kf * LN2.x), kf * LN2.y);
+                    gs[jn] = zmail_s[(cur ^ 1) * 32 + lane];
+                }
+            }
+            if (K > 0) {
+                __syncwarp();
+                if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
+            }
+        } else if (warp == CH_WARPS - 3) {
+            // raw data of block K+3
+            const int b3 = (K + 3) & 3, i = (K + 3) * 32 + lane;
+            double2 told = make_double2(0.0, 0.0), told32 = told;
+            Vec<D> pr, pc;
+#pragma unroll
+            for (int c = 0; c < D; ++c) { pr.v[c] = 0.0; pc.v[c] = 0.0; }
+            double c0 = 0.0;
+            told = ldcg2(&g[min(i, N)]); // flat beyond the last column (see load_raw)
+            if (lane == 0) told32 = ldcg2(&g[min(i + 32, N)]);
+            if (i < N) {
+                pr = ldvec<D>(rho, i);
+                pc = ldvec<D>(sig, i);
+                if (i < N - 1) c0 = cc[i];
+            }
+            traw_s[b3 * 34 + lane] = told;
+            if (lane == 0) traw_s[b3 * 34 + 32] = told32;
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                rho_s[(b3 * 32 + lane) * D + c] = pr.v[c];
+                ring_sig[(i & (RB - 1)) * D + c] = pc.v[c];
+            }
+            cc_s[b3 * 32 + lane] = c0;
+        } else if (warp == CH_WARPS - 2) {
+            long long hc0 = clock64();
+            fetch_panel(K + 1);
+            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[9] += clock64() - hc0;
+        } else if ((warp & 3) != 0) {
+            // 9 helper warps; the three that share warp 0's scheduler partition (4, 8, 12) stay out of its way
+            const int hw = warp - 1 - (warp >> 2), ht = hw * 32 + lane; // 0..8, 288 threads
+            const bool th = a.phase != nullptr && dir == 0 && lane == 0;
+            long long hc0 = clock64();
+            if (hw == 0) {
+                gauges(K + 2);
+            } else if (hw <= 4) {
+                build_M(K + 1, ht - 32, 4 * 32);
+            } else {
+                build_base(K + 1, hw - 5);
+            }
+            if (th && hw == 0) ph_s[4] += clock64() - hc0;
+            if (th && hw == 1) ph_s[5] += clock64() - hc0;
+            if (th && hw == 5) ph_s[6] += clock64() - hc0;
+            bar_sync_named(1, 9 * 32); // the gauges of block K+2 are in place
+            if (th && hw == 0) ph_s[7] += clock64() - hc0;
+            build_ue(K + 2, ht, 9 * 32);
+            if (th && hw == 0) ph_s[8] += clock64() - hc0;
+        }
+    }
+    __syncthreads();
+#undef PH
+    if (tim) {
+        for (int k = 0; k < 16; ++k) a.phase[k] += (unsigned long long)ph_s[k];
+    }
+    if (warp == 0) {
+        if (lane == (N - 1) % 32) {
+            a.p.rfin[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
+            a.p.rsgn[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
+        }
+        if (bad & 3) atomicOr(a.p.status, bad & 3);
+        if (bad & 4) atomicOr(a.p.status + 2, 1);
+    }
+    if (warp == CH_WARPS - 1) {
+        const int jn = (NBk - 1) * 32 + lane + 1;
+        if (jn <= N) {
+            const double kf = (double)kacc_s[(NBk - 1) & 7];
+            g[jn] = dd_add_d(dd_add_d(ring_T[jn & (RB - 1)], kf * LN2.x), kf * LN2.y);
+            gs[jn] = zmail_s[((NBk - 1) & 1) * 32 + lane];
+        }
+        // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
         __syncwarp();
         if (lane == 0) st_release(&a.p.cols_ready[dir], N);
     }
@@ -776,8 +1190,10 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
         const int ntile = K - LOOK;
         Lse acc = lse_empty();
         double2 ref = make_double2(0.0, 0.0);
-        for (int J = warp; J < ntile; J += CH_WARPS) {
-            const int need = 32 * (J + 1);
+        // unit of work = 8 columns; chunk c goes to warp c mod 16, so the four chunks of the newest tile (the
+        // ones the chain is waiting for) are done by four warps at once
+        for (int c8 = warp; c8 < 4 * ntile; c8 += CH_WARPS) {
+            const int need = 32 * ((c8 >> 2) + 1);
             if (known_ready < need) {
                 if (lane == 0) {
                     int v;
@@ -787,8 +1203,8 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 known_ready = __shfl_sync(0xffffffffu, known_ready, 0);
             }
             __syncwarp();
-            {
-                const int j = 32 * J + lane;
+            if (lane < 8) {
+                const int j = 8 * c8 + lane;
                 st_g[lane] = ldcg2(&g[j]);
                 st_sg[lane] = ldcg1(&gs[j]);
                 Vec<D> pc = ldvec<D>(sig, j);
@@ -799,27 +1215,27 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             const double2 nref = st_g[0];
             lse_shift(acc, dd_diff(ref, nref));
             ref = nref;
-#pragma unroll 1
-            for (int c0 = 0; c0 < 32; c0 += 8) {
-                double tau[8];
-                double cm = -INFINITY;
+            double tau[8];
+            double cm = -INFINITY;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    Vec<D> pc;
+            for (int k = 0; k < 8; ++k) {
+                Vec<D> pc;
 #pragma unroll
-                    for (int c = 0; c < D; ++c) pc.v[c] = st_sig[(c0 + k) * D + c];
-                    tau[k] = dd_diff(st_g[c0 + k], ref) - kk * dist2<D>(pr, pc);
-                    cm = fmax(cm, tau[k]);
-                }
-                if (cm > acc.m) {
-                    acc.s *= exp_tab(acc.m - cm, etab);
-                    acc.m = cm;
-                }
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    acc.s = fma(exp_tab(tau[k] - acc.m, etab), st_sg[c0 + k], acc.s);
-                }
+                for (int c = 0; c < D; ++c) pc.v[c] = st_sig[k * D + c];
+                tau[k] = dd_diff(st_g[k], ref) - kk * dist2<D>(pr, pc);
+                cm = fmax(cm, tau[k]);
             }
+            if (cm > acc.m) {
+                acc.s *= exp_tab(acc.m - cm, etab);
+                acc.m = cm;
+            }
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 8; k += 2) {
+                s0 = fma(exp_tab(tau[k] - acc.m, etab), st_sg[k], s0);
+                s1 = fma(exp_tab(tau[k + 1] - acc.m, etab), st_sg[k + 1], s1);
+            }
+            acc.s += s0 + s1;
             __syncwarp();
         }
         // common reference of the published partial: g_{32 ntile} (first "recent" column of block K)
@@ -841,13 +1257,19 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
         mg_s[warp * 32 + lane] = acc.s;
         __syncthreads();
         if (warp == 0) {
+            // 16 partials per row: maximum first, then 16 independent exponentials
             Lse t = lse_empty();
-            for (int w = 0; w < CH_WARPS; ++w) lse_merge(t, Lse{mg_m[w * 32 + lane], mg_s[w * 32 + lane]});
+#pragma unroll
+            for (int w = 0; w < CH_WARPS; ++w) t.m = fmax(t.m, mg_m[w * 32 + lane]);
+            if (t.m > -INFINITY) {
+#pragma unroll
+                for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_tab(mg_m[w * 32 + lane] - t.m, etab), t.s);
+            }
             if (i < N) {
                 a.p.pan_m[dir][i] = t.m;
                 a.p.pan_s[dir][i] = t.s;
             }
-            __threadfence();
+            // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
             __syncwarp();
             if (lane == 0) st_release(&a.p.panel_ready[dir][K], 1);
         }
@@ -863,8 +1285,39 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
     if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
     __syncthreads();
     const int dir = blockIdx.y;
+    if (a.cond) {
+        // queued behind k_chain_spec: needed only if that kernel found its gauge out of range
+        if (ld_acquire(a.p.status + 2) == 0) return; // the same answer in every CTA
+        if (blockIdx.x == 0 && blockIdx.y == 0) {
+            for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { a.p.panel_ready[0][k] = 0; a.p.panel_ready[1][k] = 0; }
+            if (threadIdx.x < 2) a.p.cols_ready[threadIdx.x] = 1;
+        }
+        __threadfence();
+        cooperative_groups::this_grid().sync();
+    }
     if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw, etab);
     else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab);
+}
+
+// the recursion with the previous evaluation's gauge (see chain_cta_spec); same grid, same workers
+template <int D, bool SGN>
+__global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double etab[32], etab64[64];
+    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __syncthreads();
+    const int dir = blockIdx.y;
+    if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, smem_raw, etab64);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab);
+}
+
+template <int D> size_t chain_spec_smem_bytes_host()
+{
+    const size_t chain = SpecSmem<D>().total * 8;
+    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
+    return chain > worker ? chain : worker;
 }
 
 // ==========================================================================================
