@@ -422,7 +422,7 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     h->nprep = (N + PREP_TB - 1) / PREP_TB;
     h->nasm = (N + ASM_TB - 1) / ASM_TB;
     h->look = 2;
-    h->look_spec = 2;
+    h->look_spec = 3;
     if (const char *e = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
         const int v = std::atoi(e);
         if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;

@@ -884,26 +884,40 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         if (r == 31) trefn_s[(B + 1) & 3] = Tn;
     };
     // M tile of block B: M[p][r] = exp(t~_p + tau[p][r] - G_r), p <= r (sx folded in for p >= 1)
+    // The exponent arguments of a batch of four entries are formed first, then the four exponentials, then the
+    // stores: written as a plain loop the compiler keeps the iterations in order (a shared-memory store of one
+    // might alias the loads of the next) and every entry pays its full ~250-cycle dependent chain.
     auto build_M = [&](int B, int t, int nt) {
         // only p <= r is needed: columns pp and 31-pp share one pass of 32 lanes (33 entries; the odd one,
         // row 31 of column 31-pp, goes to a 17th pass); everything above the diagonal stays 0 from the start
         const int b3 = B & 3;
         double *mB = mt_s + (B & 1) * 1024;
-#pragma unroll 3
-        for (int e = t; e < 17 * 32; e += nt) {
-            const int pass = e >> 5, l = e & 31;
-            int p, r;
-            if (pass < 16) {
-                if (l >= pass) { p = pass; r = l; } else { p = 31 - pass; r = 31 - pass + l; }
-            } else {
-                p = 31 - (l & 15); r = 31; // 16 leftovers (each written twice, same value)
-            }
-            Vec<D> pr, pc;
+        for (int e0 = t; e0 < 17 * 32; e0 += 4 * nt) {
+            double arg[4];
+            int idx[4];
 #pragma unroll
-            for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
-            double m = exp_neg_tab64(-((((double)ts_s[b3 * 40 + p] - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + dlt_s[b3 * 40 + p]), etab64);
-            if constexpr (SGN) { if (p >= 1) m *= a.sx; }
-            mB[p * 32 + r] = m;
+            for (int j = 0; j < 4; ++j) {
+                const int e = e0 + j * nt;
+                const int pass = min(e >> 5, 16), l = e & 31;
+                int p, r;
+                if (pass < 16) {
+                    if (l >= pass) { p = pass; r = l; } else { p = 31 - pass; r = 31 - pass + l; }
+                } else {
+                    p = 31 - (l & 15); r = 31; // 16 leftovers (each written twice, same value)
+                }
+                Vec<D> pr, pc;
+#pragma unroll
+                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
+                arg[j] = (((double)ts_s[b3 * 40 + p] - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + dlt_s[b3 * 40 + p];
+                idx[j] = (e < 17 * 32) ? p * 32 + r : -1;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) arg[j] = exp_neg_tab64(-arg[j], etab64);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if constexpr (SGN) { if (idx[j] >= 32) arg[j] *= a.sx; }
+                if (idx[j] >= 0) mB[idx[j]] = arg[j];
+            }
         }
     };
     // E'(B)[p][r]: column p of block B-1 against row r of block B, relative to the new T of column 32B,
@@ -912,16 +926,25 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         const int b3 = B & 3, c3 = (B - 1) & 3;
         double *uB = ue_s + (B & 1) * 1024;
         const double t32 = (double)ts_s[c3 * 40 + 32], d32 = dlt_s[c3 * 40 + 32];
-#pragma unroll 4
-        for (int e = t; e < 1024; e += nt) {
-            const int p = e >> 5, r = e & 31;
-            Vec<D> pr, pc;
+        for (int e0 = t; e0 < 1024; e0 += 4 * nt) {
+            double arg[4];
 #pragma unroll
-            for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c]; }
-            double u = ((((double)ts_s[c3 * 40 + p] - t32) - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + (dlt_s[c3 * 40 + p] - d32);
-            u = exp_neg_tab64(-(u), etab64);
-            if constexpr (SGN) { if (p >= 1) u *= a.sx; }
-            uB[e] = u;
+            for (int j = 0; j < 4; ++j) {
+                const int e = min(e0 + j * nt, 1023);
+                const int p = e >> 5, r = e & 31;
+                Vec<D> pr, pc;
+#pragma unroll
+                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c]; }
+                arg[j] = ((((double)ts_s[c3 * 40 + p] - t32) - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + (dlt_s[c3 * 40 + p] - d32);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) arg[j] = exp_neg_tab64(-arg[j], etab64);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = e0 + j * nt;
+                if constexpr (SGN) { if (e >= 32) arg[j] *= a.sx; }
+                if (e < 1024) uB[e] = arg[j];
+            }
         }
     };
     // contributions of the complete column block B-q (q = 2..L) to the rows of block B, scaled by exp(-G_r(B)),
