@@ -99,15 +99,19 @@ def recursion_report(w, kern, phases, steps, clocks):
     """Latency figures of the N-long chain (neither roofline binds it)."""
     ch = kern.get("chain", {}).get("ms_avg")
     nb = (w.N + 31) // 32
-    out = {"kernel": "k_chain (forward + backward recursion, one cooperative launch)", "bound": "latency",
+    out = {"kernel": "k_chain_spec (forward + backward recursion with the previous step's gauge, one cooperative launch)",
+           "bound": "latency", "fallback_ms": kern.get("chain_fallback", {}).get("ms_avg"),
            "ms": ch, "ns_per_row": (ch * 1e6 / w.N if ch else None), "rows_per_block": 32}
-    if ch and sum(phases[:9]) > 0:
-        per = [c / float(steps * nb) for c in phases[:9]]
-        out["cycles_per_block"] = {"loop_overhead": per[0], "P1_maxplus_pass": per[1] + per[2], "P2_exponentials": per[3] + per[4],
-                                   "P3_linear_pass": per[5] + per[6], "P4_publish": per[7] + per[8], "sum": sum(per)}
-        out["floor_cycles_per_block"] = 32 * (41 + 38)
-        out["note"] = ("SM cycles of the forward chain CTA per 32-row block (clock64 inside the kernel, own time + barrier wait "
-                       "per phase); floor = 32 x (SHFL + FADD + FMNMX + FADD) + 32 x (SHFL + DFMA) from measured latencies")
+    if ch and sum(phases[:4]) > 0:
+        per = [c / float(steps * nb) for c in phases[:10]]
+        out["cycles_per_block"] = {"barrier_wait": per[0], "prologue": per[1], "dependent_steps_32": per[2], "epilogue": per[3],
+                                   "sum": sum(per[:4]),
+                                   "helpers": {"gauges": per[4], "M_tile": per[5], "older_blocks": per[6], "inner_barrier": per[7],
+                                               "E_tile_done": per[8], "panel_fetched": per[9]}}
+        out["floor_cycles_per_block"] = 32 * 38
+        out["note"] = ("SM cycles of the forward chain CTA per 32-row block (clock64 inside k_chain_spec, the stale-gauge "
+                       "kernel every timed step runs); floor = 32 x (SHFL + DFMA) from measured latencies; the block time is "
+                       "set by the helper warps / the workers' panel (barrier_wait), not by the dependent steps")
     return out
 
 

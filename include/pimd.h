@@ -140,9 +140,15 @@ uint64_t pimd_launch_count(pimd_t h);
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM
- * cycles per phase of its 32-row blocks: cycles_host[0] loop overhead; [2k-1] the dependent warp's own time
- * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish); [2k] its wait at the
- * barrier that ends phase k.  HOST out, 16 entries, accumulated since the previous call (then reset). */
+ * cycles per phase of its 32-row blocks (HOST out, 16 entries, accumulated since the previous call, then reset).
+ * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation but the first after
+ * pimd_set_state) fill
+ *   [0] wait at the block barrier (the helper warps or the workers' panel are late), [1] the dependent warp's
+ *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; helper warps, measured from the barrier:
+ *   [4] gauges, [5] M tile, [6] older column blocks, [7] helpers' inner barrier reached, [8] E' tile done,
+ *   [9] workers' panel fetched.
+ * Evaluations with a fresh max-plus gauge (k_chain) fill [0] loop overhead, [2k-1] the dependent warp's own time
+ * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish), [2k] its barrier wait. */
 int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host);
 
 /* Measured FP64 FMA issue rate of the device (a register-resident DFMA loop over all SMs; used
