@@ -79,7 +79,7 @@ int pimd_set_concurrency(pimd_t h, int on);
 
 /* Copy state in / out.  x_dev, v_dev: DEVICE pointers, [P][N][d] doubles; v_dev may be NULL
  * (set: velocities zero; get: skipped).  Setting the state resets the Nose-Hoover variables to zero
- * and invalidates cached forces.  *_host variants take HOST pointers (pageable or pinned). */
+ * and invalidates cached forces (see pimd_set_forces).  *_host variants take HOST pointers (pageable or pinned). */
 int pimd_set_state(pimd_t h, const double *x_dev, const double *v_dev);
 int pimd_get_state(pimd_t h, double *x_dev, double *v_dev);
 int pimd_set_state_host(pimd_t h, const double *x_host, const double *v_host);
@@ -98,6 +98,16 @@ int pimd_set_nhc(pimd_t h, const double *nhc_dev);
  * Synchronises the stream.  PIMD_ENUMERIC if the state is non-finite or W_N == 0. */
 int pimd_forces(pimd_t h, double *f_dev, double *vb, int *sign);
 int pimd_forces_host(pimd_t h, double *f_host, double *vb, int *sign);
+
+/* Cached total forces F = -grad(V_xi + U/P) at the current positions, [P][N][d] (DEVICE / HOST variants).
+ * get: no evaluation is made; PIMD_EINVAL if no forces are cached (state just set, nothing evaluated).  Synchronises.
+ * set: hands the library the forces that belong to the state just set with pimd_set_state() (checkpoint resume,
+ * host-resident states), so that the next pimd_step() does not have to evaluate them first.  The caller vouches for
+ * them; call after pimd_set_state(). */
+int pimd_get_forces(pimd_t h, double *f_dev);
+int pimd_get_forces_host(pimd_t h, double *f_host);
+int pimd_set_forces(pimd_t h, const double *f_dev);
+int pimd_set_forces_host(pimd_t h, const double *f_host);
 
 /* Tables of the last force evaluation, HOST out (any may be NULL):
  *   vfwd[n] = V_xi^{[1,n]}, n = 0..N  (N+1 doubles; Eq. 6)

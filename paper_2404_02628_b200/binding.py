@@ -38,6 +38,10 @@ _SYMBOLS = {
     "pimd_set_nhc": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_forces": (C.c_int, [C.c_void_p, C.c_void_p, _dp, C.POINTER(C.c_int)]),
     "pimd_forces_host": (C.c_int, [C.c_void_p, C.c_void_p, _dp, C.POINTER(C.c_int)]),
+    "pimd_get_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_get_forces_host": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_set_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_set_forces_host": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_tables": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_estimators": (C.c_int, [C.c_void_p, _dp, _dp, C.c_void_p, C.c_int, C.c_double]),
@@ -186,6 +190,20 @@ class Pimd:
         vb, sg = C.c_double(), C.c_int()
         self._check(self._lib.pimd_forces_host(self._h, _ptr(f_host), C.byref(vb), C.byref(sg)))
         return vb.value, sg.value
+
+    def get_forces(self, out=None):
+        f = out if out is not None else self._empty_state()
+        self._check(self._lib.pimd_get_forces(self._h, _ptr(f)))
+        return f
+
+    def get_forces_host(self, f_host):
+        self._check(self._lib.pimd_get_forces_host(self._h, _ptr(f_host)))
+
+    def set_forces(self, f_dev):
+        self._check(self._lib.pimd_set_forces(self._h, _ptr(f_dev)))
+
+    def set_forces_host(self, f_host):
+        self._check(self._lib.pimd_set_forces_host(self._h, _ptr(f_host)))
 
     def get_tables(self):
         import numpy as np

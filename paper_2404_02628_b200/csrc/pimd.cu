@@ -539,7 +539,8 @@ static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpy
     if (h->thermostat == PIMD_THERMOSTAT_NHC) CU(cudaMemsetAsync(h->nhc, 0, h->ndof * 8 * PIMD_NHC_LENGTH, h->s0));
     CU(cudaMemsetAsync(h->status, 0, 4 * sizeof(int), h->s0));
     h->forces_valid = false;
-    h->gauge_valid = false;
+    // the exchange gauge of the last evaluation is kept: if the new positions are far from the old ones the
+    // stale-gauge kernel notices and the max-plus kernel queued behind it takes over
     return PIMD_OK;
 }
 
@@ -613,6 +614,38 @@ static int forces_impl(pimd_t h, double *f, bool host, double *vb, int *sign)
     if (sign) *sign = h->h_scal->sign < 0 ? -1 : 1;
     return PIMD_OK;
 }
+
+static int get_forces_impl(pimd_t h, double *f, bool host)
+{
+    if (!h || !f) return PIMD_EINVAL;
+    if (!h->forces_valid) return fail(h, PIMD_EINVAL, "no forces cached for the current positions");
+    double *dst = host ? h->Fout : f;
+    {
+        ProfScope ps(h, PIMD_PROF_COMBINE, h->s0);
+        k_combine<<<(unsigned)((h->ndof + 255) / 256), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P);
+    }
+    CU(cudaGetLastError());
+    if (host) CU(cudaMemcpyAsync(f, h->Fout, h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
+    CU(cudaStreamSynchronize(h->s0));
+    return PIMD_OK;
+}
+
+static int set_forces_impl(pimd_t h, const double *f, cudaMemcpyKind kind)
+{
+    if (!h || !f) return PIMD_EINVAL;
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->F, f, h->ndof * 8, kind, h->s0));
+    CU(cudaMemsetAsync(h->Fex1, 0, h->slice * 8, h->s0));
+    CU(cudaMemsetAsync(h->FexP, 0, h->slice * 8, h->s0));
+    h->forces_valid = true;
+    return PIMD_OK;
+}
+
+int pimd_get_forces(pimd_t h, double *f_dev) { return get_forces_impl(h, f_dev, false); }
+int pimd_get_forces_host(pimd_t h, double *f_host) { return get_forces_impl(h, f_host, true); }
+int pimd_set_forces(pimd_t h, const double *f_dev) { return set_forces_impl(h, f_dev, cudaMemcpyDeviceToDevice); }
+int pimd_set_forces_host(pimd_t h, const double *f_host) { return set_forces_impl(h, f_host, cudaMemcpyHostToDevice); }
 
 int pimd_forces(pimd_t h, double *f_dev, double *vb, int *sign) { return forces_impl(h, f_dev, false, vb, sign); }
 int pimd_forces_host(pimd_t h, double *f_host, double *vb, int *sign) { return forces_impl(h, f_host, true, vb, sign); }

@@ -912,7 +912,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 idx[j] = (e < 17 * 32) ? p * 32 + r : -1;
             }
 #pragma unroll
-            for (int j = 0; j < 4; ++j) arg[j] = exp_neg_tab64(-arg[j], etab64);
+            for (int j = 0; j < 4; ++j) arg[j] = exp_cap_tab64(arg[j], etab64);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 if constexpr (SGN) { if (idx[j] >= 32) arg[j] *= a.sx; }
@@ -938,7 +938,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 arg[j] = ((((double)ts_s[c3 * 40 + p] - t32) - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + (dlt_s[c3 * 40 + p] - d32);
             }
 #pragma unroll
-            for (int j = 0; j < 4; ++j) arg[j] = exp_neg_tab64(-arg[j], etab64);
+            for (int j = 0; j < 4; ++j) arg[j] = exp_cap_tab64(arg[j], etab64);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int e = e0 + j * nt;
@@ -971,7 +971,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                     u[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
                 }
 #pragma unroll
-                for (int k = 0; k < 8; ++k) u[k] = exp_neg_tab64(-(u[k]), etab64);
+                for (int k = 0; k < 8; ++k) u[k] = exp_cap_tab64(u[k], etab64);
 #pragma unroll
                 for (int k = 0; k < 8; k += 2) {
                     s0 = fma(ring_Z[(C * 32 + qt * 8 + k) & (RB - 1)], u[k], s0);
@@ -994,7 +994,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const int i = B * 32 + lane;
             if (i < N) {
                 const double m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0 & (RB - 1)], trefn_s[b3]);
-                v = ldcg1(&a.p.pan_s[dir][i]) * exp_neg_tab64(-(m - G_s[b3 * 32 + lane]), etab64);
+                v = ldcg1(&a.p.pan_s[dir][i]) * exp_cap_tab64(m - G_s[b3 * 32 + lane], etab64);
             }
         }
         baseP_s[(B & 1) * 32 + lane] = v;

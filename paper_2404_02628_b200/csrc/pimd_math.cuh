@@ -124,6 +124,10 @@ PIMD_DEV double exp_neg_tab64(double r2, const double *tab)
     return __hiloint2double(__double2hiint(v) + (j >> 6) * 1048576, __double2loint(v));
 }
 
+// exp(x) for any x through the same table: x is capped at 700 so that a wildly wrong exponent (a gauge that no
+// longer fits) gives ~1e304 and trips the caller's range check instead of wrapping the exponent field
+PIMD_DEV double exp_cap_tab64(double x, const double *tab) { return exp_neg_tab64(-fmin(x, 700.0), tab); }
+
 // ---------------------------------------------------------------------------------------------
 // double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
 // tables a[u], q[l] reach 1e5..1e7 in magnitude while only their DIFFERENCES enter an exp, so

@@ -325,3 +325,31 @@ def test_stale_gauge_evaluations_match_oracle(binding, oracle):
         assert sg == sgo
         assert abs(vb - vbo) <= tol * abs(vbo)
         check_forces(F.cpu().numpy(), Fo, tol)
+
+
+def test_forces_round_trip_and_resume(binding, oracle):
+    """pimd_get_forces returns what pimd_forces computed; a second handle fed (x, v, F) through set_state +
+    set_forces continues bit-identically to the first one (NVE: no noise involved), without re-evaluating."""
+    w = wl.custom(97, 6, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.8)
+    x, v = wl.make_state(w, 6)
+    a = make(binding, w)
+    a.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    with pytest.raises(binding.PimdError):
+        a.get_forces()
+    F, _, _ = a.forces()
+    assert torch.equal(a.get_forces(), F)
+    a.step(2)
+    xa, va = a.get_state()
+    Fa = a.get_forces()
+    b = make(binding, w)
+    b.set_state(xa, va)
+    b.set_forces(Fa)
+    l0 = b.launch_count()
+    b.step(1)
+    assert b.launch_count() - l0 <= 12  # one evaluation, not two
+    a.step(1)
+    xb, vb_ = b.get_state()
+    xa2, va2 = a.get_state()
+    a.close(); b.close()
+    assert relerr(xb.cpu().numpy(), xa2.cpu().numpy()) <= 1e-13
+    assert relerr(vb_.cpu().numpy(), va2.cpu().numpy()) <= 1e-12
