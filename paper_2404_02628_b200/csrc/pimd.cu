@@ -4,6 +4,7 @@
 #include "../../include/pimd.h"
 #include "pimd_kernels.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -216,7 +217,9 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         // pair forces, added to F (Newton's third law, one Gaussian per unordered pair)
         const int NT = (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
-        const int nchunk = hmax > 0 ? (hmax + PAIR_CH / 2) / PAIR_CH + ((hmax + PAIR_CH / 2) / PAIR_CH == 0) : 0; // ~PAIR_CH offsets per task
+        int target = NT <= 64 ? 2 : 4; // offsets per task: small tasks balance small grids (tuning knob PIMD_PAIR_CH)
+        if (const char *e = std::getenv("PIMD_PAIR_CH")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) target = v; }
+        const int nchunk = hmax > 0 ? std::max(1, (hmax + target / 2) / target) : 0;
         const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
         const long long tasks = (long long)NT * (nchunk + 1);
         const dim3 pgrid((unsigned)((tasks + PAIR_WARPS - 1) / PAIR_WARPS), h->P);
