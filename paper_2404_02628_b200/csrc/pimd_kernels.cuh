@@ -788,7 +788,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 // ==========================================================================================
 template <int D> struct SpecSmem {
     int RB;
-    size_t ringT, ringZ, ringSig, rho, cc, traw, ts, dlt, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, total;
+    size_t ringT, ringZ, ringSig, rho, cc, traw, colT, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, total;
     __host__ __device__ SpecSmem()
     {
         RB = 256;
@@ -796,16 +796,15 @@ template <int D> struct SpecSmem {
         ringT = o; o += 2 * (size_t)RB;
         ringZ = o; o += RB;
         ringSig = o; o += (size_t)RB * D;
-        rho = o; o += 4 * 32 * D;     // rows of blocks B & 3
-        cc = o; o += 4 * 32;
-        traw = o; o += 4 * 2 * 34;    // old T (double-double) of columns 32B .. 32B+32
-        ts = o; o += 4 * 20;          // float[4][40]
-        dlt = o; o += 4 * 40;
-        Gs = o; o += 4 * 32;
-        trefn = o; o += 4 * 2;        // new T of column 32B (double-double)
+        rho = o; o += 8 * 32 * D;     // rows of blocks B & 7
+        cc = o; o += 8 * 32;
+        traw = o; o += 8 * 2 * 34;    // old T (double-double) of columns 32B .. 32B+32
+        colT = o; o += 8 * 2 * 34;    // column gauges of block B & 7: (t_p as float value, remainder), p = 0..32
+        Gs = o; o += 8 * 32;
+        trefn = o; o += 8 * 2;        // new T of column 32B (double-double)
         mt = o; o += 2 * 1024;        // M tiles of blocks B & 1
         ue = o; o += 2 * 1024;        // E'(B & 1)
-        baseT = o; o += 2 * 2 * 4 * 32; // [B & 1][q - 2][quarter][row] partial sums of the older column blocks
+        baseT = o; o += 2 * 2 * 9 * 32; // [B & 1][q - 2][helper warp][row] partial sums of the older column blocks
         baseP = o; o += 2 * 32;       // scaled panel for block B & 1
         zmail = o; o += 2 * 32;       // Zhat of the columns block B & 1 produced, for the io warp
         kacc = o; o += 4;             // int[8]: power of two taken out of Zhat up to the start of block B & 7
@@ -825,8 +824,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     double2 *ring_T = reinterpret_cast<double2 *>(sm + lay.ringT);
     double *ring_Z = sm + lay.ringZ, *ring_sig = sm + lay.ringSig, *rho_s = sm + lay.rho, *cc_s = sm + lay.cc;
     double2 *traw_s = reinterpret_cast<double2 *>(sm + lay.traw);
-    float *ts_s = reinterpret_cast<float *>(sm + lay.ts);
-    double *dlt_s = sm + lay.dlt, *G_s = sm + lay.Gs;
+    double2 *colT_s = reinterpret_cast<double2 *>(sm + lay.colT);
+    double *G_s = sm + lay.Gs;
     double2 *trefn_s = reinterpret_cast<double2 *>(sm + lay.trefn);
     double *mt_s = sm + lay.mt, *ue_s = sm + lay.ue, *baseT_s = sm + lay.baseT, *baseP_s = sm + lay.baseP, *zmail_s = sm + lay.zmail;
     int *kacc_s = reinterpret_cast<int *>(sm + lay.kacc);
@@ -840,7 +839,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     // ---- pieces of the preparation, written for a group of `nt` threads with index `t`
     // coordinates, cc and the old gauge of block B -> shared (32 threads are enough); zeros beyond N
     auto load_raw = [&](int B, int t, int nt) {
-        const int b3 = B & 3;
+        const int b3 = B & 7;
         for (int e = t; e < 33; e += nt) {
             const int i = B * 32 + e;
             // beyond the last column the gauge continues flat: padded rows must stay finite (0 * inf = NaN would
@@ -867,124 +866,122 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         }
     };
     // gauges of block B (one warp, lane = row r): t_{r+1} from the old T, G_r = t_{r+1} - cc_r, the new
-    // gauge t~_{r+1} = G_r + cc_r exactly (float t + remainder dlt), the new T of column 32B+r+1
+    // gauge t~_{r+1} = G_r + cc_r exactly (float t + remainder dlt, kept as one double2 per column), the new T of
+    // column 32B+r+1
     auto gauges = [&](int B) {
-        const int b3 = B & 3, r = lane;
-        const double told = dd_diff(traw_s[b3 * 34 + r + 1], traw_s[b3 * 34]);
-        const double my_cc = cc_s[b3 * 32 + r];
+        const int b7 = B & 7, r = lane;
+        const double told = dd_diff(traw_s[b7 * 34 + r + 1], traw_s[b7 * 34]);
+        const double my_cc = cc_s[b7 * 32 + r];
         const float Gf = (float)(told - my_cc);
         const float tn = Gf + (float)my_cc;
         const double dl = ((double)Gf - (double)tn) + my_cc;
-        G_s[b3 * 32 + r] = (double)Gf;
-        ts_s[b3 * 40 + r + 1] = tn;
-        dlt_s[b3 * 40 + r + 1] = dl;
-        if (r == 0) { ts_s[b3 * 40] = 0.f; dlt_s[b3 * 40] = 0.0; }
-        const double2 Tn = dd_add_d(dd_add_d(trefn_s[b3], (double)tn), dl);
+        G_s[b7 * 32 + r] = (double)Gf;
+        colT_s[b7 * 34 + r + 1] = make_double2((double)tn, dl);
+        if (r == 0) colT_s[b7 * 34] = make_double2(0.0, 0.0);
+        const double2 Tn = dd_add_d(dd_add_d(trefn_s[b7], (double)tn), dl);
         ring_T[(B * 32 + r + 1) & (RB - 1)] = Tn;
-        if (r == 31) trefn_s[(B + 1) & 3] = Tn;
+        if (r == 31) trefn_s[(B + 1) & 7] = Tn;
     };
-    // M tile of block B: M[p][r] = exp(t~_p + tau[p][r] - G_r), p <= r (sx folded in for p >= 1)
-    // The exponent arguments of a batch of four entries are formed first, then the four exponentials, then the
-    // stores: written as a plain loop the compiler keeps the iterations in order (a shared-memory store of one
-    // might alias the loads of the next) and every entry pays its full ~250-cycle dependent chain.
-    auto build_M = [&](int B, int t, int nt) {
-        // only p <= r is needed: columns pp and 31-pp share one pass of 32 lanes (33 entries; the odd one,
-        // row 31 of column 31-pp, goes to a 17th pass); everything above the diagonal stays 0 from the start
-        const int b3 = B & 3;
-        double *mB = mt_s + (B & 1) * 1024;
-        for (int e0 = t; e0 < 17 * 32; e0 += 4 * nt) {
-            double arg[4];
-            int idx[4];
+    // What the helper warps prepare during window K, lane = row throughout (row data in registers, column data by
+    // broadcast loads, no shuffles), helper warp hw of 9 takes columns hw, hw+9, hw+18, hw+27 of every tile as one
+    // batch: four exponent arguments first, then four exponentials, then the stores:
+    //   M(B)[p][r]  = exp(t~_p + tau[p][r] - G_r), p <= r, sx folded in for p >= 1              (B = K+1)
+    //   base(B)     = sum over the columns of block B-q (q = 2..L) of Zhat exp(T - T_ref(B) + tau - G_r), one
+    //                 partial sum per (q, helper warp, row), in the frame of block B-q              (B = K+1)
+    //   E'(B)[p][r] = column p of block B-1 against row r of block B, relative to the new T of column 32B,
+    //                 scaled by exp(-G_r(B)), everything but the factor Zhat_p, sx folded in for p >= 1 (B = K+2)
+    auto helper_tasks = [&](int K, int hw) {
+        {   // ---- M(K+1)
+            const int B = K + 1, b7 = B & 7;
+            Vec<D> pr;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int e = e0 + j * nt;
-                const int pass = min(e >> 5, 16), l = e & 31;
-                int p, r;
-                if (pass < 16) {
-                    if (l >= pass) { p = pass; r = l; } else { p = 31 - pass; r = 31 - pass + l; }
-                } else {
-                    p = 31 - (l & 15); r = 31; // 16 leftovers (each written twice, same value)
-                }
-                Vec<D> pr, pc;
-#pragma unroll
-                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
-                arg[j] = (((double)ts_s[b3 * 40 + p] - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + dlt_s[b3 * 40 + p];
-                idx[j] = (e < 17 * 32) ? p * 32 + r : -1;
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) arg[j] = exp_cap_tab64(arg[j], etab64);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if constexpr (SGN) { if (idx[j] >= 32) arg[j] *= a.sx; }
-                if (idx[j] >= 0) mB[idx[j]] = arg[j];
-            }
-        }
-    };
-    // E'(B)[p][r]: column p of block B-1 against row r of block B, relative to the new T of column 32B,
-    // scaled by exp(-G_r(B)); everything but the factor Zhat_p (sx folded in for p >= 1)
-    auto build_ue = [&](int B, int t, int nt) {
-        const int b3 = B & 3, c3 = (B - 1) & 3;
-        double *uB = ue_s + (B & 1) * 1024;
-        const double t32 = (double)ts_s[c3 * 40 + 32], d32 = dlt_s[c3 * 40 + 32];
-        for (int e0 = t; e0 < 1024; e0 += 4 * nt) {
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
+            const double Gr = G_s[b7 * 32 + lane];
+            double *mB = mt_s + (B & 1) * 1024;
             double arg[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int e = min(e0 + j * nt, 1023);
-                const int p = e >> 5, r = e & 31;
-                Vec<D> pr, pc;
+            for (int k = 0; k < 4; ++k) {
+                const int p = min(hw + 9 * k, 31);
+                Vec<D> pc;
 #pragma unroll
-                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b3 * 32 + r) * D + c]; pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c]; }
-                arg[j] = ((((double)ts_s[c3 * 40 + p] - t32) - G_s[b3 * 32 + r]) - kk * dist2<D>(pr, pc)) + (dlt_s[c3 * 40 + p] - d32);
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c];
+                const double2 ct = colT_s[b7 * 34 + p];
+                arg[k] = ((ct.x - Gr) - kk * dist2<D>(pr, pc)) + ct.y;
             }
 #pragma unroll
-            for (int j = 0; j < 4; ++j) arg[j] = exp_cap_tab64(arg[j], etab64);
+            for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int e = e0 + j * nt;
-                if constexpr (SGN) { if (e >= 32) arg[j] *= a.sx; }
-                if (e < 1024) uB[e] = arg[j];
+            for (int k = 0; k < 4; ++k) {
+                const int p = hw + 9 * k;
+                if (p < 32) {
+                    double m = (p <= lane) ? arg[k] : 0.0;
+                    if constexpr (SGN) { if (p >= 1) m *= a.sx; }
+                    mB[p * 32 + lane] = m;
+                }
             }
         }
-    };
-    // contributions of the complete column block B-q (q = 2..L) to the rows of block B, scaled by exp(-G_r(B)),
-    // in the gauge as the gauges() chain wrote it: quarter `qt` (8 columns), lane = row.  One partial sum per
-    // (q, quarter, row); warp 0 rescales it by the power of two that separates the two blocks' frames.
-    auto build_base = [&](int B, int qt) {
-        const int b3 = B & 3, r = lane;
-        Vec<D> pr;
+        {   // ---- base(K+1)
+            const int B = K + 1, b7 = B & 7;
+            Vec<D> pr;
 #pragma unroll
-        for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b3 * 32 + r) * D + c];
-        const double2 TrefB = trefn_s[b3];
-        const double Gr = G_s[b3 * 32 + r];
-        for (int q = 2; q <= L; ++q) {
-            const int C = B - q;
-            double s0 = 0.0, s1 = 0.0;
-            if (C >= 0) {
-                double u[8];
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
+            const double Gr = G_s[b7 * 32 + lane];
+            const double2 TrefB = trefn_s[b7];
+            for (int q = 2; q <= L; ++q) {
+                const int C = B - q;
+                double sum = 0.0;
+                if (C >= 0) {
+                    double arg[4], z[4];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const int slot = (C * 32 + qt * 8 + k) & (RB - 1);
-                    Vec<D> pc;
+                    for (int k = 0; k < 4; ++k) {
+                        const int p = min(hw + 9 * k, 31), slot = (C * 32 + p) & (RB - 1);
+                        Vec<D> pc;
 #pragma unroll
-                    for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
-                    u[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
+                        for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
+                        arg[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
+                        z[k] = (hw + 9 * k < 32) ? ring_Z[slot] : 0.0;
+                    }
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                    sum = (z[0] * arg[0] + z[1] * arg[1]) + (z[2] * arg[2] + z[3] * arg[3]);
                 }
+                baseT_s[(((B & 1) * 2 + (q - 2)) * 9 + hw) * 32 + lane] = sum;
+            }
+        }
+        {   // ---- E'(K+2)
+            const int B = K + 2, b7 = B & 7, c7 = (B - 1) & 7;
+            Vec<D> pr;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) u[k] = exp_cap_tab64(u[k], etab64);
+            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
+            const double Gr = G_s[b7 * 32 + lane];
+            const double2 c32 = colT_s[c7 * 34 + 32];
+            double *uB = ue_s + (B & 1) * 1024;
+            double arg[4];
 #pragma unroll
-                for (int k = 0; k < 8; k += 2) {
-                    s0 = fma(ring_Z[(C * 32 + qt * 8 + k) & (RB - 1)], u[k], s0);
-                    s1 = fma(ring_Z[(C * 32 + qt * 8 + k + 1) & (RB - 1)], u[k + 1], s1);
+            for (int k = 0; k < 4; ++k) {
+                const int p = min(hw + 9 * k, 31);
+                Vec<D> pc;
+#pragma unroll
+                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c];
+                const double2 ct = colT_s[c7 * 34 + p];
+                arg[k] = (((ct.x - c32.x) - Gr) - kk * dist2<D>(pr, pc)) + (ct.y - c32.y);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int p = hw + 9 * k;
+                if (p < 32) {
+                    if constexpr (SGN) { if (p >= 1) arg[k] *= a.sx; }
+                    uB[p * 32 + lane] = arg[k];
                 }
             }
-            baseT_s[(((B & 1) * 2 + (q - 2)) * 4 + qt) * 32 + r] = s0 + s1;
         }
     };
     // the workers' panel of block B (columns < 32 (B-L), published relative to the T of column 32 (B-L)),
     // scaled like the rest; one warp, lane = row; waits for the workers
     auto fetch_panel = [&](int B) {
-        const int b3 = B & 3, jrec0 = 32 * (B - L);
+        const int b3 = B & 7, jrec0 = 32 * (B - L);
         double v = 0.0;
         if (jrec0 > 0 && B < NBk) {
             if (lane == 0) {
@@ -1002,25 +999,23 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     // 2^e as a double, 0 for e < -1000 (a contribution that far down is nothing), e <= 1000 assumed
     auto pow2i = [](int e) { return e < -1000 ? 0.0 : __hiloint2double((1023 + min(e, 1000)) << 20, 0); };
 
-    // ---- prologue: raw data of blocks 0..2, gauges of blocks 0 and 1, then the helpers' window "-1"
-    for (int B = 0; B < 3; ++B) load_raw(B, tid, CH_THREADS);
+    // ---- prologue: raw data of blocks 0..3, gauges of blocks 0..2, then the helpers' window "-1"
+    for (int B = 0; B < 4; ++B) load_raw(B, tid, CH_THREADS);
     if (tid == 0) {
         const double2 T0 = ldcg2(&g[0]);
         trefn_s[0] = T0;
         ring_T[0] = T0;
         ring_Z[0] = 1.0;
     }
-    __syncthreads();
-    if (warp == 0) gauges(0);
-    __syncthreads();
-    if (warp == 0) gauges(1);
-    for (int e = tid; e < 2 * 2 * 4 * 32; e += CH_THREADS) baseT_s[e] = 0.0;
-    for (int e = tid; e < 2 * 1024; e += CH_THREADS) mt_s[e] = 0.0;
+    for (int e = tid; e < 2 * 2 * 9 * 32; e += CH_THREADS) baseT_s[e] = 0.0;
     if (tid < 64) baseP_s[tid] = 0.0;
     if (tid < 8) kacc_s[tid] = 0;
-    build_M(0, tid, CH_THREADS);
+    for (int B = 0; B < 3; ++B) {
+        __syncthreads();
+        if (warp == 0) gauges(B);
+    }
     __syncthreads();
-    build_ue(1, tid, CH_THREADS);
+    if (warp < 9) helper_tasks(-1, warp);
 
     int bad = 0;                     // warp 0: status of its rows
     int kacc = 0;                    // warp 0: power of two taken out of Zhat up to the start of block K
@@ -1045,15 +1040,18 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const double *mK = mt_s + cur * 1024 + lane, *uN = ue_s + (cur ^ 1) * 1024 + lane;
             // earlier columns, each group brought from its own frame to this block's (exact powers of two);
             // all loads first, the frames of the last blocks are kept in registers (kh[q] = frame of block K-q)
-            const double *bq = baseT_s + (cur * 2 * 4) * 32 + lane;
-            const double b20 = bq[0], b21 = bq[32], b22 = bq[64], b23 = bq[96];
-            const double b30 = bq[128], b31 = bq[160], b32 = bq[192], b33 = bq[224];
+            const double *bq = baseT_s + (cur * 2 * 9) * 32 + lane;
+            double b2v[9], b3v[9];
+#pragma unroll
+            for (int k = 0; k < 9; ++k) { b2v[k] = bq[k * 32]; b3v[k] = bq[(9 + k) * 32]; }
+            const double b2s = (((b2v[0] + b2v[1]) + (b2v[2] + b2v[3])) + ((b2v[4] + b2v[5]) + (b2v[6] + b2v[7]))) + b2v[8];
+            const double b3s = (((b3v[0] + b3v[1]) + (b3v[2] + b3v[3])) + ((b3v[4] + b3v[5]) + (b3v[6] + b3v[7]))) + b3v[8];
             const double bp = baseP_s[cur * 32 + lane];
             double m_n = mK[0], u_n = uN[32];
             const double u0 = uN[0];
             double acc = acc_next * pow2i(kh1 - kacc);
-            if (K >= 2) acc = fma((b20 + b21) + (b22 + b23), pow2i(kh2 - kacc), acc);
-            if (L >= 3 && K >= 3) acc = fma((b30 + b31) + (b32 + b33), pow2i(kh3 - kacc), acc);
+            if (K >= 2) acc = fma(b2s, pow2i(kh2 - kacc), acc);
+            if (L >= 3 && K >= 3) acc = fma(b3s, pow2i(kh3 - kacc), acc);
             if (K - L - 1 >= 0) acc = fma(bp, pow2i((L == 1 ? kh2 : (L == 2 ? kh3 : kh4)) - kacc), acc);
             double zc = z0;
             acc_next = u0 * z0;
@@ -1090,8 +1088,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 }
             }
             if (K + 1 == NBk) {
-                fin_T = dd_add_d(dd_add_d(trefn_s[k3], (double)kacc * LN2.x), (double)kacc * LN2.y);
-                fin_G = G_s[k3 * 32 + lane];
+                fin_T = dd_add_d(dd_add_d(trefn_s[K & 7], (double)kacc * LN2.x), (double)kacc * LN2.y);
+                fin_G = G_s[(K & 7) * 32 + lane];
                 fin_acc = acc;
             }
             kh4 = kh3; kh3 = kh2; kh2 = kh1; kh1 = kacc;
@@ -1112,8 +1110,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
             }
         } else if (warp == CH_WARPS - 3) {
-            // raw data of block K+3
-            const int b3 = (K + 3) & 3, i = (K + 3) * 32 + lane;
+            // gauges of block K+3 (its raw data arrived during the previous window), then the raw data of block K+4
+            gauges(K + 3);
+            const int b3 = (K + 4) & 7, i = (K + 4) * 32 + lane;
             double2 told = make_double2(0.0, 0.0), told32 = told;
             Vec<D> pr, pc;
 #pragma unroll
@@ -1140,23 +1139,11 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[9] += clock64() - hc0;
         } else if ((warp & 3) != 0) {
             // 9 helper warps; the three that share warp 0's scheduler partition (4, 8, 12) stay out of its way
-            const int hw = warp - 1 - (warp >> 2), ht = hw * 32 + lane; // 0..8, 288 threads
-            const bool th = a.phase != nullptr && dir == 0 && lane == 0;
-            long long hc0 = clock64();
-            if (hw == 0) {
-                gauges(K + 2);
-            } else if (hw <= 4) {
-                build_M(K + 1, ht - 32, 4 * 32);
-            } else {
-                build_base(K + 1, hw - 5);
-            }
-            if (th && hw == 0) ph_s[4] += clock64() - hc0;
-            if (th && hw == 1) ph_s[5] += clock64() - hc0;
-            if (th && hw == 5) ph_s[6] += clock64() - hc0;
-            bar_sync_named(1, 9 * 32); // the gauges of block K+2 are in place
-            if (th && hw == 0) ph_s[7] += clock64() - hc0;
-            build_ue(K + 2, ht, 9 * 32);
-            if (th && hw == 0) ph_s[8] += clock64() - hc0;
+            const int hw = warp - 1 - (warp >> 2);
+            const bool th = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
+            const long long hc0 = clock64();
+            helper_tasks(K, hw);
+            if (th) ph_s[8] += clock64() - hc0;
         }
     }
     __syncthreads();
