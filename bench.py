@@ -106,8 +106,7 @@ def recursion_report(w, kern, phases, steps, clocks):
         per = [c / float(steps * nb) for c in phases[:10]]
         out["cycles_per_block"] = {"barrier_wait": per[0], "prologue": per[1], "dependent_steps_32": per[2], "epilogue": per[3],
                                    "sum": sum(per[:4]),
-                                   "helpers": {"gauges": per[4], "M_tile": per[5], "older_blocks": per[6], "inner_barrier": per[7],
-                                               "E_tile_done": per[8], "panel_fetched": per[9]}}
+                                   "helpers": {"tiles_prepared": per[8], "panel_fetched": per[9]}}
         out["floor_cycles_per_block"] = 32 * 38
         out["note"] = ("SM cycles of the forward chain CTA per 32-row block (clock64 inside k_chain_spec, the stale-gauge "
                        "kernel every timed step runs); floor = 32 x (SHFL + DFMA) from measured latencies; the block time is "

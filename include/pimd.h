@@ -154,9 +154,8 @@ int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
  * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation but the first after
  * pimd_set_state) fill
  *   [0] wait at the block barrier (the helper warps or the workers' panel are late), [1] the dependent warp's
- *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; helper warps, measured from the barrier:
- *   [4] gauges, [5] M tile, [6] older column blocks, [7] helpers' inner barrier reached, [8] E' tile done,
- *   [9] workers' panel fetched.
+ *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; measured from the barrier:
+ *   [8] a helper warp has prepared its share of the next blocks' tiles, [9] the workers' panel is fetched.
  * Evaluations with a fresh max-plus gauge (k_chain) fill [0] loop overhead, [2k-1] the dependent warp's own time
  * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish), [2k] its barrier wait. */
 int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host);

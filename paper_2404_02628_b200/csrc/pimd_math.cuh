@@ -126,7 +126,12 @@ PIMD_DEV double exp_neg_tab64(double r2, const double *tab)
 
 // exp(x) for any x through the same table: x is capped at 700 so that a wildly wrong exponent (a gauge that no
 // longer fits) gives ~1e304 and trips the caller's range check instead of wrapping the exponent field
-PIMD_DEV double exp_cap_tab64(double x, const double *tab) { return exp_neg_tab64(-fmin(x, 700.0), tab); }
+PIMD_DEV double exp_cap_tab64(double x, const double *tab)
+{
+    // x > 700 (or +NaN) -> 700, decided on the high word with integer compares (off the FP64 pipe)
+    const bool big = __double2hiint(x) > 0x4085e000;
+    return exp_neg_tab64(-__hiloint2double(big ? 0x4085e000 : __double2hiint(x), big ? 0 : __double2loint(x)), tab);
+}
 
 // ---------------------------------------------------------------------------------------------
 // double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
