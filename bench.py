@@ -159,7 +159,7 @@ def run_reference(args, w):
     if rank != 0:
         return 0
     budget = min(150.0, max(10.0, 0.6 * args.steps))
-    sps, n, dt = time_oracle(w, budget, max_steps=args.steps + args.warmup)
+    sps, n, dt = time_oracle(w, budget, max_steps=args.steps)
     line = {
         "impl": "reference", "metric": METRIC, "value": sps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 / sps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -1173,7 +1173,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
 }
 
 template <int D, bool SGN>
-__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw, const double *etab)
+__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw, const double *etab64)
 {
     const int N = a.N, LOOK = a.look;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -1236,14 +1236,14 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 cm = fmax(cm, tau[k]);
             }
             if (cm > acc.m) {
-                acc.s *= exp_tab(acc.m - cm, etab);
+                acc.s *= exp_neg_tab64(-(acc.m - cm), etab64);
                 acc.m = cm;
             }
             double s0 = 0.0, s1 = 0.0;
 #pragma unroll
             for (int k = 0; k < 8; k += 2) {
-                s0 = fma(exp_tab(tau[k] - acc.m, etab), st_sg[k], s0);
-                s1 = fma(exp_tab(tau[k + 1] - acc.m, etab), st_sg[k + 1], s1);
+                s0 = fma(exp_neg_tab64(-(tau[k] - acc.m), etab64), st_sg[k], s0);
+                s1 = fma(exp_neg_tab64(-(tau[k + 1] - acc.m), etab64), st_sg[k + 1], s1);
             }
             acc.s += s0 + s1;
             __syncwarp();
@@ -1273,7 +1273,7 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             for (int w = 0; w < CH_WARPS; ++w) t.m = fmax(t.m, mg_m[w * 32 + lane]);
             if (t.m > -INFINITY) {
 #pragma unroll
-                for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_tab(mg_m[w * 32 + lane] - t.m, etab), t.s);
+                for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_neg_tab64(-(mg_m[w * 32 + lane] - t.m), etab64), t.s);
             }
             if (i < N) {
                 a.p.pan_m[dir][i] = t.m;
@@ -1291,8 +1291,9 @@ template <int D, bool SGN>
 __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double etab[32]; // 2^(i/32) for exp_tab
+    __shared__ double etab[32], etab64[64]; // 2^(i/32), 2^(i/64)
     if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int dir = blockIdx.y;
     if (a.cond) {
@@ -1306,7 +1307,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
         cooperative_groups::this_grid().sync();
     }
     if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw, etab);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
 }
 
 // the recursion with the previous evaluation's gauge (see chain_cta_spec); same grid, same workers
@@ -1320,7 +1321,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
     __syncthreads();
     const int dir = blockIdx.y;
     if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, smem_raw, etab64);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
 }
 
 template <int D> size_t chain_spec_smem_bytes_host()
@@ -1347,8 +1348,8 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 {
     const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
     if (ct > rt) return;
-    __shared__ double etab[32];
-    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    __shared__ double etab64[64];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __shared__ double2 sg_g[FP_TB];
     __shared__ double sg_s[FP_TB];
     __shared__ double sg_sig[FP_TB * D];
@@ -1391,7 +1392,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
         const double2 gj = sg_g[k];
         const double kr2 = kk * dist2<D>(pr, pc);
-        const double w = exp_tab(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab) * sg_s[k];
+        const double w = exp_cap_tab64(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab64) * sg_s[k];
         sw += w;
         swc = fma(w, kr2, swc);
 #pragma unroll
