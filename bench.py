@@ -370,6 +370,33 @@ def run_ours(args, w):
                           "kernels_ms": {k: ms / n for k, (ms, n) in pr.items() if n}})
             s2.close()
         line["sweep"] = sweep
+    if world == 1 and not args.no_nxn:
+        # the paper's N x N intermediates, materialised on request (not on the hot path): HBM-write rooflines at N = 10000
+        wk = wl.WORKLOADS["cfg5_N10000"]
+        s3, _, _ = make_sim(wk, 0)
+        s3.forces(want_forces=False)
+        buf = torch.empty((wk.N, wk.N), dtype=torch.float64, device="cuda")
+        s3.set_profiling(True)
+        for _ in range(2):
+            s3.cycle_energies(out=buf)
+            s3.connection_probabilities(out=buf)
+        s3.get_profile()
+        reps = 5
+        for _ in range(reps):
+            flush.zero_()
+            s3.cycle_energies(out=buf)
+            flush.zero_()
+            s3.connection_probabilities(out=buf)
+        pr3 = s3.get_profile()
+        nbytes_nn = 8.0 * wk.N * wk.N
+        line["nxn_passes"] = {"workload": "cfg5_N10000", "bound": "hbm", "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
+                              "bytes_per_launch": nbytes_nn, "peak_source": peak_src}
+        for key, name in (("emat", "k_emat (cycle energies, Eq. 7-10)"), ("prmat", "k_prmat (connection probabilities, Eq. 12-14)")):
+            ms = pr3[key][0] / max(pr3[key][1], 1)
+            gbs = nbytes_nn / (ms * 1e-3) / 1e9
+            line["nxn_passes"][key] = {"kernel": name, "ms": ms, "achieved": gbs, "frac": gbs / peaks.get("hbm_gbs")}
+        del buf
+        s3.close()
     if world == 1 and not args.no_cpu:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_seconds)
     print(json.dumps(line))
@@ -389,6 +416,7 @@ def main():
     ap.add_argument("--sweep-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-nxn", action="store_true", help="skip the materialised N x N passes (0.8 GB at N=10000)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     args = ap.parse_args()
     from paper_2404_02628_b200 import workloads as wl

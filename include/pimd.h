@@ -115,6 +115,16 @@ int pimd_set_forces_host(pimd_t h, const double *f_host);
  *   pnext[l] = Pr[G(l) = l+1], l = 1..N stored at l-1 (N doubles; Eq. 13). */
 int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext);
 
+/* The paper's N x N intermediates, materialised on request into caller memory (DEVICE, N*N doubles, row-major;
+ * the hot path never stores them).  Both synchronise.  N <= 65535.
+ *   pimd_cycle_energies:            e[u*N + v] = E^{[u+1,v+1]} for u <= v (Eq. 7-10), 0 below the
+ *                                   diagonal; computed from the current positions alone.
+ *   pimd_connection_probabilities:  pr[l*N + m] = Pr[G(l+1) = m+1] (Eq. 12-14); signed
+ *                                   quasi-probabilities for xi < 0, the identity for xi = 0.  Uses the tables of the
+ *                                   last force evaluation at the current positions (evaluates first if there is none). */
+int pimd_cycle_energies(pimd_t h, double *e_dev);
+int pimd_connection_probabilities(pimd_t h, double *pr_dev);
+
 /* Advance nsteps MD steps (asynchronous on the stream):
  *   thermostat half step ; v += dt/2 F ; x += dt v ; F = F(x) ; v += dt/2 F ; thermostat half step
  * Forces of the starting state are evaluated first if they are not cached. */
@@ -146,7 +156,9 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_COMBINE 7   /* force output */
 #define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
 #define PIMD_PROF_CHAIN_FALLBACK 9 /* the max-plus recursion queued behind the stale-gauge one (returns at once if unused) */
-#define PIMD_PROF_NSLOTS 10
+#define PIMD_PROF_EMAT 10     /* pimd_cycle_energies: the N x N write */
+#define PIMD_PROF_PRMAT 11    /* pimd_connection_probabilities: the N x N write */
+#define PIMD_PROF_NSLOTS 12
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM

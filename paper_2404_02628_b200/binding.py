@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpimd.so")
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 THERMOSTAT_NVE, THERMOSTAT_LANGEVIN, THERMOSTAT_NHC = 0, 1, 2
 NHC_LENGTH = 4
-PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine", "pair", "chain_fallback")
+PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine", "pair", "chain_fallback", "emat", "prmat")
 
 # every symbol include/pimd.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
@@ -43,6 +43,8 @@ _SYMBOLS = {
     "pimd_set_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_forces_host": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_tables": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_cycle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_connection_probabilities": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_estimators": (C.c_int, [C.c_void_p, _dp, _dp, C.c_void_p, C.c_int, C.c_double]),
     "pimd_launch_count": (C.c_uint64, [C.c_void_p]),
@@ -218,6 +220,18 @@ class Pimd:
         pn = np.zeros(self.N)
         self._check(self._lib.pimd_get_tables(self._h, None, None, _ptr(pn)))
         return pn
+
+    def cycle_energies(self, out=None):
+        """E[u, v] = E^{[u+1,v+1]} (u <= v), device tensor [N][N]."""
+        e = out if out is not None else self._torch.empty((self.N, self.N), dtype=self._torch.float64, device="cuda")
+        self._check(self._lib.pimd_cycle_energies(self._h, _ptr(e)))
+        return e
+
+    def connection_probabilities(self, out=None):
+        """Pr[l, m] = Pr[G(l+1) = m+1], device tensor [N][N]."""
+        pr = out if out is not None else self._torch.empty((self.N, self.N), dtype=self._torch.float64, device="cuda")
+        self._check(self._lib.pimd_connection_probabilities(self._h, _ptr(pr)))
+        return pr
 
     def step(self, nsteps=1):
         self._check(self._lib.pimd_step(self._h, int(nsteps)))

@@ -43,7 +43,7 @@ struct pimd_s {
     unsigned char *ws;
     size_t ws_bytes;
     bool own_ws, carved;
-    double *x, *v, *F, *Fout, *nhc, *Fex1, *FexP, *ecpart, *hist;
+    double *x, *v, *F, *Fout, *nhc, *Fex1, *FexP, *ecpart, *hist, *Sarr, *Tarr;
     ExchPtrs ex;
     Scalars *scal;
     EstAccum *est;
@@ -54,6 +54,7 @@ struct pimd_s {
     EstAccum *h_est;
     int *h_status;
     bool forces_valid;
+    bool tables_valid; // the exchange tables (g, gs, pnext, rfin) belong to the current positions
     bool gauge_valid; // g/gs hold the (T, Zhat) of a completed evaluation of nearby positions
     bool use_spec;    // PIMD_NOSPEC=1 turns the stale-gauge kernel off
     size_t spec_smem;
@@ -154,6 +155,8 @@ size_t carve(pimd_t h, unsigned char *base)
     h->ex.tpart = (double *)take((size_t)h->nprep * 2 * 8);
     h->ex.rfin = (double2 *)take(2 * 16);
     h->ex.rsgn = (double *)take(2 * 8);
+    h->Sarr = (double *)take(N * 8);
+    h->Tarr = (double *)take(N * 8);
     h->phase = (unsigned long long *)take(16 * 8);
     h->status = (int *)take(4 * 4);
     h->ex.status = h->status;
@@ -347,6 +350,7 @@ int eval_forces(pimd_t h, bool scalars, bool est, int nbins, double rmax)
         CU(cudaStreamWaitEvent(h->s0, h->ev_join, 0));
     }
     h->forces_valid = true;
+    h->tables_valid = true;
     return PIMD_OK;
 }
 
@@ -388,6 +392,32 @@ bool finite_all(std::initializer_list<double> v)
 }
 
 } // namespace
+
+template <int D> static int cycle_energies_impl(pimd_t h, double *e_dev)
+{
+    int rc = launch_prep<D>(h, h->s0); // E_int, C(l,l+1), bead-1 / bead-P slices of the current positions
+    if (rc) return rc;
+    k_prefix_st<<<1, 1024, 0, h->s0>>>(h->N, h->beta, h->ex.eint, h->ex.cnext, h->Sarr, h->Tarr);
+    CU(cudaGetLastError());
+    const dim3 grid((h->N + 1023) / 1024, h->N);
+    {
+        ProfScope ps(h, PIMD_PROF_EMAT, h->s0);
+        k_emat<D><<<grid, 256, 0, h->s0>>>(h->N, h->ks, h->ex.rho[0], h->ex.sig[0], h->Sarr, h->Tarr, e_dev);
+    }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(h->s0));
+    return PIMD_OK;
+}
+
+template <int D> static int prmat_impl(pimd_t h, double *pr_dev)
+{
+    const dim3 grid((h->N + 1023) / 1024, h->N), gridp((h->N + 1023) / 1024, (h->N + PRMAT_ROWS - 1) / PRMAT_ROWS);
+    ProfScope ps(h, PIMD_PROF_PRMAT, h->s0);
+    if (h->xi == 0.0) k_identity<<<grid, 256, 0, h->s0>>>(h->N, pr_dev);
+    else if (h->xi < 0.0) k_prmat<D, true><<<gridp, 256, 0, h->s0>>>(h->N, h->kk, h->ex, pr_dev);
+    else k_prmat<D, false><<<gridp, 256, 0, h->s0>>>(h->N, h->kk, h->ex, pr_dev);
+    return PIMD_OK;
+}
 
 extern "C" {
 
@@ -542,6 +572,7 @@ static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpy
     if (h->thermostat == PIMD_THERMOSTAT_NHC) CU(cudaMemsetAsync(h->nhc, 0, h->ndof * 8 * PIMD_NHC_LENGTH, h->s0));
     CU(cudaMemsetAsync(h->status, 0, 4 * sizeof(int), h->s0));
     h->forces_valid = false;
+    h->tables_valid = false;
     // the exchange gauge of the last evaluation is kept: if the new positions are far from the old ones the
     // stale-gauge kernel notices and the max-plus kernel queued behind it takes over
     return PIMD_OK;
@@ -656,7 +687,7 @@ int pimd_forces_host(pimd_t h, double *f_host, double *vb, int *sign) { return f
 int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
 {
     if (!h) return PIMD_EINVAL;
-    if (!h->forces_valid) return fail(h, PIMD_EINVAL, "no force evaluation to report");
+    if (!h->tables_valid) return fail(h, PIMD_EINVAL, "no force evaluation to report");
     const int N = h->N;
     if (pnext) CU(cudaMemcpyAsync(pnext, h->ex.pnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
     if (vfwd || vbwd) {
@@ -710,6 +741,39 @@ int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
         CU(cudaStreamSynchronize(h->s0));
     }
     return PIMD_OK;
+}
+
+int pimd_cycle_energies(pimd_t h, double *e_dev)
+{
+    if (!h || !e_dev) return PIMD_EINVAL;
+    if (h->N > 65535) return fail(h, PIMD_EINVAL, "N x N output supported up to N = 65535");
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    switch (h->d) {
+    case 1: return cycle_energies_impl<1>(h, e_dev);
+    case 2: return cycle_energies_impl<2>(h, e_dev);
+    default: return cycle_energies_impl<3>(h, e_dev);
+    }
+}
+
+int pimd_connection_probabilities(pimd_t h, double *pr_dev)
+{
+    if (!h || !pr_dev) return PIMD_EINVAL;
+    if (h->N > 65535) return fail(h, PIMD_EINVAL, "N x N output supported up to N = 65535");
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    if (!h->tables_valid) {
+        rc = eval_forces(h, false, false, 0, 0.0);
+        if (rc) return rc;
+    }
+    switch (h->d) {
+    case 1: rc = prmat_impl<1>(h, pr_dev); break;
+    case 2: rc = prmat_impl<2>(h, pr_dev); break;
+    default: rc = prmat_impl<3>(h, pr_dev); break;
+    }
+    if (rc) return rc;
+    CU(cudaGetLastError());
+    return read_status(h);
 }
 
 int pimd_step(pimd_t h, int nsteps)

@@ -1475,6 +1475,122 @@ __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, double xi, Ex
     if (threadIdx.x == 0) ecpart[blockIdx.x] = s;
 }
 
+// ==========================================================================================
+// The paper's N x N intermediates, materialised on request (they are never needed by the hot path,
+// which recomputes their entries on the fly):
+//   k_emat   E^{[u,v]} = T[v] - S[u-1] + C[v][u], u <= v (Eq. 7-10)
+//   k_prmat  Pr[G(l) = l'] (Eq. 12-14) from the tables of a completed evaluation
+// Both are pure streaming writes of 8 N^2 bytes (inputs are O(N) and L2 resident): HBM-write bound.
+// One CTA per (row, 1024-column segment); consecutive threads write consecutive columns.
+// ==========================================================================================
+// S[v] = sum_{l<=v} (E_int[l] + C(l,l+1)), T[v] = S[v-1] + E_int[v] (0-based v); one block, any N
+__global__ void __launch_bounds__(1024) k_prefix_st(int N, double beta, const double *__restrict__ eint,
+                                                    const double *__restrict__ cnext_beta, double *__restrict__ S, double *__restrict__ T)
+{
+    __shared__ double wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int per = (N + 1023) / 1024, lo = tid * per, hi = min(N, lo + per);
+    double loc = 0.0;
+    for (int l = lo; l < hi; ++l) loc += eint[l] + cnext_beta[l] / beta;
+    double inc = loc; // inclusive scan of the per-thread sums
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double t = shfl_bcast(inc, max(lane - o, 0));
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        double w = wsum[lane], wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double t = shfl_bcast(wi, max(lane - o, 0));
+            if (lane >= o) wi += t;
+        }
+        wsum[lane] = wi - w; // exclusive
+    }
+    __syncthreads();
+    double run = wsum[warp] + (inc - loc); // sum of everything before this thread's segment
+    for (int l = lo; l < hi; ++l) {
+        T[l] = run + eint[l];
+        run += eint[l] + cnext_beta[l] / beta;
+        S[l] = run;
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(256) k_emat(int N, double ks, const double *__restrict__ xP /* rho[0] */,
+                                              const double *__restrict__ x1 /* sig[0] */, const double *__restrict__ S,
+                                              const double *__restrict__ T, double *__restrict__ E)
+{
+    const int u = blockIdx.y;
+    const int v0 = blockIdx.x * 1024 + threadIdx.x;
+    const Vec<D> r1 = ldvec<D>(x1, u);
+    const double Sm = (u > 0) ? S[u - 1] : 0.0;
+    double *row = E + (size_t)u * N;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int v = v0 + 256 * k;
+        if (v < N) {
+            double e = 0.0;
+            if (v >= u) e = (T[v] - Sm) + 0.5 * ks * dist2<D>(ldvec<D>(xP, v), r1);
+            __stcs(row + v, e);
+        }
+    }
+}
+
+constexpr int PRMAT_ROWS = 8; // rows per CTA: the column tables are read once and kept in registers for all of them
+
+template <int D, bool SGN>
+__global__ void __launch_bounds__(256) k_prmat(int N, double kk, ExchPtrs p, double *__restrict__ Pr)
+{
+    __shared__ double etab64[64];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __syncthreads();
+    const int l0 = blockIdx.y * PRMAT_ROWS;
+    const int c0 = blockIdx.x * 1024 + threadIdx.x;
+    if (c0 - threadIdx.x > l0 + PRMAT_ROWS) {
+        // the whole segment lies two or more above the diagonal of all these rows: zeros
+        for (int r = 0; r < PRMAT_ROWS && l0 + r < N; ++r) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int lp = c0 + 256 * k;
+                if (lp < N) __stcs(Pr + (size_t)(l0 + r) * N + lp, 0.0);
+            }
+        }
+        return;
+    }
+    double2 gj[4];
+    double zj[4];
+    Vec<D> sj[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int lp = min(c0 + 256 * k, N - 1);
+        gj[k] = p.g[0][lp];
+        zj[k] = p.gs[0][lp];
+        sj[k] = ldvec<D>(p.sig[0], lp);
+    }
+    for (int r = 0; r < PRMAT_ROWS; ++r) {
+        const int l = l0 + r;
+        if (l >= N) break;
+        const Vec<D> rP = ldvec<D>(p.rho[0], l);
+        const double2 A = dd_sub(p.g[1][N - 1 - l], p.rfin[0]);
+        double osg = p.gs[1][N - 1 - l];
+        if constexpr (SGN) osg *= p.rsgn[0];
+        const double pn = p.pnext[l];
+        double *row = Pr + (size_t)l * N;
+        double w[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            w[k] = exp_cap_tab64(((A.x + gj[k].x) + (A.y + gj[k].y)) - kk * dist2<D>(rP, sj[k]), etab64);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int lp = c0 + 256 * k;
+            if (lp < N) __stcs(row + lp, lp <= l ? osg * zj[k] * w[k] : (lp == l + 1 ? pn : 0.0));
+        }
+    }
+}
+
 // xi = 0 (0^0 = 1): only k = 1 survives in Eq. 6, Pr is the identity, every ring closes
 // on itself.  V = sum_l E^{[l,l]} + (1/beta) ln N!.
 template <int D, int TB>
@@ -1798,6 +1914,17 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
             atomicAdd(&est->upair, g * se);
             atomicAdd(&est->virpair, g * (se + sea));
         }
+    }
+}
+
+// Pr of distinguishable particles (xi = 0): the identity
+__global__ void __launch_bounds__(256) k_identity(int N, double *__restrict__ Pr)
+{
+    const int l = blockIdx.y, c0 = blockIdx.x * 1024 + threadIdx.x;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int lp = c0 + 256 * k;
+        if (lp < N) __stcs(Pr + (size_t)l * N + lp, lp == l ? 1.0 : 0.0);
     }
 }
 

@@ -353,3 +353,55 @@ def test_forces_round_trip_and_resume(binding, oracle):
     a.close(); b.close()
     assert relerr(xb.cpu().numpy(), xa2.cpu().numpy()) <= 1e-13
     assert relerr(vb_.cpu().numpy(), va2.cpu().numpy()) <= 1e-12
+
+
+@pytest.mark.parametrize("case", [(70, 6, 2, 2.5, 1.0), (133, 5, 3, 2.0, 0.5), (45, 4, 1, 2.0, -0.4), (33, 4, 2, 2.0, 0.0)],
+                         ids=["n70", "n133_d3", "n45_d1_neg", "n33_xi0"])
+def test_materialised_matrices_match_oracle(binding, oracle, case):
+    """pimd_cycle_energies (Eq. 7-10) and pimd_connection_probabilities (Eq. 12-14) against the oracle's
+    matrices, element by element; rows and columns of Pr sum to one."""
+    N, P, d, beta, xi = case
+    w = wl.custom(N, P, d=d, beta=beta, g=0.0, xi=xi, init="ring", sigma=1.0)
+    x, _ = wl.make_state(w, 8)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda())
+    E = sim.cycle_energies().cpu().numpy()
+    Pr = sim.connection_probabilities().cpu().numpy()
+    sim.close()
+    Eo = oracle.cycle_energies(x, beta)
+    assert np.all(np.tril(E, -1) == 0.0)
+    assert np.max(np.abs(E - np.triu(Eo))) <= 1e-10 * np.max(np.abs(Eo))
+    Pro = oracle.pr_matrix(x, beta, xi)
+    tol = 1e-9 if xi >= 0 else 1e-7
+    assert np.max(np.abs(Pr - Pro)) <= tol
+    np.testing.assert_allclose(Pr.sum(axis=1), 1.0, atol=10 * tol)
+    np.testing.assert_allclose(Pr.sum(axis=0), 1.0, atol=10 * tol)
+
+
+def test_materialised_matrices_full_size(binding):
+    """N = 10000 (0.8 GB each): every row and column of Pr sums to one, Pr is zero two above the diagonal;
+    E on the diagonal is the single-ring energy, E^{[u,v]} - E^{[u,v-1]} telescopes as Eq. 10 says for sampled entries."""
+    w = wl.WORKLOADS["cfg5_N10000"]
+    x, _ = wl.make_state(w, 0)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda())
+    Pr = sim.connection_probabilities()
+    rows, cols = Pr.sum(dim=1).cpu().numpy(), Pr.sum(dim=0).cpu().numpy()
+    assert np.max(np.abs(rows - 1.0)) <= 1e-9 and np.max(np.abs(cols - 1.0)) <= 1e-9
+    assert float(torch.triu(Pr, 2).abs().max()) == 0.0
+    del Pr
+    E = sim.cycle_energies()
+    sim.close()
+    ks = w.P / w.beta ** 2
+    ring = np.concatenate([x, x[:1]], axis=0)
+    e_self = 0.5 * ks * np.sum(np.diff(ring, axis=0) ** 2, axis=(0, 2))          # every particle closed on itself
+    assert np.max(np.abs(torch.diagonal(E).cpu().numpy() - e_self)) <= 1e-9 * np.max(e_self)
+    rng = np.random.default_rng(2)
+    for _ in range(50):
+        u = int(rng.integers(0, w.N - 1)); v = int(rng.integers(u + 1, w.N))
+        # Eq. 10: E^{[u,v]} = E^{[u,v-1]} - C(v-1,u) + C(v-1,v) + E_int(v) + C(v,u)
+        c = lambda a, b: 0.5 * ks * float(np.sum((x[w.P - 1, a] - x[0, b]) ** 2))
+        eint_v = 0.5 * ks * float(np.sum(np.diff(x[:, v], axis=0) ** 2))
+        lhs = float(E[u, v])
+        rhs = float(E[u, v - 1]) - c(v - 1, u) + c(v - 1, v) + eint_v + c(v, u)
+        assert abs(lhs - rhs) <= 1e-9 * abs(lhs)
