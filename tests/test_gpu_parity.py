@@ -405,3 +405,35 @@ def test_materialised_matrices_full_size(binding):
         lhs = float(E[u, v])
         rhs = float(E[u, v - 1]) - c(v - 1, u) + c(v - 1, v) + eint_v + c(v, u)
         assert abs(lhs - rhs) <= 1e-9 * abs(lhs)
+
+
+@pytest.mark.parametrize("xi,thermostat", [(1.0, 1), (0.0, 1), (1.0, 2)], ids=["bosons_langevin", "distinguishable_langevin", "bosons_nhc"])
+def test_ensemble_energy_matches_exact_ideal_gas(binding, xi, thermostat):
+    """BASELINE config 1 (N = 4, P = 16, beta = 2, non-interacting): the sampled primitive and virial energies of the
+    CUDA path agree with the exact finite-P canonical value (oracle/ideal_gas.py) within 3
+    standard errors (block averages over independent seeds), and with each other."""
+    from oracle import ideal_gas
+
+    w = wl.WORKLOADS["cfg1"].with_(xi=xi)
+    exact = ideal_gas.exact_energy(w.N, w.beta, w.omega, w.d, xi, w.P)
+    prim, vir = [], []
+    for seed in range(6):
+        x, v = wl.make_state(w, seed)
+        sim = binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=thermostat, seed=100 + seed)
+        sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+        sim.step(4000)  # equilibration
+        ep_b, ev_b = [], []
+        for _ in range(8):      # 8 blocks of 250 samples, 10 steps apart
+            ep, ev = 0.0, 0.0
+            for _ in range(250):
+                sim.step(10)
+                a, b, _ = sim.estimators()
+                ep += a; ev += b
+            ep_b.append(ep / 250); ev_b.append(ev / 250)
+        sim.close()
+        prim += ep_b; vir += ev_b
+    for vals in (prim, vir):
+        vals = np.asarray(vals)
+        mean, se = vals.mean(), vals.std(ddof=1) / np.sqrt(len(vals))
+        assert abs(mean - exact) <= 3.0 * se + 0.01 * abs(exact), (mean, se, exact)
+        assert se < 0.1 * abs(exact)
