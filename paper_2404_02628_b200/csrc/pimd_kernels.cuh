@@ -786,6 +786,12 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 // raises status[2]; the host always queues the max-plus kernel behind this one, and that kernel returns at
 // once unless the flag is set.
 // ==========================================================================================
+#ifndef PIMD_SPEC_NHW
+#define PIMD_SPEC_NHW 9
+#endif
+constexpr int SPEC_NHW = PIMD_SPEC_NHW;                     // helper warps of the stale-gauge chain CTA: 9 or 12
+constexpr int SPEC_NCOL = (32 + SPEC_NHW - 1) / SPEC_NHW;  // columns of a tile per helper warp
+
 template <int D> struct SpecSmem {
     int RB;
     size_t ringT, ringZ, ringSig, rho, cc, traw, colT, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, total;
@@ -804,7 +810,7 @@ template <int D> struct SpecSmem {
         trefn = o; o += 8 * 2;        // new T of column 32B (double-double)
         mt = o; o += 2 * 1024;        // M tiles of blocks B & 1
         ue = o; o += 2 * 1024;        // E'(B & 1)
-        baseT = o; o += 2 * 2 * 9 * 32; // [B & 1][q - 2][helper warp][row] partial sums of the older column blocks
+        baseT = o; o += 2 * 2 * SPEC_NHW * 32; // [B & 1][q - 2][helper warp][row] partial sums of the older column blocks
         baseP = o; o += 2 * 32;       // scaled panel for block B & 1
         zmail = o; o += 2 * 32;       // Zhat of the columns block B & 1 produced, for the io warp
         kacc = o; o += 4;             // int[8]: power of two taken out of Zhat up to the start of block B & 7
@@ -898,10 +904,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
             const double Gr = G_s[b7 * 32 + lane];
             double *mB = mt_s + (B & 1) * 1024;
-            double arg[4];
+            double arg[SPEC_NCOL];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int p = min(hw + 9 * k, 31);
+            for (int k = 0; k < SPEC_NCOL; ++k) {
+                const int p = min(hw + SPEC_NHW * k, 31);
                 Vec<D> pc;
 #pragma unroll
                 for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c];
@@ -909,10 +915,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 arg[k] = ((ct.x - Gr) - kk * dist2<D>(pr, pc)) + ct.y;
             }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+            for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int p = hw + 9 * k;
+            for (int k = 0; k < SPEC_NCOL; ++k) {
+                const int p = hw + SPEC_NHW * k;
                 if (p < 32) {
                     double m = (p <= lane) ? arg[k] : 0.0;
                     if constexpr (SGN) { if (p >= 1) m *= a.sx; }
@@ -931,21 +937,22 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 const int C = B - q;
                 double sum = 0.0;
                 if (C >= 0) {
-                    double arg[4], z[4];
+                    double arg[SPEC_NCOL], z[SPEC_NCOL];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const int p = min(hw + 9 * k, 31), slot = (C * 32 + p) & (RB - 1);
+                    for (int k = 0; k < SPEC_NCOL; ++k) {
+                        const int p = min(hw + SPEC_NHW * k, 31), slot = (C * 32 + p) & (RB - 1);
                         Vec<D> pc;
 #pragma unroll
                         for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
                         arg[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
-                        z[k] = (hw + 9 * k < 32) ? ring_Z[slot] : 0.0;
+                        z[k] = (hw + SPEC_NHW * k < 32) ? ring_Z[slot] : 0.0;
                     }
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
-                    sum = (z[0] * arg[0] + z[1] * arg[1]) + (z[2] * arg[2] + z[3] * arg[3]);
+                    for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+#pragma unroll
+                    for (int k = 0; k < SPEC_NCOL; ++k) sum = fma(z[k], arg[k], sum);
                 }
-                baseT_s[(((B & 1) * 2 + (q - 2)) * 9 + hw) * 32 + lane] = sum;
+                baseT_s[(((B & 1) * 2 + (q - 2)) * SPEC_NHW + hw) * 32 + lane] = sum;
             }
         }
         {   // ---- E'(K+2)
@@ -956,10 +963,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const double Gr = G_s[b7 * 32 + lane];
             const double2 c32 = colT_s[c7 * 34 + 32];
             double *uB = ue_s + (B & 1) * 1024;
-            double arg[4];
+            double arg[SPEC_NCOL];
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int p = min(hw + 9 * k, 31);
+            for (int k = 0; k < SPEC_NCOL; ++k) {
+                const int p = min(hw + SPEC_NHW * k, 31);
                 Vec<D> pc;
 #pragma unroll
                 for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c];
@@ -967,10 +974,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 arg[k] = (((ct.x - c32.x) - Gr) - kk * dist2<D>(pr, pc)) + (ct.y - c32.y);
             }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+            for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int p = hw + 9 * k;
+            for (int k = 0; k < SPEC_NCOL; ++k) {
+                const int p = hw + SPEC_NHW * k;
                 if (p < 32) {
                     if constexpr (SGN) { if (p >= 1) arg[k] *= a.sx; }
                     uB[p * 32 + lane] = arg[k];
@@ -1007,7 +1014,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         ring_T[0] = T0;
         ring_Z[0] = 1.0;
     }
-    for (int e = tid; e < 2 * 2 * 9 * 32; e += CH_THREADS) baseT_s[e] = 0.0;
+    for (int e = tid; e < 2 * 2 * SPEC_NHW * 32; e += CH_THREADS) baseT_s[e] = 0.0;
     if (tid < 64) baseP_s[tid] = 0.0;
     if (tid < 8) kacc_s[tid] = 0;
     for (int B = 0; B < 3; ++B) {
@@ -1015,7 +1022,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         if (warp == 0) gauges(B);
     }
     __syncthreads();
-    if (warp < 9) helper_tasks(-1, warp);
+    if (warp < SPEC_NHW) helper_tasks(-1, warp);
 
     int bad = 0;                     // warp 0: status of its rows
     int kacc = 0;                    // warp 0: power of two taken out of Zhat up to the start of block K
@@ -1040,12 +1047,16 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const double *mK = mt_s + cur * 1024 + lane, *uN = ue_s + (cur ^ 1) * 1024 + lane;
             // earlier columns, each group brought from its own frame to this block's (exact powers of two);
             // all loads first, the frames of the last blocks are kept in registers (kh[q] = frame of block K-q)
-            const double *bq = baseT_s + (cur * 2 * 9) * 32 + lane;
-            double b2v[9], b3v[9];
+            const double *bq = baseT_s + (cur * 2 * SPEC_NHW) * 32 + lane;
+            double b2s = 0.0, b3s = 0.0, b2t = 0.0, b3t = 0.0; // loads are independent, two add chains each
 #pragma unroll
-            for (int k = 0; k < 9; ++k) { b2v[k] = bq[k * 32]; b3v[k] = bq[(9 + k) * 32]; }
-            const double b2s = (((b2v[0] + b2v[1]) + (b2v[2] + b2v[3])) + ((b2v[4] + b2v[5]) + (b2v[6] + b2v[7]))) + b2v[8];
-            const double b3s = (((b3v[0] + b3v[1]) + (b3v[2] + b3v[3])) + ((b3v[4] + b3v[5]) + (b3v[6] + b3v[7]))) + b3v[8];
+            for (int k = 0; k < SPEC_NHW; k += 2) {
+                b2s += bq[k * 32];
+                b3s += bq[(SPEC_NHW + k) * 32];
+                if (k + 1 < SPEC_NHW) { b2t += bq[(k + 1) * 32]; b3t += bq[(SPEC_NHW + k + 1) * 32]; }
+            }
+            b2s += b2t;
+            b3s += b3t;
             const double bp = baseP_s[cur * 32 + lane];
             double m_n = mK[0], u_n = uN[32];
             const double u0 = uN[0];
@@ -1137,9 +1148,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             long long hc0 = clock64();
             fetch_panel(K + 1);
             if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[9] += clock64() - hc0;
-        } else if ((warp & 3) != 0) {
-            // 9 helper warps; the three that share warp 0's scheduler partition (4, 8, 12) stay out of its way
-            const int hw = warp - 1 - (warp >> 2);
+        } else if (SPEC_NHW == 12 || (warp & 3) != 0) {
+            // helper warps: with SPEC_NHW = 9 the three that share warp 0's scheduler partition (4, 8, 12) stay idle
+            const int hw = (SPEC_NHW == 12) ? warp - 1 : warp - 1 - (warp >> 2);
             const bool th = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
             const long long hc0 = clock64();
             helper_tasks(K, hw);
