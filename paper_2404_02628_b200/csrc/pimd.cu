@@ -20,7 +20,7 @@ namespace {
 thread_local char g_create_error[512] = "";
 
 constexpr int BEAD_TB = 128;
-constexpr int PREP_TB = 128;
+constexpr int PREP_TB = 64;
 constexpr int ASM_TB = 128;
 constexpr int MAX_BINS = 1 << 16;
 
@@ -239,7 +239,7 @@ template <int D> int launch_prep(pimd_t h, cudaStream_t st)
 {
     {
         ProfScope ps(h, PIMD_PROF_PREP, st);
-        k_prep<D, PREP_TB><<<h->nprep, PREP_TB, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
+        k_prep<D, PREP_TB><<<h->nprep, PREP_TB * PREP_SPLIT, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
     }
     CU(cudaGetLastError());
     return PIMD_OK;

@@ -222,23 +222,39 @@ struct ExchPtrs {
     int *status;
 };
 
+constexpr int PREP_SPLIT = 4; // thread groups that share the bead loop of a particle
+
 template <int D, int TB>
-__global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N, int P, int NB, double ks, double kk,
-                                            double lambda, ExchPtrs p)
+__global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restrict__ x, int N, int P, int NB, double ks, double kk,
+                                                        double lambda, ExchPtrs p)
 {
-    __shared__ double red[TB / 32];
-    const int l = blockIdx.x * TB + threadIdx.x;
-    double e_int = 0.0, cn = 0.0;
-    if (l < N) {
-        const size_t sl = (size_t)N * D;
-        Vec<D> prev = ldvec<D>(x, l);
-        const Vec<D> x1 = prev;
-        double acc = 0.0;
-        for (int j = 1; j < P; ++j) {
-            Vec<D> cur = ldvec<D>(x + (size_t)j * sl, l);
-            acc += dist2<D>(cur, prev);
-            prev = cur;
+    __shared__ double red[TB * PREP_SPLIT / 32];
+    __shared__ double part_s[PREP_SPLIT][TB];
+    const int lt = threadIdx.x % TB, part = threadIdx.x / TB;
+    const int l = blockIdx.x * TB + lt;
+    const size_t sl = (size_t)N * D;
+    {
+        // the P-1 bead differences of particle l, in PREP_SPLIT contiguous segments
+        const int per = (P - 1 + PREP_SPLIT - 1) / PREP_SPLIT, j0 = 1 + part * per, j1 = min(P, j0 + per);
+        double accp = 0.0;
+        if (l < N && j0 < j1) {
+            Vec<D> prev = ldvec<D>(x + (size_t)(j0 - 1) * sl, l);
+            for (int j = j0; j < j1; ++j) {
+                Vec<D> cur = ldvec<D>(x + (size_t)j * sl, l);
+                accp += dist2<D>(cur, prev);
+                prev = cur;
+            }
         }
+        part_s[part][lt] = accp;
+    }
+    __syncthreads();
+    double e_int = 0.0, cn = 0.0;
+    if (part == 0 && l < N) {
+        double acc = 0.0;
+#pragma unroll
+        for (int q = 0; q < PREP_SPLIT; ++q) acc += part_s[q][lt];
+        const Vec<D> x1 = ldvec<D>(x, l);
+        const Vec<D> prev = ldvec<D>(x + (size_t)(P - 1) * sl, l);
         const Vec<D> xP = prev;
         e_int = 0.5 * ks * acc;
         stvec<D>(p.rho[0], l, xP);
@@ -284,8 +300,8 @@ __global__ void __launch_bounds__(TB) k_prep(const double *__restrict__ x, int N
             p.status[2] = 0;
         }
     }
-    double s1 = block_sum<TB>(e_int, red);
-    double s2 = block_sum<TB>(cn, red);
+    double s1 = block_sum<TB * PREP_SPLIT>(e_int, red);
+    double s2 = block_sum<TB * PREP_SPLIT>(cn, red);
     if (threadIdx.x == 0) {
         p.tpart[2 * blockIdx.x] = s1;
         p.tpart[2 * blockIdx.x + 1] = s2;
