@@ -28,6 +28,9 @@
  *     stream) and on one internal helper stream that is fork/joined to it with events.  Calls that
  *     return host scalars synchronise that stream; pimd_step() is asynchronous.
  *   - One handle is not thread-safe; different handles are independent.
+ *   - Environment knobs read by pimd_create() (tuning / debugging only): PIMD_LOOK (column blocks kept inside the
+ *     chain CTA, 1..3), PIMD_WORKERS (panel worker CTAs per direction), PIMD_NOSPEC=1 (always run the max-plus
+ *     recursion kernel, never the stale-gauge one), PIMD_PAIR_CH (tile offsets per pair-kernel task).
  *   - There is no CPU fallback: without a CUDA device pimd_create() fails with PIMD_ECUDA.
  */
 #ifndef PIMD_H

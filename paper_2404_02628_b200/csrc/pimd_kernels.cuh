@@ -856,7 +856,6 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     double2 *g = a.p.g[dir];
     double *gs = a.p.gs[dir];
     const double kk = a.kk;
-    const bool is_io = (warp == CH_WARPS - 1);
 
     // ---- pieces of the preparation, written for a group of `nt` threads with index `t`
     // coordinates, cc and the old gauge of block B -> shared (32 threads are enough); zeros beyond N
@@ -1057,7 +1056,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     for (int K = 0; K < NBk; ++K) {
         __syncthreads(); // everything block K needs is ready; everything of block K-1 has been consumed
         PH(0);
-        const int i0 = K * 32, cur = K & 1, k3 = K & 3;
+        const int i0 = K * 32, cur = K & 1;
         const int nrows = min(32, N - i0);
         if (warp == 0) {
             const double *mK = mt_s + cur * 1024 + lane, *uN = ue_s + (cur ^ 1) * 1024 + lane;
