@@ -310,7 +310,11 @@ def test_stale_gauge_evaluations_match_oracle(binding, oracle):
         (wl.custom(333, 8, d=2, beta=3.0, g=0.2, xi=1.0, init="ring", sigma=2.0), 0.01, 1.0, 1e-9),
         (wl.custom(200, 8, d=3, beta=2.0, g=0.1, xi=0.5, init="iid", sigma=0.8), 0.01, 1.0, 1e-9),
         (wl.custom(150, 8, d=2, beta=3.0, g=0.2, xi=-0.5, init="ring", sigma=3.0), 0.01, 1.0, 1e-7),
-        (wl.custom(333, 8, d=2, beta=3.0, g=0.0, xi=1.0, init="ring", sigma=2.0), 1.0, 30.0, 1e-9),  # jump: fallback
+        (wl.custom(333, 8, d=2, beta=3.0, g=0.0, xi=1.0, init="ring", sigma=2.0), 1.0, 30.0, 1e-9),  # jump: fallback        (wl.custom(1, 4, d=2, beta=2.0, g=0.0, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),      # one block, one row
+        (wl.custom(2, 4, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),
+        (wl.custom(33, 6, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),     # ragged second block
+        (wl.custom(64, 6, d=1, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),
+        (wl.custom(129, 6, d=2, beta=2.0, g=0.0, xi=-1.0, init="ring", sigma=2.0), 0.01, 1.0, 1e-7),  # fermionic weights
     ]
     for w, dt, vscale, tol in cases:
         x, v = wl.make_state(w, 9)
