@@ -30,7 +30,8 @@
  *   - One handle is not thread-safe; different handles are independent.
  *   - Environment knobs read by pimd_create() (tuning / debugging only): PIMD_LOOK (column blocks kept inside the
  *     chain CTA, 1..3), PIMD_WORKERS (panel worker CTAs per direction), PIMD_NOSPEC=1 (always run the max-plus
- *     recursion kernel, never the stale-gauge one), PIMD_PAIR_CH (tile offsets per pair-kernel task).
+ *     recursion kernel, never the stale-gauge one), PIMD_PAIR_CH (tile offsets per pair-kernel task), PIMD_GRAPH=0
+ *     (pimd_step launches every kernel itself instead of replaying a captured CUDA graph).
  *   - There is no CPU fallback: without a CUDA device pimd_create() fails with PIMD_ECUDA.
  */
 #ifndef PIMD_H
@@ -130,7 +131,8 @@ int pimd_connection_probabilities(pimd_t h, double *pr_dev);
 
 /* Advance nsteps MD steps (asynchronous on the stream):
  *   thermostat half step ; v += dt/2 F ; x += dt v ; F = F(x) ; v += dt/2 F ; thermostat half step
- * Forces of the starting state are evaluated first if they are not cached. */
+ * Forces of the starting state are evaluated first if they are not cached.  For nsteps >= 3 (profiling off) all
+ * but the last step replay one captured CUDA graph on an internal stream that is event-ordered with the caller's. */
 int pimd_step(pimd_t h, int nsteps);
 
 /* Estimators at the current positions (R9, R15), HOST outputs:

@@ -49,6 +49,13 @@ struct pimd_s {
     EstAccum *est;
     int *status;
     unsigned long long *phase; // chain phase clock (profiling)
+    unsigned long long *dstep; // MD step counter on the device (graph replay)
+    // one MD step (force evaluation, then close + open) captured as a CUDA graph on an internal stream
+    cudaStream_t sg;
+    cudaEvent_t ev_gin, ev_gout;
+    cudaGraphExec_t gexec;
+    bool use_graph, graph_failed, graph_conc;
+    uint64_t graph_launches;
     // pinned host mirrors
     Scalars *h_scal;
     EstAccum *h_est;
@@ -158,6 +165,7 @@ size_t carve(pimd_t h, unsigned char *base)
     h->Sarr = (double *)take(N * 8);
     h->Tarr = (double *)take(N * 8);
     h->phase = (unsigned long long *)take(16 * 8);
+    h->dstep = (unsigned long long *)take(8);
     h->status = (int *)take(4 * 4);
     h->ex.status = h->status;
     h->ecpart = (double *)take((size_t)h->nasm * 8);
@@ -354,15 +362,16 @@ int eval_forces(pimd_t h, bool scalars, bool est, int nbins, double rmax)
     return PIMD_OK;
 }
 
-int launch_integrate(pimd_t h, bool do_close, bool do_open, uint64_t step_close, uint64_t step_open)
+int launch_integrate(pimd_t h, bool do_close, bool do_open, uint64_t step_close, uint64_t step_open, bool device_counter = false)
 {
+    const unsigned long long *dstep = device_counter ? h->dstep : nullptr;
     const double c1 = std::exp(-h->gamma * h->dt * 0.5);
     const double c2 = std::sqrt((1.0 - c1 * c1) / h->beta);
     const double Q = h->beta / (double)h->P;
     const unsigned grid = (unsigned)((h->ndof + 255) / 256);
 #define LI(T) \
     k_integrate<T><<<grid, 256, 0, h->s0>>>(h->x, h->v, h->F, h->Fex1, h->FexP, h->nhc, h->ndof, h->slice, h->P, h->dt, c1, c2, \
-                                            h->beta, Q, h->seed, step_close, step_open, do_close ? 1 : 0, do_open ? 1 : 0, h->status)
+                                            h->beta, Q, h->seed, step_close, step_open, do_close ? 1 : 0, do_open ? 1 : 0, h->status, dstep)
     {
         ProfScope ps(h, PIMD_PROF_INTEGRATE, h->s0);
         if (h->thermostat == PIMD_THERMOSTAT_LANGEVIN) LI(1);
@@ -392,6 +401,48 @@ bool finite_all(std::initializer_list<double> v)
 }
 
 } // namespace
+
+// Capture "force evaluation ; close step s + open step s+1 ; counter += 1" once, on an internal stream (the caller's
+// stream may be the legacy default stream, which cannot be captured).  Any failure (e.g. a driver that cannot put a
+// cooperative launch into a graph) switches the feature off for this handle; nothing else depends on it.
+static int ensure_graph(pimd_t h)
+{
+    if (h->gexec && h->graph_conc == h->concurrent) return PIMD_OK;
+    if (h->graph_failed) return PIMD_ECUDA;
+    if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    cudaStream_t user = h->s0;
+    const uint64_t l0 = h->launches;
+    const bool fv = h->forces_valid, tv = h->tables_valid;
+    cudaGraph_t graph = nullptr;
+    int rc = PIMD_OK;
+    if (cudaStreamBeginCapture(h->sg, cudaStreamCaptureModeRelaxed) != cudaSuccess) rc = PIMD_ECUDA;
+    if (rc == PIMD_OK) {
+        h->s0 = h->sg;
+        rc = eval_forces(h, false, false, 0, 0.0);
+        if (rc == PIMD_OK) rc = launch_integrate(h, true, true, 0, 0, true);
+        if (rc == PIMD_OK) {
+            k_step_counter<<<1, 32, 0, h->sg>>>(h->dstep, 0ull, 1);
+            h->launches++;
+            if (cudaGetLastError() != cudaSuccess) rc = PIMD_ECUDA;
+        }
+        h->s0 = user;
+        if (cudaStreamEndCapture(h->sg, &graph) != cudaSuccess || !graph) rc = PIMD_ECUDA;
+    }
+    if (rc == PIMD_OK && cudaGraphInstantiate(&h->gexec, graph, 0) != cudaSuccess) rc = PIMD_ECUDA;
+    if (graph) cudaGraphDestroy(graph);
+    h->graph_launches = h->launches - l0;
+    h->launches = l0;
+    h->forces_valid = fv;
+    h->tables_valid = tv;
+    if (rc != PIMD_OK) {
+        cudaGetLastError();
+        h->gexec = nullptr;
+        h->graph_failed = true;
+        return PIMD_ECUDA;
+    }
+    h->graph_conc = h->concurrent;
+    return PIMD_OK;
+}
 
 template <int D> static int cycle_energies_impl(pimd_t h, double *e_dev)
 {
@@ -461,6 +512,7 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
         if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;
     }
     h->concurrent = true;
+    h->use_graph = !(std::getenv("PIMD_GRAPH") && std::atoi(std::getenv("PIMD_GRAPH")) == 0);
     h->gauge_valid = false;
     h->use_spec = !(std::getenv("PIMD_NOSPEC") && std::atoi(std::getenv("PIMD_NOSPEC")) != 0);
     h->prof_ev = new std::vector<cudaEvent_t>();
@@ -489,6 +541,9 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
         if (want > 0 && h->nworkers < 1) return bail(fail(h, PIMD_ECUDA, "not enough co-resident CTAs for the recursion"));
     }
     if (cudaStreamCreateWithFlags(&h->s1, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&h->sg, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_gin, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_gout, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess ||
         cudaMallocHost((void **)&h->h_scal, sizeof(Scalars)) != cudaSuccess ||
@@ -504,6 +559,10 @@ int pimd_destroy(pimd_t h)
     if (!h) return PIMD_OK;
     if (h->s0 || h->s1) cudaDeviceSynchronize();
     if (h->own_ws && h->ws) cudaFree(h->ws);
+    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    if (h->sg) cudaStreamDestroy(h->sg);
+    if (h->ev_gin) cudaEventDestroy(h->ev_gin);
+    if (h->ev_gout) cudaEventDestroy(h->ev_gout);
     if (h->s1) cudaStreamDestroy(h->s1);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
@@ -790,7 +849,24 @@ int pimd_step(pimd_t h, int nsteps)
     // open step s ; forces ; [close s + open s+1] ; forces ; ... ; close last
     rc = launch_integrate(h, false, true, 0, h->step);
     if (rc) return rc;
-    for (int it = 0; it < nsteps; ++it) {
+    int it = 0;
+    const bool gauge_ok = h->gauge_valid || h->xi == 0.0;
+    if (h->use_graph && !h->profiling && gauge_ok && nsteps >= 3 && ensure_graph(h) == PIMD_OK) {
+        // all but the last step replay the captured graph; the step counter of the noise lives on the device meanwhile
+        k_step_counter<<<1, 32, 0, h->s0>>>(h->dstep, (unsigned long long)h->step, 0);
+        CU(cudaGetLastError());
+        CU(cudaEventRecord(h->ev_gin, h->s0));
+        CU(cudaStreamWaitEvent(h->sg, h->ev_gin, 0));
+        for (; it < nsteps - 1; ++it) {
+            CU(cudaGraphLaunch(h->gexec, h->sg));
+            h->launches += h->graph_launches;
+            h->step++;
+        }
+        CU(cudaEventRecord(h->ev_gout, h->sg));
+        CU(cudaStreamWaitEvent(h->s0, h->ev_gout, 0));
+        h->forces_valid = false; // set again below
+    }
+    for (; it < nsteps; ++it) {
         rc = eval_forces(h, false, false, 0, 0.0);
         if (rc) return rc;
         const bool last = it == nsteps - 1;

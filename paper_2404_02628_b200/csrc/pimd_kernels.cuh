@@ -1713,10 +1713,13 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
                                                   double *__restrict__ nhc, size_t ndof, size_t slice /* N*d */, int P,
                                                   double dt, double c1, double c2, double beta, double Q, uint64_t seed,
                                                   uint64_t step_close, uint64_t step_open, int do_close, int do_open,
-                                                  int *status)
+                                                  int *status, const unsigned long long *dstep)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= ndof) return;
+    // step counter kept on the device when launches are replayed from a CUDA graph (no per-step arguments there)
+    [[maybe_unused]] const uint64_t s_close = dstep ? *dstep : step_close;
+    [[maybe_unused]] const uint64_t s_open = dstep ? *dstep + (do_close ? 1 : 0) : step_open;
     const size_t j = idx / slice, rem = idx - j * slice;
     double f = F[idx];
     if (j == 0) f += Fex1[rem];
@@ -1732,7 +1735,7 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
         vi = fma(hdt, f, vi);
         if constexpr (THERMO == 1) {
             double z0, z1;
-            philox_normal(seed, idx, step_close, z0, z1);
+            philox_normal(seed, idx, s_close, z0, z1);
             vi = c1 * vi + c2 * z1;
         } else if constexpr (THERMO == 2) {
             nhc_half(vi, vx, hdt, 1.0 / beta, Q);
@@ -1741,7 +1744,7 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
     if (do_open) {
         if constexpr (THERMO == 1) {
             double z0, z1;
-            philox_normal(seed, idx, step_open, z0, z1);
+            philox_normal(seed, idx, s_open, z0, z1);
             vi = c1 * vi + c2 * z0;
         } else if constexpr (THERMO == 2) {
             nhc_half(vi, vx, hdt, 1.0 / beta, Q);
@@ -1952,6 +1955,11 @@ __global__ void __launch_bounds__(256) k_identity(int N, double *__restrict__ Pr
         const int lp = c0 + 256 * k;
         if (lp < N) __stcs(Pr + (size_t)l * N + lp, lp == l ? 1.0 : 0.0);
     }
+}
+
+__global__ void k_step_counter(unsigned long long *dstep, unsigned long long set, int add)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) *dstep = add ? *dstep + 1 : set;
 }
 
 __global__ void k_zero(double *p, size_t n)
