@@ -168,8 +168,8 @@ int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM
  * cycles per phase of its 32-row blocks (HOST out, 16 entries, accumulated since the previous call, then reset).
- * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation but the first after
- * pimd_set_state) fill
+ * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation of a handle but its
+ * first) fill
  *   [0] wait at the block barrier (the helper warps or the workers' panel are late), [1] the dependent warp's
  *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; measured from the barrier:
  *   [8] a helper warp has prepared its share of the next blocks' tiles, [9] the workers' panel is fetched.
