@@ -840,6 +840,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     int N = a.N, L = a.look, NBk = a.NB;
     asm volatile("" : "+r"(N), "+r"(L), "+r"(NBk));
     const SpecSmem<D> lay;
+    __shared__ long long ph_s[16]; // phase clock (profiling)
     constexpr int RB = 256;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     double *sm = reinterpret_cast<double *>(smem_raw);
@@ -911,7 +912,15 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     //                 partial sum per (q, helper warp, row), in the frame of block B-q              (B = K+1)
     //   E'(B)[p][r] = column p of block B-1 against row r of block B, relative to the new T of column 32B,
     //                 scaled by exp(-G_r(B)), everything but the factor Zhat_p, sx folded in for p >= 1 (B = K+2)
+    auto batch_is_live = [&](const double *arg) {
+        bool live = false;
+#pragma unroll
+        for (int k = 0; k < SPEC_NCOL; ++k) live = live || !(arg[k] < -64.0); // NaN counts as live
+        return __any_sync(0xffffffffu, live) != 0;
+    };
     auto helper_tasks = [&](int K, int hw) {
+        const bool tht = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
+        const long long ht0 = clock64();
         {   // ---- M(K+1)
             const int B = K + 1, b7 = B & 7;
             Vec<D> pr;
@@ -929,8 +938,16 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 const double2 ct = colT_s[b7 * 34 + p];
                 arg[k] = ((ct.x - Gr) - kk * dist2<D>(pr, pc)) + ct.y;
             }
+            // entries below e^-64 of the row's gauge are nothing (the sums they enter are O(1) in that gauge, give or
+            // take the drift of a stale gauge): when a whole batch is that small -- the usual case for blocks of
+            // particles that are not neighbours in space -- the exponentials are skipped (warp-uniform)
+            if (batch_is_live(arg)) {
 #pragma unroll
-            for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+            } else {
+#pragma unroll
+                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = 0.0;
+            }
 #pragma unroll
             for (int k = 0; k < SPEC_NCOL; ++k) {
                 const int p = hw + SPEC_NHW * k;
@@ -941,6 +958,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 }
             }
         }
+        if (tht) ph_s[4] += clock64() - ht0;
         {   // ---- base(K+1)
             const int B = K + 1, b7 = B & 7;
             Vec<D> pr;
@@ -962,14 +980,20 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                         arg[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
                         z[k] = (hw + SPEC_NHW * k < 32) ? ring_Z[slot] : 0.0;
                     }
+                    if (batch_is_live(arg)) {
 #pragma unroll
-                    for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                        for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = 0.0;
+                    }
 #pragma unroll
                     for (int k = 0; k < SPEC_NCOL; ++k) sum = fma(z[k], arg[k], sum);
                 }
                 baseT_s[(((B & 1) * 2 + (q - 2)) * SPEC_NHW + hw) * 32 + lane] = sum;
             }
         }
+        if (tht) ph_s[5] += clock64() - ht0;
         {   // ---- E'(K+2)
             const int B = K + 2, b7 = B & 7, c7 = (B - 1) & 7;
             Vec<D> pr;
@@ -988,8 +1012,16 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 const double2 ct = colT_s[c7 * 34 + p];
                 arg[k] = (((ct.x - c32.x) - Gr) - kk * dist2<D>(pr, pc)) + (ct.y - c32.y);
             }
+            // entries below e^-64 of the row's gauge are nothing (the sums they enter are O(1) in that gauge, give or
+            // take the drift of a stale gauge): when a whole batch is that small -- the usual case for blocks of
+            // particles that are not neighbours in space -- the exponentials are skipped (warp-uniform)
+            if (batch_is_live(arg)) {
 #pragma unroll
-            for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+            } else {
+#pragma unroll
+                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = 0.0;
+            }
 #pragma unroll
             for (int k = 0; k < SPEC_NCOL; ++k) {
                 const int p = hw + SPEC_NHW * k;
@@ -1047,7 +1079,6 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     double fin_G = 0.0, fin_acc = 1.0;
     const double2 LN2 = make_double2(0.6931471805599453, 2.3190468138462996e-17);
 
-    __shared__ long long ph_s[16];
     const bool tim = a.phase != nullptr && dir == 0 && tid == 0;
     if (tid < 16) ph_s[tid] = 0;
     long long tprev = clock64();
