@@ -527,11 +527,13 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     if (rc) return bail(rc);
     {
         // Panel workers per direction.  A worker spins while it waits for columns and owns a whole SM,
-        // so only as many as the panel work needs are launched: at ~7e3 cycles per 32-row block of the
-        // chain one SM keeps up with ~16 column tiles per block.
+        // so only as many as the panel work needs are launched.
         const int want = h->NB - h->look - 1;
         int cap = h->coop_max_blocks / 2 - 1;
-        int need = (h->NB + 7) / 8;
+        // A worker needs about 480 NB cycles for its last row blocks and gets nworkers x (one chain block, about 3000
+        // cycles) for each, so NB/5 workers keep the panels ahead of the chain; when the pair kernel dominates the step
+        // (g != 0 and P N large: its work over the chain's grows like P N) the SMs are worth more there and NB/8 is enough.
+        int need = (h->g != 0.0 && (long long)h->P * h->N > 80000) ? (h->NB + 7) / 8 : (h->NB + 4) / 5;
         if (const char *e = std::getenv("PIMD_WORKERS")) {
             const int v = std::atoi(e);
             if (v >= 1) need = v;

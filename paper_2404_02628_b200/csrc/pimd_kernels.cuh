@@ -61,6 +61,19 @@ PIMD_DEV void st_release(int *p, int v)
 }
 PIMD_DEV double2 ldcg2(const double2 *p) { return __ldcg(p); }
 PIMD_DEV double ldcg1(const double *p) { return __ldcg(p); }
+// A value that is its own "ready" flag: the consumer spins on the 8-byte word until it no longer holds this quiet-NaN
+// payload (no arithmetic produces it); 8-byte accesses are single-copy atomic, so no fence and no second round trip.
+constexpr unsigned long long PAN_EMPTY = 0x7ff8dead00c0ffeeull;
+PIMD_DEV unsigned long long ld_relaxed_u64(const double *p)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.b64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+PIMD_DEV void st_relaxed_f64(double *p, double v)
+{
+    asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+}
 
 // status word bits (device -> host)
 enum { ST_NONFINITE = 1, ST_NODE = 2 };
@@ -277,6 +290,11 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
             p.acc[1][(size_t)l * (D + 2) + c] = 0.0;
         }
         if (l < NB) { p.panel_ready[0][l] = 0; p.panel_ready[1][l] = 0; }
+#pragma unroll
+        for (int dir = 0; dir < 2; ++dir) { // k_chain_spec reads the panel words as their own flags
+            reinterpret_cast<unsigned long long *>(p.pan_m[dir])[l] = PAN_EMPTY;
+            reinterpret_cast<unsigned long long *>(p.pan_s[dir])[l] = PAN_EMPTY;
+        }
         // refresh the gauge the previous evaluation left behind: (T, Zhat) -> (T + k ln2, Zhat 2^-k) with
         // |Zhat 2^-k| in [1, 2), so that T tracks the solution from step to step (k_chain_spec)
 #pragma unroll
@@ -921,40 +939,36 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     auto helper_tasks = [&](int K, int hw) {
         const bool tht = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
         const long long ht0 = clock64();
-        {   // ---- M(K+1)
+        {   // ---- M(K+1): only p <= r is needed, so columns pp and 31-pp share one pass of 32 lanes (33 entries; the
+            // odd one, row 31 of column 31-pp, goes to a 17th pass); above the diagonal the tile stays 0 from the start.
+            // Helper warp hw takes passes hw and hw + 9.
             const int B = K + 1, b7 = B & 7;
-            Vec<D> pr;
-#pragma unroll
-            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
-            const double Gr = G_s[b7 * 32 + lane];
             double *mB = mt_s + (B & 1) * 1024;
-            double arg[SPEC_NCOL];
+            double arg[2];
+            int idx[2];
 #pragma unroll
-            for (int k = 0; k < SPEC_NCOL; ++k) {
-                const int p = min(hw + SPEC_NHW * k, 31);
-                Vec<D> pc;
+            for (int k = 0; k < 2; ++k) {
+                const int pass = hw + SPEC_NHW * k;
+                int p, r;
+                if (pass < 16) {
+                    if (lane >= pass) { p = pass; r = lane; } else { p = 31 - pass; r = 31 - pass + lane; }
+                } else {
+                    p = 31 - (lane & 15); r = 31; // 16 leftovers (each written twice, same value)
+                }
+                Vec<D> pr, pc;
 #pragma unroll
-                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c];
+                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b7 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
                 const double2 ct = colT_s[b7 * 34 + p];
-                arg[k] = ((ct.x - Gr) - kk * dist2<D>(pr, pc)) + ct.y;
-            }
-            // entries below e^-64 of the row's gauge are nothing (the sums they enter are O(1) in that gauge, give or
-            // take the drift of a stale gauge): when a whole batch is that small -- the usual case for blocks of
-            // particles that are not neighbours in space -- the exponentials are skipped (warp-uniform)
-            if (batch_is_live(arg)) {
-#pragma unroll
-                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
-            } else {
-#pragma unroll
-                for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = 0.0;
+                arg[k] = ((ct.x - G_s[b7 * 32 + r]) - kk * dist2<D>(pr, pc)) + ct.y;
+                idx[k] = (pass <= 16) ? p * 32 + r : -1;
             }
 #pragma unroll
-            for (int k = 0; k < SPEC_NCOL; ++k) {
-                const int p = hw + SPEC_NHW * k;
-                if (p < 32) {
-                    double m = (p <= lane) ? arg[k] : 0.0;
-                    if constexpr (SGN) { if (p >= 1) m *= a.sx; }
-                    mB[p * 32 + lane] = m;
+            for (int k = 0; k < 2; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (idx[k] >= 0) {
+                    if constexpr (SGN) { if (idx[k] >= 32) arg[k] *= a.sx; }
+                    mB[idx[k]] = arg[k];
                 }
             }
         }
@@ -1038,14 +1052,20 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         const int b3 = B & 7, jrec0 = 32 * (B - L);
         double v = 0.0;
         if (jrec0 > 0 && B < NBk) {
-            if (lane == 0) {
-                while (ld_acquire(&a.p.panel_ready[dir][B]) == 0) { }
-            }
-            __syncwarp();
             const int i = B * 32 + lane;
             if (i < N) {
-                const double m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0 & (RB - 1)], trefn_s[b3]);
-                v = ldcg1(&a.p.pan_s[dir][i]) * exp_cap_tab64(m - G_s[b3 * 32 + lane], etab64);
+                const double shift = dd_diff(ring_T[jrec0 & (RB - 1)], trefn_s[b3]) - G_s[b3 * 32 + lane];
+                unsigned long long um, us;
+                int npoll = 0;
+                const long long tp0 = clock64();
+                do { // each lane waits for its own row (k_prep emptied the words, the worker fills them)
+                    um = ld_relaxed_u64(&a.p.pan_m[dir][i]);
+                    us = ld_relaxed_u64(&a.p.pan_s[dir][i]);
+                    if (npoll == 0 && lane == 0 && a.phase != nullptr && dir == 0) ph_s[11] += clock64() - tp0;
+                    ++npoll;
+                } while (um == PAN_EMPTY || us == PAN_EMPTY);
+                if (lane == 0 && a.phase != nullptr && dir == 0) { ph_s[10] += npoll; ph_s[12] += clock64() - tp0; }
+                v = __longlong_as_double((long long)us) * exp_cap_tab64(__longlong_as_double((long long)um) + shift, etab64);
             }
         }
         baseP_s[(B & 1) * 32 + lane] = v;
@@ -1062,6 +1082,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         ring_Z[0] = 1.0;
     }
     for (int e = tid; e < 2 * 2 * SPEC_NHW * 32; e += CH_THREADS) baseT_s[e] = 0.0;
+    for (int e = tid; e < 2 * 1024; e += CH_THREADS) mt_s[e] = 0.0;
     if (tid < 64) baseP_s[tid] = 0.0;
     if (tid < 8) kacc_s[tid] = 0;
     for (int B = 0; B < 3; ++B) {
@@ -1153,6 +1174,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             kacc += kstep;
             PH(3);
         } else if (warp == CH_WARPS - 1) {
+            const long long hcp = clock64();
             if (K > 0) { // publish the columns block K-1 produced, in its frame (column N is kept too: its T is
                          // the last row's gauge next time)
                 const int jn = i0 - 32 + lane + 1;
@@ -1166,8 +1188,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 __syncwarp();
                 if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
             }
+            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[7] += clock64() - hcp;
         } else if (warp == CH_WARPS - 3) {
             // gauges of block K+3 (its raw data arrived during the previous window), then the raw data of block K+4
+            const long long hcg = clock64();
             gauges(K + 3);
             const int b3 = (K + 4) & 7, i = (K + 4) * 32 + lane;
             double2 told = make_double2(0.0, 0.0), told32 = told;
@@ -1190,6 +1214,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 ring_sig[(i & (RB - 1)) * D + c] = pc.v[c];
             }
             cc_s[b3 * 32 + lane] = c0;
+            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[15] += clock64() - hcg;
         } else if (warp == CH_WARPS - 2) {
             long long hc0 = clock64();
             fetch_panel(K + 1);
@@ -1201,6 +1226,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const long long hc0 = clock64();
             helper_tasks(K, hw);
             if (th) ph_s[8] += clock64() - hc0;
+            if (a.phase != nullptr && dir == 0 && lane == 0 && hw == 4) ph_s[13] += clock64() - hc0;
+            if (a.phase != nullptr && dir == 0 && lane == 0 && hw == 8) ph_s[14] += clock64() - hc0;
         }
     }
     __syncthreads();
@@ -1279,12 +1306,20 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             }
             return known_ready >= need;
         };
+        // lane 8 of a warp that takes a chunk of the newest tile also fetches column 32 ntile, the reference the
+        // panel is published against (cols_ready is 32 K' + 1 or N, so that column came with the same publication)
+        double2 pub_pre = make_double2(0.0, 0.0);
+        bool have_pub = false;
         auto load_cols = [&](int c8) {
             if (lane < 8) {
                 const int j = 8 * c8 + lane;
                 pre_g = ldcg2(&g[j]);
                 pre_z = ldcg1(&gs[j]);
                 pre_c = ldvec<D>(sig, j);
+            }
+            if ((c8 >> 2) == ntile - 1) {
+                if (lane == 8) pub_pre = ldcg2(&g[32 * ntile]);
+                have_pub = true;
             }
         };
         for (int c8 = warp; c8 < 4 * ntile; c8 += CH_WARPS) {
@@ -1329,7 +1364,10 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             __syncwarp();
         }
         // common reference of the published partial: g_{32 ntile} (first "recent" column of block K)
-        {
+        if (have_pub) {
+            const double2 pub = make_double2(shfl_bcast(pub_pre.x, 8), shfl_bcast(pub_pre.y, 8));
+            lse_shift(acc, dd_diff(ref, pub));
+        } else {
             const int need = 32 * ntile + 1;
             if (known_ready < need) {
                 if (lane == 0) {
@@ -1356,8 +1394,8 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_neg_tab64(-(mg_m[w * 32 + lane] - t.m), etab64), t.s);
             }
             if (i < N) {
-                a.p.pan_m[dir][i] = t.m;
-                a.p.pan_s[dir][i] = t.s;
+                st_relaxed_f64(&a.p.pan_m[dir][i], t.m);
+                st_relaxed_f64(&a.p.pan_s[dir][i], t.s);
             }
             // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
             __syncwarp();
