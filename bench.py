@@ -104,10 +104,12 @@ def recursion_report(w, kern, phases, steps, clocks):
            "bound": "latency", "fallback_ms": kern.get("chain_fallback", {}).get("ms_avg"),
            "ms": ch, "ns_per_row": (ch * 1e6 / w.N if ch else None), "rows_per_block": 32}
     if ch and sum(phases[:4]) > 0:
-        per = [c / float(steps * nb) for c in phases[:10]]
+        per = [c / float(steps * nb) for c in phases[:16]]
         out["cycles_per_block"] = {"barrier_wait": per[0], "prologue": per[1], "dependent_steps_32": per[2], "epilogue": per[3],
                                    "sum": sum(per[:4]),
-                                   "helpers": {"tiles_prepared": per[8], "panel_fetched": per[9]}}
+                                   "helpers": {"m_tile": per[4], "older_blocks": per[5], "tiles_prepared": per[8],
+                                               "columns_published": per[7], "panel_fetched": per[9],
+                                               "panel_reads_per_block": per[10], "tables_and_prefetch": per[15]}}
         out["floor_cycles_per_block"] = 32 * 38
         out["note"] = ("SM cycles of the forward chain CTA per 32-row block (clock64 inside k_chain_spec, the stale-gauge "
                        "kernel every timed step runs); floor = 32 x (SHFL + DFMA) from measured latencies; the block time is "

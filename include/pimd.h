@@ -171,8 +171,11 @@ int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
  * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation of a handle but its
  * first) fill
  *   [0] wait at the block barrier (the helper warps or the workers' panel are late), [1] the dependent warp's
- *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; measured from the barrier:
- *   [8] a helper warp has prepared its share of the next blocks' tiles, [9] the workers' panel is fetched.
+ *   prologue, [2] its 32 dependent steps (DFMA + SHFL), [3] its epilogue; measured from the barrier, one warp each:
+ *   [4] a helper warp has its share of the next M tile, [5] of the older column blocks too, [8] of everything
+ *   ([13], [14]: two more helper warps, on the other scheduler partitions), [7] the last block's columns are published,
+ *   [9] the workers' panel is fetched ([10]: reads of the panel words it took, one per block = it never waited),
+ *   [15] gauges, exponent tables and prefetch of the blocks ahead are in place.
  * Evaluations with a fresh max-plus gauge (k_chain) fill [0] loop overhead, [2k-1] the dependent warp's own time
  * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish), [2k] its barrier wait. */
 int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host);

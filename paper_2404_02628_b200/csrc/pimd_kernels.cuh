@@ -828,7 +828,7 @@ constexpr int SPEC_NCOL = (32 + SPEC_NHW - 1) / SPEC_NHW;  // columns of a tile 
 
 template <int D> struct SpecSmem {
     int RB;
-    size_t ringT, ringZ, ringSig, rho, cc, traw, colT, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, total;
+    size_t ringT, ringZ, ringSig, rho, cc, traw, colT, Gs, trefn, mt, ue, baseT, baseP, zmail, kacc, ctab, rtab, total;
     __host__ __device__ SpecSmem()
     {
         RB = 256;
@@ -848,6 +848,8 @@ template <int D> struct SpecSmem {
         baseP = o; o += 2 * 32;       // scaled panel for block B & 1
         zmail = o; o += 2 * 32;       // Zhat of the columns block B & 1 produced, for the io warp
         kacc = o; o += 4;             // int[8]: power of two taken out of Zhat up to the start of block B & 7
+        ctab = o; o += 2 * 4 * 32 * (1 + D); // [window & 1][set][column]: (A_p, sigma'_p), see col_row_terms
+        rtab = o; o += 2 * 2 * 32 * (1 + D); // [window & 1][set][row]: (B_r, 2 kk rho'_r)
         total = o;
     }
 };
@@ -870,6 +872,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     double2 *trefn_s = reinterpret_cast<double2 *>(sm + lay.trefn);
     double *mt_s = sm + lay.mt, *ue_s = sm + lay.ue, *baseT_s = sm + lay.baseT, *baseP_s = sm + lay.baseP, *zmail_s = sm + lay.zmail;
     int *kacc_s = reinterpret_cast<int *>(sm + lay.kacc);
+    double *ctab_s = sm + lay.ctab, *rtab_s = sm + lay.rtab;
 
     const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
     double2 *g = a.p.g[dir];
@@ -930,6 +933,60 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     //                 partial sum per (q, helper warp, row), in the frame of block B-q              (B = K+1)
     //   E'(B)[p][r] = column p of block B-1 against row r of block B, relative to the new T of column 32B,
     //                 scaled by exp(-G_r(B)), everything but the factor Zhat_p, sx folded in for p >= 1 (B = K+2)
+    // Exponent arguments in three FP64 instructions per entry.  With an origin o (row 0 of the row block, so that every
+    // term stays of the size of the distances themselves) and rho' = rho_r - o, sigma' = sigma_p - o,
+    //     (column term) - G_r - kk |rho_r - sigma_p|^2 = A_p + B_r + sum_c (2 kk rho'_c) sigma'_c,
+    //     A_p = (column term) - kk |sigma'_p|^2,   B_r = -G_r - kk |rho'_r|^2.
+    // One warp tabulates, during window K, what the helpers use during window K+1 (lane = column / row):
+    //   rows    set 0: block K+2 (M and base of block K+2),          set 1: block K+3 (E'(K+3))
+    //   columns set 0: block K+2 for M(K+2), origin o(K+2)            set 1: block K+2 for E'(K+3), origin o(K+3)
+    //           set 2, 3: blocks K, K-1 for base(K+2), origin o(K+2)
+    auto col_row_terms = [&](int K) {
+        constexpr int W = 1 + D;
+        double *cA = ctab_s + (K & 1) * (4 * 32 * W), *rA = rtab_s + (K & 1) * (2 * 32 * W);
+        const int B2 = K + 2, B3 = K + 3, b2 = B2 & 7, b3 = B3 & 7;
+        Vec<D> o2, o3;
+#pragma unroll
+        for (int c = 0; c < D; ++c) { o2.v[c] = rho_s[(b2 * 32) * D + c]; o3.v[c] = rho_s[(b3 * 32) * D + c]; }
+#pragma unroll
+        for (int set = 0; set < 2; ++set) {
+            const int b = set ? b3 : b2;
+            double n2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                const double rp = rho_s[(b * 32 + lane) * D + c] - (set ? o3.v[c] : o2.v[c]);
+                n2 = fma(rp, rp, n2);
+                rA[(set * 32 + lane) * W + 1 + c] = 2.0 * kk * rp;
+            }
+            rA[(set * 32 + lane) * W] = fma(-kk, n2, -G_s[b * 32 + lane]);
+        }
+        const double2 ct = colT_s[b2 * 34 + lane], c32 = colT_s[b2 * 34 + 32], Tref2 = trefn_s[b2];
+#pragma unroll
+        for (int set = 0; set < 4; ++set) {
+            const int C = (set < 2) ? B2 : B2 - set; // column block
+            if (C < 0) continue;
+            const int slot = (C * 32 + lane) & (RB - 1);
+            double t;
+            if (set == 0) t = ct.x + ct.y;
+            else if (set == 1) t = (ct.x - c32.x) + (ct.y - c32.y);
+            else t = dd_diff(ring_T[slot], Tref2);
+            double n2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                const double sp = ring_sig[slot * D + c] - (set == 1 ? o3.v[c] : o2.v[c]);
+                n2 = fma(sp, sp, n2);
+                cA[(set * 32 + lane) * W + 1 + c] = sp;
+            }
+            cA[(set * 32 + lane) * W] = fma(-kk, n2, t);
+        }
+    };
+    // A_p + B_r + sum_c w_c sigma'_c for one entry (cp, rp point at the column's and the row's table entries)
+    auto entry_arg = [&](const double *cp, const double *rp) {
+        double t = cp[0] + rp[0];
+#pragma unroll
+        for (int c = 0; c < D; ++c) t = fma(rp[1 + c], cp[1 + c], t);
+        return t;
+    };
     auto batch_is_live = [&](const double *arg) {
         bool live = false;
 #pragma unroll
@@ -942,8 +999,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         {   // ---- M(K+1): only p <= r is needed, so columns pp and 31-pp share one pass of 32 lanes (33 entries; the
             // odd one, row 31 of column 31-pp, goes to a 17th pass); above the diagonal the tile stays 0 from the start.
             // Helper warp hw takes passes hw and hw + 9.
-            const int B = K + 1, b7 = B & 7;
+            const int B = K + 1;
             double *mB = mt_s + (B & 1) * 1024;
+            const double *cA = ctab_s + ((K + 1) & 1) * (4 * 32 * (1 + D)), *rA = rtab_s + ((K + 1) & 1) * (2 * 32 * (1 + D));
             double arg[2];
             int idx[2];
 #pragma unroll
@@ -955,11 +1013,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 } else {
                     p = 31 - (lane & 15); r = 31; // 16 leftovers (each written twice, same value)
                 }
-                Vec<D> pr, pc;
-#pragma unroll
-                for (int c = 0; c < D; ++c) { pr.v[c] = rho_s[(b7 * 32 + r) * D + c]; pc.v[c] = ring_sig[((B * 32 + p) & (RB - 1)) * D + c]; }
-                const double2 ct = colT_s[b7 * 34 + p];
-                arg[k] = ((ct.x - G_s[b7 * 32 + r]) - kk * dist2<D>(pr, pc)) + ct.y;
+                arg[k] = entry_arg(cA + p * (1 + D), rA + r * (1 + D));
                 idx[k] = (pass <= 16) ? p * 32 + r : -1;
             }
 #pragma unroll
@@ -974,57 +1028,61 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         }
         if (tht) ph_s[4] += clock64() - ht0;
         {   // ---- base(K+1)
-            const int B = K + 1, b7 = B & 7;
-            Vec<D> pr;
+            const int B = K + 1;
+            const double *cA = ctab_s + ((K + 1) & 1) * (4 * 32 * (1 + D)), *rA = rtab_s + ((K + 1) & 1) * (2 * 32 * (1 + D));
+            double rt[1 + D];
 #pragma unroll
-            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
-            const double Gr = G_s[b7 * 32 + lane];
-            const double2 TrefB = trefn_s[b7];
-            for (int q = 2; q <= L; ++q) {
-                const int C = B - q;
-                double sum = 0.0;
-                if (C >= 0) {
-                    double arg[SPEC_NCOL], z[SPEC_NCOL];
+            for (int c = 0; c < 1 + D; ++c) rt[c] = rA[lane * (1 + D) + c];
+            // both older column blocks as one batch, so that eight independent exponentials are in flight
+            double arg[2][SPEC_NCOL], z[2][SPEC_NCOL];
 #pragma unroll
-                    for (int k = 0; k < SPEC_NCOL; ++k) {
-                        const int p = min(hw + SPEC_NHW * k, 31), slot = (C * 32 + p) & (RB - 1);
-                        Vec<D> pc;
+            for (int qq = 0; qq < 2; ++qq) {
+                const int q = 2 + qq, C = B - q;
+                const bool valid = q <= L && C >= 0;
 #pragma unroll
-                        for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[slot * D + c];
-                        arg[k] = (dd_diff(ring_T[slot], TrefB) - Gr) - kk * dist2<D>(pr, pc);
-                        z[k] = (hw + SPEC_NHW * k < 32) ? ring_Z[slot] : 0.0;
-                    }
-                    if (batch_is_live(arg)) {
+                for (int k = 0; k < SPEC_NCOL; ++k) {
+                    const int p = min(hw + SPEC_NHW * k, 31), slot = (C * 32 + p) & (RB - 1);
+                    arg[qq][k] = valid ? entry_arg(cA + (q * 32 + p) * (1 + D), rt) : -1e4;
+                    z[qq][k] = (valid && hw + SPEC_NHW * k < 32) ? ring_Z[slot] : 0.0;
+                }
+            }
+            const bool live0 = batch_is_live(arg[0]), live1 = batch_is_live(arg[1]);
+            if (live0 && live1) {
 #pragma unroll
-                        for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
+                for (int k = 0; k < 2 * SPEC_NCOL; ++k) arg[k / SPEC_NCOL][k % SPEC_NCOL] = exp_cap_tab64(arg[k / SPEC_NCOL][k % SPEC_NCOL], etab64);
+            } else {
+#pragma unroll
+                for (int qq = 0; qq < 2; ++qq) {
+                    if (qq ? live1 : live0) {
+#pragma unroll
+                        for (int k = 0; k < SPEC_NCOL; ++k) arg[qq][k] = exp_cap_tab64(arg[qq][k], etab64);
                     } else {
 #pragma unroll
-                        for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = 0.0;
+                        for (int k = 0; k < SPEC_NCOL; ++k) arg[qq][k] = 0.0;
                     }
-#pragma unroll
-                    for (int k = 0; k < SPEC_NCOL; ++k) sum = fma(z[k], arg[k], sum);
                 }
-                baseT_s[(((B & 1) * 2 + (q - 2)) * SPEC_NHW + hw) * 32 + lane] = sum;
+            }
+#pragma unroll
+            for (int qq = 0; qq < 2; ++qq) {
+                double sum = 0.0;
+#pragma unroll
+                for (int k = 0; k < SPEC_NCOL; ++k) sum = fma(z[qq][k], arg[qq][k], sum);
+                baseT_s[(((B & 1) * 2 + qq) * SPEC_NHW + hw) * 32 + lane] = sum;
             }
         }
         if (tht) ph_s[5] += clock64() - ht0;
         {   // ---- E'(K+2)
-            const int B = K + 2, b7 = B & 7, c7 = (B - 1) & 7;
-            Vec<D> pr;
+            const int B = K + 2;
+            const double *cA = ctab_s + ((K + 1) & 1) * (4 * 32 * (1 + D)) + 32 * (1 + D), *rA = rtab_s + ((K + 1) & 1) * (2 * 32 * (1 + D)) + 32 * (1 + D);
+            double rt[1 + D];
 #pragma unroll
-            for (int c = 0; c < D; ++c) pr.v[c] = rho_s[(b7 * 32 + lane) * D + c];
-            const double Gr = G_s[b7 * 32 + lane];
-            const double2 c32 = colT_s[c7 * 34 + 32];
+            for (int c = 0; c < 1 + D; ++c) rt[c] = rA[lane * (1 + D) + c];
             double *uB = ue_s + (B & 1) * 1024;
             double arg[SPEC_NCOL];
 #pragma unroll
             for (int k = 0; k < SPEC_NCOL; ++k) {
                 const int p = min(hw + SPEC_NHW * k, 31);
-                Vec<D> pc;
-#pragma unroll
-                for (int c = 0; c < D; ++c) pc.v[c] = ring_sig[(((B - 1) * 32 + p) & (RB - 1)) * D + c];
-                const double2 ct = colT_s[c7 * 34 + p];
-                arg[k] = (((ct.x - c32.x) - Gr) - kk * dist2<D>(pr, pc)) + (ct.y - c32.y);
+                arg[k] = entry_arg(cA + p * (1 + D), rt);
             }
             // entries below e^-64 of the row's gauge are nothing (the sums they enter are O(1) in that gauge, give or
             // take the drift of a stale gauge): when a whole batch is that small -- the usual case for blocks of
@@ -1057,14 +1115,12 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 const double shift = dd_diff(ring_T[jrec0 & (RB - 1)], trefn_s[b3]) - G_s[b3 * 32 + lane];
                 unsigned long long um, us;
                 int npoll = 0;
-                const long long tp0 = clock64();
                 do { // each lane waits for its own row (k_prep emptied the words, the worker fills them)
                     um = ld_relaxed_u64(&a.p.pan_m[dir][i]);
                     us = ld_relaxed_u64(&a.p.pan_s[dir][i]);
-                    if (npoll == 0 && lane == 0 && a.phase != nullptr && dir == 0) ph_s[11] += clock64() - tp0;
                     ++npoll;
                 } while (um == PAN_EMPTY || us == PAN_EMPTY);
-                if (lane == 0 && a.phase != nullptr && dir == 0) { ph_s[10] += npoll; ph_s[12] += clock64() - tp0; }
+                if (lane == 0 && a.phase != nullptr && dir == 0) ph_s[10] += npoll; // 1 per block = never waited
                 v = __longlong_as_double((long long)us) * exp_cap_tab64(__longlong_as_double((long long)um) + shift, etab64);
             }
         }
@@ -1089,6 +1145,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         __syncthreads();
         if (warp == 0) gauges(B);
     }
+    __syncthreads();
+    if (warp == 1) col_row_terms(-2);
+    if (warp == 2) col_row_terms(-1);
     __syncthreads();
     if (warp < SPEC_NHW) helper_tasks(-1, warp);
 
@@ -1206,6 +1265,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 pc = ldvec<D>(sig, i);
                 if (i < N - 1) c0 = cc[i];
             }
+            __syncwarp(); // G of block K+3 is in place
+            col_row_terms(K); // while the loads are in flight
             traw_s[b3 * 34 + lane] = told;
             if (lane == 0) traw_s[b3 * 34 + 32] = told32;
 #pragma unroll
