@@ -310,7 +310,8 @@ def test_stale_gauge_evaluations_match_oracle(binding, oracle):
         (wl.custom(333, 8, d=2, beta=3.0, g=0.2, xi=1.0, init="ring", sigma=2.0), 0.01, 1.0, 1e-9),
         (wl.custom(200, 8, d=3, beta=2.0, g=0.1, xi=0.5, init="iid", sigma=0.8), 0.01, 1.0, 1e-9),
         (wl.custom(150, 8, d=2, beta=3.0, g=0.2, xi=-0.5, init="ring", sigma=3.0), 0.01, 1.0, 1e-7),
-        (wl.custom(333, 8, d=2, beta=3.0, g=0.0, xi=1.0, init="ring", sigma=2.0), 1.0, 30.0, 1e-9),  # jump: fallback        (wl.custom(1, 4, d=2, beta=2.0, g=0.0, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),      # one block, one row
+        (wl.custom(333, 8, d=2, beta=3.0, g=0.0, xi=1.0, init="ring", sigma=2.0), 1.0, 30.0, 1e-9),  # jump: fallback
+        (wl.custom(1, 4, d=2, beta=2.0, g=0.0, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),      # one block, one row
         (wl.custom(2, 4, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),
         (wl.custom(33, 6, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),     # ragged second block
         (wl.custom(64, 6, d=1, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.7), 0.01, 1.0, 1e-9),
@@ -329,6 +330,25 @@ def test_stale_gauge_evaluations_match_oracle(binding, oracle):
         assert sg == sgo
         assert abs(vb - vbo) <= tol * abs(vbo)
         check_forces(F.cpu().numpy(), Fo, tol)
+
+
+def test_shifted_cloud_keeps_parity(binding, oracle):
+    """The helper warps of k_chain_spec expand |rho - sigma|^2 about a block-local origin; a cloud that
+    sits far from the coordinate origin, with the particle index unrelated to the position, must not cost accuracy.
+    First evaluation: max-plus kernel; second and third: stale-gauge kernel with the tabulated terms."""
+    for d, shift in ((2, (40.0, -25.0)), (3, (-30.0, 12.5, 55.0)), (1, (80.0,))):
+        w = wl.custom(300, 8, d=d, beta=2.5, omega=0.01, g=0.0, xi=1.0, init="iid", sigma=1.2)  # weak trap: spring forces set the scale
+        x, _ = wl.make_state(w, 21)
+        x = x + np.asarray(shift).reshape((1, 1, d))
+        sim = make(binding, w)
+        sim.set_state(torch.from_numpy(x).cuda(), None)
+        Fo, vbo, sgo = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
+        for _ in range(3):
+            F, vb, sg = sim.forces()
+            assert sg == sgo
+            assert abs(vb - vbo) <= 1e-9 * abs(vbo)
+            check_forces(F.cpu().numpy(), Fo, 1e-9)
+        sim.close()
 
 
 def test_forces_round_trip_and_resume(binding, oracle):
