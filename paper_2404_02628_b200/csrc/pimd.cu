@@ -34,7 +34,7 @@ struct pimd_s {
     // derived
     double ks, kk, lambda;
     size_t ndof, slice;
-    int NB, nprep, nasm, look, look_spec, nworkers;
+    int NB, nprep, nasm, look, look_spec, nworkers, sms;
     // streams
     cudaStream_t s0, s1;
     cudaEvent_t ev_fork, ev_join;
@@ -209,6 +209,7 @@ template <int D> int setup_chain_attr(pimd_t h)
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     h->coop_max_blocks = nb * sms;
+    h->sms = sms;
     if (h->coop_max_blocks < 2) return fail(h, PIMD_ECUDA, "k_chain cannot be made co-resident (%d blocks)", h->coop_max_blocks);
     return PIMD_OK;
 }
@@ -294,11 +295,15 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         }
         h->gauge_valid = true;
         const int NT = (h->N + FP_TB - 1) / FP_TB;
-        const dim3 fgrid(NT, NT, 2);
+        // NT (NT+1) tiles at or below the diagonal (both directions); fewer than 8 per SM leave the kernel latency
+        // bound (a thread walks its row's columns one after the other), so the columns of a tile are cut in 2 or 4
+        const long long tiles = (long long)NT * (NT + 1);
+        const int cw = tiles >= 8LL * h->sms ? FP_TB : (2 * tiles >= 8LL * h->sms ? FP_TB / 2 : FP_TB / 4);
+        const dim3 fgrid(NT, NT * (FP_TB / cw), 2);
         {
             ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
-            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
-            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex, cw);
+            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex, cw);
         }
         CU(cudaGetLastError());
         {

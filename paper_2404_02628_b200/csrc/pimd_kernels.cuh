@@ -1523,9 +1523,12 @@ template <int D> size_t chain_spec_smem_bytes_host()
 constexpr int FP_TB = 128;
 
 template <int D, bool SGN>
-__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p)
+__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, int cw)
 {
-    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
+    // a CTA takes FP_TB rows x cw columns (cw = 32, 64 or FP_TB: the host cuts the column range of a tile into
+    // FP_TB / cw CTAs when the tiles alone would leave the SMs with a warp or two each)
+    const int nsub = FP_TB / cw;
+    const int rt = blockIdx.x, ct = blockIdx.y / nsub, sub = blockIdx.y - ct * nsub, dir = blockIdx.z;
     if (ct > rt) return;
     __shared__ double etab64[64];
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
@@ -1534,8 +1537,9 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
     __shared__ double sg_sig[FP_TB * D];
     const double2 *gd = p.g[dir], *go = p.g[1 - dir];
     const int i = rt * FP_TB + threadIdx.x;
-    const int j0 = ct * FP_TB;
-    {
+    const int j0 = ct * FP_TB + sub * cw;
+    if (j0 >= N || j0 > rt * FP_TB + FP_TB - 1) return; // nothing at or below the diagonal in this slice
+    if (threadIdx.x < cw) {
         const int j = j0 + threadIdx.x;
         double2 gj = make_double2(-INFINITY, 0.0);
         double sj = 1.0;
@@ -1553,13 +1557,13 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) sg_sig[threadIdx.x * D + c] = sc.v[c];
     }
     __syncthreads();
-    if (i >= N) return;
+    if (i >= N || i < j0) return;
     const Vec<D> pr = ldvec<D>(p.rho[dir], i);
     // A = g^{other}[N-1-i] - R_N as dd, rounded once per element after adding g^{dir}[j]
     const double2 A = dd_sub(go[N - 1 - i], p.rfin[0]);
     double osg = p.gs[1 - dir][N - 1 - i];
     if constexpr (SGN) osg *= p.rsgn[0];
-    const int ncol = min(FP_TB, i - j0 + 1); // columns j0 .. min(j0+127, i)
+    const int ncol = min(cw, i - j0 + 1); // columns j0 .. min(j0 + cw - 1, i)
     double sw = 0.0, swc = 0.0;
     Vec<D> sws;
 #pragma unroll
