@@ -101,7 +101,7 @@ def recursion_report(w, kern, phases, steps, clocks):
     ch = kern.get("chain", {}).get("ms_avg")
     nb = (w.N + 31) // 32
     out = {"kernel": "k_chain_spec (forward + backward recursion with the previous step's gauge, one cooperative launch)",
-           "bound": "latency", "fallback_ms": kern.get("chain_fallback", {}).get("ms_avg"),
+           "bound": "latency",
            "ms": ch, "ns_per_row": (ch * 1e6 / w.N if ch else None), "rows_per_block": 32}
     if ch and sum(phases[:4]) > 0:
         per = [c / float(steps * nb) for c in phases[:16]]

@@ -160,7 +160,7 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
 #define PIMD_PROF_COMBINE 7   /* force output */
 #define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
-#define PIMD_PROF_CHAIN_FALLBACK 9 /* the max-plus recursion queued behind the stale-gauge one (returns at once if unused) */
+#define PIMD_PROF_CHAIN_FALLBACK 9 /* unused (always 0 launches): the safety net now runs inside the CHAIN launch */
 #define PIMD_PROF_EMAT 10     /* pimd_cycle_energies: the N x N write */
 #define PIMD_PROF_PRMAT 11    /* pimd_connection_probabilities: the N x N write */
 #define PIMD_PROF_NSLOTS 12

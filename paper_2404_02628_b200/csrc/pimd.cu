@@ -202,10 +202,11 @@ template <int D> int setup_chain_attr(pimd_t h)
     CU(cudaFuncSetAttribute(k_chain<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CU(cudaFuncSetAttribute(k_chain<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     h->spec_smem = chain_spec_smem_bytes_host<D>();
+    if (h->spec_smem < smem) h->spec_smem = smem; // k_chain_spec holds the max-plus recursion as its safety net
     CU(cudaFuncSetAttribute(k_chain_spec<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->spec_smem));
     CU(cudaFuncSetAttribute(k_chain_spec<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->spec_smem));
     int nb = 0, dev = 0, sms = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_chain<D, true>, CH_THREADS, smem));
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_chain_spec<D, true>, CH_THREADS, h->spec_smem));
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     h->coop_max_blocks = nb * sms;
@@ -268,27 +269,18 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         a.N = h->N; a.NB = h->NB; a.look = h->look; a.nworkers = h->nworkers;
         a.kk = h->kk; a.sx = sgn ? -1.0 : 1.0; a.p = h->ex;
         a.phase = h->profiling ? h->phase : nullptr;
-        a.cond = 0;
+        a.look_fb = h->look;
         const int look_spec = h->look_spec;
         void *args[] = {&a};
         const dim3 grid(1 + h->nworkers, 2), block(CH_THREADS);
         const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
         if (h->gauge_valid && h->use_spec) {
-            // the previous evaluation's gauge is at hand: linear pass only; the max-plus kernel is queued
-            // behind it and returns at once unless the gauge turned out not to fit
+            // the previous evaluation's gauge is at hand: linear pass only; the kernel redoes the recursion with a
+            // fresh max-plus gauge itself (after a grid barrier) if the gauge turned out not to fit
             const void *fs = sgn ? (const void *)k_chain_spec<D, true> : (const void *)k_chain_spec<D, false>;
             a.look = look_spec; // the workers need one more block of head start when the chain runs this fast
-            {
-                ProfScope ps(h, PIMD_PROF_CHAIN, st);
-                CU(cudaLaunchCooperativeKernel(fs, grid, block, args, h->spec_smem, st));
-            }
-            a.look = h->look;
-            a.cond = 1;
-            a.phase = nullptr;
-            {
-                ProfScope ps(h, PIMD_PROF_CHAIN_FALLBACK, st);
-                CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
-            }
+            ProfScope ps(h, PIMD_PROF_CHAIN, st);
+            CU(cudaLaunchCooperativeKernel(fs, grid, block, args, h->spec_smem, st));
         } else {
             ProfScope ps(h, PIMD_PROF_CHAIN, st);
             CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
@@ -640,7 +632,7 @@ static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpy
     h->forces_valid = false;
     h->tables_valid = false;
     // the exchange gauge of the last evaluation is kept: if the new positions are far from the old ones the
-    // stale-gauge kernel notices and the max-plus kernel queued behind it takes over
+    // stale-gauge kernel notices and redoes the recursion with a fresh max-plus gauge
     return PIMD_OK;
 }
 

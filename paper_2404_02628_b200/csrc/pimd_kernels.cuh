@@ -347,7 +347,7 @@ struct ChainArgs {
     int N, NB, look, nworkers;
     double kk, sx;
     ExchPtrs p;
-    int cond;                  // 1: run only if status[2] is set (fallback behind k_chain_spec)
+    int look_fb;               // k_chain_spec: look-ahead of the max-plus recursion it falls back to
     unsigned long long *phase; // optional [16]: cycles of the forward chain CTA per phase (profiling), or NULL
 };
 
@@ -817,8 +817,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 //   warp 0 folds E'(K+1) Zhat into the next block's start value inside its own loop (one more DFMA per
 //   step, off the dependent path), so one block-wide barrier per block is all the synchronisation.
 // A row sum outside [1e-270, 1e270] (the gauge no longer fits: first evaluation, state replaced, a jump)
-// raises status[2]; the host always queues the max-plus kernel behind this one, and that kernel returns at
-// once unless the flag is set.
+// raises status[2]; k_chain_spec then redoes the recursion with the max-plus code after a grid barrier.
 // ==========================================================================================
 #ifndef PIMD_SPEC_NHW
 #define PIMD_SPEC_NHW 9
@@ -1475,16 +1474,6 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int dir = blockIdx.y;
-    if (a.cond) {
-        // queued behind k_chain_spec: needed only if that kernel found its gauge out of range
-        if (ld_acquire(a.p.status + 2) == 0) return; // the same answer in every CTA
-        if (blockIdx.x == 0 && blockIdx.y == 0) {
-            for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { a.p.panel_ready[0][k] = 0; a.p.panel_ready[1][k] = 0; }
-            if (threadIdx.x < 2) a.p.cols_ready[threadIdx.x] = 1;
-        }
-        __threadfence();
-        cooperative_groups::this_grid().sync();
-    }
     if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw, etab);
     else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
 }
@@ -1501,6 +1490,24 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
     const int dir = blockIdx.y;
     if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, smem_raw, etab64);
     else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
+    // Safety net in the same launch (a second, conditional cooperative launch cost 7 us per evaluation): if a row sum
+    // left the range the stale gauge covers, every CTA sees status[2] after the grid barrier and the whole grid redoes
+    // the recursion with a fresh max-plus gauge (chain_cta), which overwrites everything this pass published.
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __threadfence();
+    grid.sync();
+    if (ld_acquire(a.p.status + 2) == 0) return; // the same answer in every CTA
+    if (blockIdx.x == 0 && blockIdx.y == 0) {
+        for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { a.p.panel_ready[0][k] = 0; a.p.panel_ready[1][k] = 0; }
+        if (threadIdx.x < 2) a.p.cols_ready[threadIdx.x] = 1;
+    }
+    __threadfence();
+    grid.sync();
+    ChainArgs b = a;
+    b.look = a.look_fb;
+    b.phase = nullptr;
+    if (blockIdx.x == 0) chain_cta<D, SGN>(b, dir, smem_raw, etab);
+    else worker_cta<D, SGN>(b, dir, blockIdx.x - 1, smem_raw, etab64);
 }
 
 template <int D> size_t chain_spec_smem_bytes_host()
