@@ -230,7 +230,8 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         // pair forces, added to F (Newton's third law, one Gaussian per unordered pair)
         const int NT = (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
-        int target = NT <= 64 ? 2 : 4; // offsets per task: small tasks balance small grids (tuning knob PIMD_PAIR_CH)
+        // offsets per task: small tasks balance small grids (measured: 1 is best up to N = 2500, 4 at N = 10000; tuning knob PIMD_PAIR_CH)
+        int target = NT <= 100 ? 1 : (NT <= 200 ? 2 : 4);
         if (const char *e = std::getenv("PIMD_PAIR_CH")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) target = v; }
         const int nchunk = hmax > 0 ? std::max(1, (hmax + target / 2) / target) : 0;
         const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
@@ -287,15 +288,21 @@ template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
         }
         h->gauge_valid = true;
         const int NT = (h->N + FP_TB - 1) / FP_TB;
-        // NT (NT+1) tiles at or below the diagonal (both directions); fewer than 8 per SM leave the kernel latency
-        // bound (a thread walks its row's columns one after the other), so the columns of a tile are cut in 2 or 4
+        // NT (NT+1) tiles at or below the diagonal (both directions); with fewer than 8 per SM one thread per row leaves
+        // the kernel latency bound, so four threads share a row (measured at cfg3: 0.023 -> 0.017 ms with the columns cut
+        // into four CTAs, less again with the partial sums combined inside one CTA)
         const long long tiles = (long long)NT * (NT + 1);
-        const int cw = tiles >= 8LL * h->sms ? FP_TB : (2 * tiles >= 8LL * h->sms ? FP_TB / 2 : FP_TB / 4);
-        const dim3 fgrid(NT, NT * (FP_TB / cw), 2);
+        const bool wide = tiles < 8LL * h->sms;
+        const dim3 fgrid(wide ? (h->N + FP_TB / 4 - 1) / (FP_TB / 4) : NT, NT, 2);
         {
             ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
-            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex, cw);
-            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex, cw);
+            if (wide) {
+                if (sgn) k_forcepass<D, true, 4><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+                else k_forcepass<D, false, 4><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+            } else {
+                if (sgn) k_forcepass<D, true, 1><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+                else k_forcepass<D, false, 1><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+            }
         }
         CU(cudaGetLastError());
         {

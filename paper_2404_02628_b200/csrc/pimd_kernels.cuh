@@ -1529,24 +1529,28 @@ template <int D> size_t chain_spec_smem_bytes_host()
 // ==========================================================================================
 constexpr int FP_TB = 128;
 
-template <int D, bool SGN>
-__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, int cw)
+template <int D, bool SGN, int NQ>
+__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p)
 {
-    // a CTA takes FP_TB rows x cw columns (cw = 32, 64 or FP_TB: the host cuts the column range of a tile into
-    // FP_TB / cw CTAs when the tiles alone would leave the SMs with a warp or two each)
-    const int nsub = FP_TB / cw;
-    const int rt = blockIdx.x, ct = blockIdx.y / nsub, sub = blockIdx.y - ct * nsub, dir = blockIdx.z;
-    if (ct > rt) return;
+    // a CTA of FP_TB threads takes RT rows x FP_TB columns at or below the diagonal.  NQ = 1: RT = FP_TB, one thread per
+    // row walks the tile's columns (large N: enough tiles to fill the GPU).  NQ = 4: RT = 32, four threads per row with 32
+    // columns each, partial sums combined in shared memory before the atomics (small N: a thread per row alone leaves
+    // the SMs with a warp or two each and the kernel latency bound; four times as many, smaller CTAs also spread evenly
+    // over the SMs).
+    constexpr int CW = FP_TB / NQ, RT = FP_TB / NQ;
+    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
+    const int j0 = ct * FP_TB;
+    if (j0 > rt * RT + RT - 1) return; // above the diagonal
     __shared__ double etab64[64];
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __shared__ double2 sg_g[FP_TB];
     __shared__ double sg_s[FP_TB];
     __shared__ double sg_sig[FP_TB * D];
+    __shared__ double part_s[(NQ > 1) ? NQ * (D + 2) * RT : 1];
     const double2 *gd = p.g[dir], *go = p.g[1 - dir];
-    const int i = rt * FP_TB + threadIdx.x;
-    const int j0 = ct * FP_TB + sub * cw;
-    if (j0 >= N || j0 > rt * FP_TB + FP_TB - 1) return; // nothing at or below the diagonal in this slice
-    if (threadIdx.x < cw) {
+    const int r = threadIdx.x % RT, q = threadIdx.x / RT;
+    const int i = rt * RT + r;
+    {
         const int j = j0 + threadIdx.x;
         double2 gj = make_double2(-INFINITY, 0.0);
         double sj = 1.0;
@@ -1564,35 +1568,56 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
         for (int c = 0; c < D; ++c) sg_sig[threadIdx.x * D + c] = sc.v[c];
     }
     __syncthreads();
-    if (i >= N || i < j0) return;
-    const Vec<D> pr = ldvec<D>(p.rho[dir], i);
-    // A = g^{other}[N-1-i] - R_N as dd, rounded once per element after adding g^{dir}[j]
-    const double2 A = dd_sub(go[N - 1 - i], p.rfin[0]);
-    double osg = p.gs[1 - dir][N - 1 - i];
-    if constexpr (SGN) osg *= p.rsgn[0];
-    const int ncol = min(cw, i - j0 + 1); // columns j0 .. min(j0 + cw - 1, i)
-    double sw = 0.0, swc = 0.0;
+    const int k0 = q * CW;
+    const int ncol = (i < N) ? min(CW, i - (j0 + k0) + 1) : 0; // columns j0+k0 .. min(j0+k0+CW-1, i)
+    double sw = 0.0, swc = 0.0, osg = 0.0;
     Vec<D> sws;
 #pragma unroll
     for (int c = 0; c < D; ++c) sws.v[c] = 0.0;
+    if (ncol > 0) {
+        const Vec<D> pr = ldvec<D>(p.rho[dir], i);
+        // A = g^{other}[N-1-i] - R_N as dd, rounded once per element after adding g^{dir}[j]
+        const double2 A = dd_sub(go[N - 1 - i], p.rfin[0]);
+        osg = p.gs[1 - dir][N - 1 - i];
+        if constexpr (SGN) osg *= p.rsgn[0];
 #pragma unroll 4
-    for (int k = 0; k < ncol; ++k) {
-        Vec<D> pc;
+        for (int k = k0; k < k0 + ncol; ++k) {
+            Vec<D> pc;
 #pragma unroll
-        for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
-        const double2 gj = sg_g[k];
-        const double kr2 = kk * dist2<D>(pr, pc);
-        const double w = exp_cap_tab64(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab64) * sg_s[k];
-        sw += w;
-        swc = fma(w, kr2, swc);
+            for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
+            const double2 gj = sg_g[k];
+            const double kr2 = kk * dist2<D>(pr, pc);
+            const double w = exp_cap_tab64(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab64) * sg_s[k];
+            sw += w;
+            swc = fma(w, kr2, swc);
 #pragma unroll
-        for (int c = 0; c < D; ++c) sws.v[c] = fma(w, pc.v[c], sws.v[c]);
+            for (int c = 0; c < D; ++c) sws.v[c] = fma(w, pc.v[c], sws.v[c]);
+        }
     }
-    double *o = p.acc[dir] + (size_t)i * (D + 2);
-    atomicAdd(&o[0], osg * sw);
+    if constexpr (NQ > 1) {
+        part_s[(q * (D + 2)) * RT + r] = osg * sw;
 #pragma unroll
-    for (int c = 0; c < D; ++c) atomicAdd(&o[1 + c], osg * sws.v[c]);
-    atomicAdd(&o[D + 1], osg * swc);
+        for (int c = 0; c < D; ++c) part_s[(q * (D + 2) + 1 + c) * RT + r] = osg * sws.v[c];
+        part_s[(q * (D + 2) + D + 1) * RT + r] = osg * swc;
+        __syncthreads();
+        // thread (r, q) adds up components q, q + NQ, .. of row r
+        if (i < N && i >= j0) {
+            for (int c = q; c < D + 2; c += NQ) {
+                double t = 0.0;
+#pragma unroll
+                for (int qq = 0; qq < NQ; ++qq) t += part_s[(qq * (D + 2) + c) * RT + r];
+                atomicAdd(p.acc[dir] + (size_t)i * (D + 2) + c, t);
+            }
+        }
+    } else {
+        if (ncol > 0) {
+            double *o = p.acc[dir] + (size_t)i * (D + 2);
+            atomicAdd(&o[0], osg * sw);
+#pragma unroll
+            for (int c = 0; c < D; ++c) atomicAdd(&o[1 + c], osg * sws.v[c]);
+            atomicAdd(&o[D + 1], osg * swc);
+        }
+    }
 }
 
 // ==========================================================================================
