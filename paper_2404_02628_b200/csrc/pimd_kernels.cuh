@@ -1341,6 +1341,19 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
 #pragma unroll
         for (int c = 0; c < D; ++c) pr.v[c] = 0.0;
         if (i < N) pr = ldvec<D>(rho, i);
+        // exponent arguments in 1 + D instructions per entry, as in chain_cta_spec: with the origin o = row 0 of the
+        // block, rho' = rho_r - o, sigma' = sigma_p - o:  (T_p - T_ref) - kk |rho_r - sigma_p|^2 = A_p + B_r +
+        // sum_c (2 kk rho'_c) sigma'_c,  A_p = (T_p - T_ref) - kk |sigma'_p|^2 (per column, at staging),
+        // B_r = -kk |rho'_r|^2 (per row, here)
+        const Vec<D> org = ldvec<D>(rho, K * 32);
+        double rowB = 0.0, roww[D];
+#pragma unroll
+        for (int c = 0; c < D; ++c) {
+            const double rp = pr.v[c] - org.v[c];
+            rowB = fma(rp, rp, rowB);
+            roww[c] = 2.0 * kk * rp;
+        }
+        rowB *= -kk;
         const int ntile = K - LOOK;
         Lse acc = lse_empty();
         double2 ref = make_double2(0.0, 0.0);
@@ -1388,11 +1401,21 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 load_cols(c8);
             }
             __syncwarp();
-            if (lane < 8) {
-                st_g[lane] = pre_g;
-                st_sg[lane] = pre_z;
+            {
+                // the chunk's first column is its reference; every column leaves (A_p, sigma'_p, Zhat_p)
+                const double2 g0 = make_double2(shfl_bcast(pre_g.x, 0), shfl_bcast(pre_g.y, 0));
+                if (lane < 8) {
+                    double n2 = 0.0;
 #pragma unroll
-                for (int c = 0; c < D; ++c) st_sig[lane * D + c] = pre_c.v[c];
+                    for (int c = 0; c < D; ++c) {
+                        const double sp = pre_c.v[c] - org.v[c];
+                        n2 = fma(sp, sp, n2);
+                        st_sig[lane * D + c] = sp;
+                    }
+                    st_g[8 + lane].x = fma(-kk, n2, dd_diff(pre_g, g0));
+                    st_sg[lane] = pre_z;
+                    if (lane == 0) st_g[0] = pre_g;
+                }
             }
             __syncwarp();
             have_pre = (c8 + CH_WARPS < 4 * ntile) && cols_are_ready(c8 + CH_WARPS, false);
@@ -1404,10 +1427,10 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             double cm = -INFINITY;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
-                Vec<D> pc;
+                double t = st_g[8 + k].x + rowB;
 #pragma unroll
-                for (int c = 0; c < D; ++c) pc.v[c] = st_sig[k * D + c];
-                tau[k] = dd_diff(st_g[k], ref) - kk * dist2<D>(pr, pc);
+                for (int c = 0; c < D; ++c) t = fma(roww[c], st_sig[k * D + c], t);
+                tau[k] = t;
                 cm = fmax(cm, tau[k]);
             }
             if (cm > acc.m) {
