@@ -1424,15 +1424,15 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
             lse_shift(acc, dd_diff(ref, nref));
             ref = nref;
             double tau[8];
-            double cm = -INFINITY;
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
                 double t = st_g[8 + k].x + rowB;
 #pragma unroll
                 for (int c = 0; c < D; ++c) t = fma(roww[c], st_sig[k * D + c], t);
                 tau[k] = t;
-                cm = fmax(cm, tau[k]);
             }
+            // maximum as a tree (three levels instead of a chain of eight)
+            const double cm = fmax(fmax(fmax(tau[0], tau[1]), fmax(tau[2], tau[3])), fmax(fmax(tau[4], tau[5]), fmax(tau[6], tau[7])));
             if (cm > acc.m) {
                 acc.s *= exp_neg_tab64(-(acc.m - cm), etab64);
                 acc.m = cm;
