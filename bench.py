@@ -30,7 +30,7 @@ FLOP_PER_PAIR = 50.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_d_cfg3.md for cfg3 -- unchanged since r1_b_cfg3.md --, profiles/r1_b_cfg5b.md for cfg5b); None where no
 # capture of that workload exists
-NCU_TRAFFIC = {("cfg3", "pair"): 1704448 + 0, ("cfg3", "forcepass"): 290048 + 0,
+NCU_TRAFFIC = {("cfg3", "pair"): 1704448 + 0, ("cfg3", "forcepass"): 291072 + 0,
                ("cfg5b", "pair"): 5186048 + 0, ("cfg5b", "forcepass"): 1768960 + 0}
 
 
