@@ -466,7 +466,7 @@ template <int D> static int cycle_energies_impl(pimd_t h, double *e_dev)
 
 template <int D> static int prmat_impl(pimd_t h, double *pr_dev)
 {
-    const dim3 grid((h->N + 1023) / 1024, h->N), gridp((h->N + 1023) / 1024, (h->N + PRMAT_ROWS - 1) / PRMAT_ROWS);
+    const dim3 grid((h->N + 1023) / 1024, h->N), gridp((h->N + 256 * PRMAT_COLS - 1) / (256 * PRMAT_COLS), (h->N + PRMAT_ROWS - 1) / PRMAT_ROWS);
     ProfScope ps(h, PIMD_PROF_PRMAT, h->s0);
     if (h->xi == 0.0) k_identity<<<grid, 256, 0, h->s0>>>(h->N, pr_dev);
     else if (h->xi < 0.0) k_prmat<D, true><<<gridp, 256, 0, h->s0>>>(h->N, h->kk, h->ex, pr_dev);

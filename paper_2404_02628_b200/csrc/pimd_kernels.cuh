@@ -1755,31 +1755,36 @@ __global__ void __launch_bounds__(256) k_emat(int N, double ks, const double *__
 }
 
 constexpr int PRMAT_ROWS = 8; // rows per CTA: the column tables are read once and kept in registers for all of them
+constexpr int PRMAT_COLS = 4; // columns per thread (256 apart)
+// four CTAs per SM (64 registers) instead of the three that 72 registers allow: N=10000 0.185 -> 0.170 ms; two columns per
+// thread (56 registers) measured 0.175, one 0.233, and taking row blocks alternately from the top (zeros) and the bottom
+// (exponentials) of the matrix changed nothing: the lower triangle is FP64 bound at the pair kernel's rate
+constexpr int PRMAT_MINB = 4;
 
 template <int D, bool SGN>
-__global__ void __launch_bounds__(256) k_prmat(int N, double kk, ExchPtrs p, double *__restrict__ Pr)
+__global__ void __launch_bounds__(256, PRMAT_MINB) k_prmat(int N, double kk, ExchPtrs p, double *__restrict__ Pr)
 {
     __shared__ double etab64[64];
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int l0 = blockIdx.y * PRMAT_ROWS;
-    const int c0 = blockIdx.x * 1024 + threadIdx.x;
+    const int c0 = blockIdx.x * (256 * PRMAT_COLS) + threadIdx.x;
     if (c0 - threadIdx.x > l0 + PRMAT_ROWS) {
         // the whole segment lies two or more above the diagonal of all these rows: zeros
         for (int r = 0; r < PRMAT_ROWS && l0 + r < N; ++r) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
+            for (int k = 0; k < PRMAT_COLS; ++k) {
                 const int lp = c0 + 256 * k;
                 if (lp < N) __stcs(Pr + (size_t)(l0 + r) * N + lp, 0.0);
             }
         }
         return;
     }
-    double2 gj[4];
-    double zj[4];
-    Vec<D> sj[4];
+    double2 gj[PRMAT_COLS];
+    double zj[PRMAT_COLS];
+    Vec<D> sj[PRMAT_COLS];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < PRMAT_COLS; ++k) {
         const int lp = min(c0 + 256 * k, N - 1);
         gj[k] = p.g[0][lp];
         zj[k] = p.gs[0][lp];
@@ -1794,12 +1799,12 @@ __global__ void __launch_bounds__(256) k_prmat(int N, double kk, ExchPtrs p, dou
         if constexpr (SGN) osg *= p.rsgn[0];
         const double pn = p.pnext[l];
         double *row = Pr + (size_t)l * N;
-        double w[4];
+        double w[PRMAT_COLS];
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
+        for (int k = 0; k < PRMAT_COLS; ++k)
             w[k] = exp_cap_tab64(((A.x + gj[k].x) + (A.y + gj[k].y)) - kk * dist2<D>(rP, sj[k]), etab64);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < PRMAT_COLS; ++k) {
             const int lp = c0 + 256 * k;
             if (lp < N) __stcs(row + lp, lp <= l ? osg * zj[k] * w[k] : (lp == l + 1 ? pn : 0.0));
         }
