@@ -30,7 +30,7 @@ FLOP_PER_PAIR = 50.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_d_cfg3.md for cfg3 -- unchanged since r1_b_cfg3.md --, profiles/r1_b_cfg5b.md for cfg5b); None where no
 # capture of that workload exists
-NCU_TRAFFIC = {("cfg3", "pair"): 1704448 + 0, ("cfg3", "forcepass"): 291072 + 0,
+NCU_TRAFFIC = {("cfg3", "pair"): 1706240 + 0, ("cfg3", "forcepass"): 291072 + 0,
                ("cfg5b", "pair"): 5186048 + 0, ("cfg5b", "forcepass"): 1768960 + 0}
 
 
@@ -313,7 +313,7 @@ def run_ours(args, w):
                     "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
                                    "1.965 GHz x 2 = 37.2 TFLOP/s)",
                     "convention": "50 flop (25 FP64 instructions, SURVEY.md 8(d)) per unordered bead pair, %d pairs per launch; "
-                                  "the shipped kernel spends 17 FP64 instructions per pair (table-driven exp), so frac can "
+                                  "the shipped kernel spends 16 FP64 instructions per pair (table-driven exp), so frac can "
                                   "exceed the FP64 pipe utilisation ncu reports" % int(pairs),
                     "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
                     "alone": {"ms": iso.get("pair"), "frac": pairs * FLOP_PER_PAIR / (iso["pair"] * 1e-3) / 1e12 / fp64_peak}}

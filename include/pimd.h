@@ -186,7 +186,9 @@ int pimd_probe_fp64_peak(void *cuda_stream, double *tflops);
 
 /* The device exponentials of the hot kernels, element-wise, for accuracy tests: y[i] = f(x[i]) with
  * which = 0: exp_fast(x) (x <= 700), 1: exp_tab(x) (table of 32, x <= 700), 2: exp_neg_tab64(x) = exp(-x), x >= 0
- * (the pair kernel's Gaussian; returns e^-708 for x > 708).  x_dev, y_dev DEVICE, n elements.  Synchronises. */
+ * (the recursion's and the force pass's table exponential; returns e^-708 for x > 708), 3: exp_neg_tab256(x) = exp(-x),
+ * x >= 0 (the pair kernel's Gaussian, table of 256; returns e^-708 for x > 708).  x_dev, y_dev DEVICE, n elements.
+ * Synchronises. */
 int pimd_selftest_exp(void *cuda_stream, int which, const double *x_dev, double *y_dev, size_t n);
 
 const char *pimd_last_error(pimd_t h); /* h may be NULL: error of the last failed pimd_create */

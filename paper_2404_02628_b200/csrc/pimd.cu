@@ -950,7 +950,7 @@ int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host)
 int pimd_selftest_exp(void *cuda_stream, int which, const double *x_dev, double *y_dev, size_t n)
 {
     pimd_t h = nullptr;
-    if (which < 0 || which > 2 || !x_dev || !y_dev) return fail(nullptr, PIMD_EINVAL, "pimd_selftest_exp: bad argument");
+    if (which < 0 || which > 3 || !x_dev || !y_dev) return fail(nullptr, PIMD_EINVAL, "pimd_selftest_exp: bad argument");
     if (n == 0) return PIMD_OK;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     k_exp_selftest<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x_dev, y_dev, n, which);

@@ -1980,7 +1980,8 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
 // lane to lane (one shuffle rotation per step), so each Gaussian is evaluated once and used for both
 // partners.  Tile results are added to F with FP64 atomics (F already holds the spring/trap forces).
 // The last task of a row does the 32 x 32 diagonal tile the plain way.
-// Coordinates are pre-scaled by 1/s so that the exponent is -|dx'|^2; padding particles sit at
+// The Gaussian is exp_neg_tab256 (8 FP64 instructions; the 64-entry form with one more FMA measured 0.0811 against
+// 0.0783 ms at cfg3).  Coordinates are pre-scaled by 1/s so that the exponent is -|dx'|^2; padding particles sit at
 // +-1e150 and give e^-708 ~ 3e-308 (their forces are never written).
 // grid (ceil(tasks/PAIR_WARPS), P), block PAIR_WARPS * 32; tasks = NT (nchunk + 1).
 // ==========================================================================================
@@ -1996,7 +1997,7 @@ PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, V
     double r2 = dl.v[0] * dl.v[0];
 #pragma unroll
     for (int c = 1; c < D; ++c) r2 = fma(dl.v[c], dl.v[c], r2);
-    const double e = exp_neg_tab64(r2, tab);
+    const double e = exp_neg_tab256(r2, tab);
 #pragma unroll
     for (int c = 0; c < D; ++c) {
         fi.v[c] = fma(e, dl.v[c], fi.v[c]);
@@ -2034,9 +2035,9 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
                                                          double g, EstAccum *est)
 {
     __shared__ double tiles[PAIR_WARPS][2][64 * D];
-    __shared__ double tab[64];
+    __shared__ double tab[256];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x < 64) tab[threadIdx.x] = c_exp2_64[threadIdx.x];
+    for (int k = threadIdx.x; k < 256; k += PAIR_WARPS * 32) tab[k] = g_exp2_256[k];
     __syncthreads();
     const int task = blockIdx.x * PAIR_WARPS + warp;
     if (task >= NT * (nchunk + 1)) return; // warp-uniform; no block-wide barrier below
@@ -2166,14 +2167,15 @@ __global__ void k_zero(double *p, size_t n)
 // 2 exp_neg_tab64(x) = exp(-x), x >= 0
 __global__ void __launch_bounds__(256) k_exp_selftest(const double *__restrict__ x, double *__restrict__ y, size_t n, int which)
 {
-    __shared__ double t32[32], t64[64];
+    __shared__ double t32[32], t64[64], t256[256];
     if (threadIdx.x < 32) t32[threadIdx.x] = c_exp2_32[threadIdx.x];
     if (threadIdx.x < 64) t64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    t256[threadIdx.x] = g_exp2_256[threadIdx.x];
     __syncthreads();
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double v = x[i];
-    y[i] = which == 0 ? exp_fast(v) : (which == 1 ? exp_tab(v, t32) : exp_neg_tab64(v, t64));
+    y[i] = which == 0 ? exp_fast(v) : (which == 1 ? exp_tab(v, t32) : (which == 2 ? exp_neg_tab64(v, t64) : exp_neg_tab256(v, t256)));
 }
 
 // FP64 FMA issue-rate probe: 8 independent chains per thread, register resident.

@@ -183,12 +183,13 @@ def test_device_exponentials_match_libm(binding):
         assert np.all(y[~live] == 0.0)
     r2 = -x[x <= 0.0]
     r2 = r2[np.isfinite(r2)]
-    y = binding.selftest_exp(2, torch.from_numpy(r2).cuda()).cpu().numpy()
     ref2 = np.exp(-r2)
     live = r2 <= 700.0
-    # one-FMA argument reduction: relative error grows like r2 * 1.1e-16
-    assert np.max(np.abs(y[live] - ref2[live]) / ref2[live] / (1.0 + r2[live])) <= 3e-16
-    assert np.all(y[~live] <= 1e-300) and np.all(y >= 0.0)
+    for which in (2, 3):  # 64-entry table (recursion, force pass) and 256-entry table (pair kernel)
+        y = binding.selftest_exp(which, torch.from_numpy(r2).cuda()).cpu().numpy()
+        # one-FMA argument reduction: relative error grows like r2 * 1.1e-16
+        assert np.max(np.abs(y[live] - ref2[live]) / ref2[live] / (1.0 + r2[live])) <= 3e-16
+        assert np.all(y[~live] <= 1e-300) and np.all(y >= 0.0)
 
 
 def test_chain_phase_clock(binding):
