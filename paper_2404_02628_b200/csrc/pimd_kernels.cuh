@@ -1564,8 +1564,12 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
     const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
     const int j0 = ct * FP_TB;
     if (j0 > rt * RT + RT - 1) return; // above the diagonal
-    __shared__ double etab64[64];
-    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    // one thread per row (large N): 256-entry table, 8 FP64 instructions per exponential (N=10000 0.202 -> 0.195 ms);
+    // four threads per row (small N, many small CTAs): the 64-entry table, whose fill per CTA is four times cheaper
+    // (cfg3 0.0170 against 0.0173 ms with the large table)
+    constexpr int NTAB = (NQ == 1) ? 256 : 64;
+    __shared__ double etab[NTAB];
+    for (int k = threadIdx.x; k < NTAB; k += blockDim.x) etab[k] = (NQ == 1) ? g_exp2_256[k] : c_exp2_64[k];
     __shared__ double2 sg_g[FP_TB];
     __shared__ double sg_s[FP_TB];
     __shared__ double sg_sig[FP_TB * D];
@@ -1610,7 +1614,8 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
             for (int c = 0; c < D; ++c) pc.v[c] = sg_sig[k * D + c];
             const double2 gj = sg_g[k];
             const double kr2 = kk * dist2<D>(pr, pc);
-            const double w = exp_cap_tab64(((A.x + gj.x) + (A.y + gj.y)) - kr2, etab64) * sg_s[k];
+            const double targ = ((A.x + gj.x) + (A.y + gj.y)) - kr2;
+            const double w = ((NQ == 1) ? exp_cap_tab256(targ, etab) : exp_cap_tab64(targ, etab)) * sg_s[k];
             sw += w;
             swc = fma(w, kr2, swc);
 #pragma unroll
@@ -1764,8 +1769,8 @@ constexpr int PRMAT_MINB = 4;
 template <int D, bool SGN>
 __global__ void __launch_bounds__(256, PRMAT_MINB) k_prmat(int N, double kk, ExchPtrs p, double *__restrict__ Pr)
 {
-    __shared__ double etab64[64];
-    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __shared__ double etab256[256];
+    etab256[threadIdx.x] = g_exp2_256[threadIdx.x];
     __syncthreads();
     const int l0 = blockIdx.y * PRMAT_ROWS;
     const int c0 = blockIdx.x * (256 * PRMAT_COLS) + threadIdx.x;
@@ -1802,7 +1807,7 @@ __global__ void __launch_bounds__(256, PRMAT_MINB) k_prmat(int N, double kk, Exc
         double w[PRMAT_COLS];
 #pragma unroll
         for (int k = 0; k < PRMAT_COLS; ++k)
-            w[k] = exp_cap_tab64(((A.x + gj[k].x) + (A.y + gj[k].y)) - kk * dist2<D>(rP, sj[k]), etab64);
+            w[k] = exp_cap_tab256(((A.x + gj[k].x) + (A.y + gj[k].y)) - kk * dist2<D>(rP, sj[k]), etab256);
 #pragma unroll
         for (int k = 0; k < PRMAT_COLS; ++k) {
             const int lp = c0 + 256 * k;

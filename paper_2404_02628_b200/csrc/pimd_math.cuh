@@ -222,6 +222,13 @@ PIMD_DEV double exp_cap_tab64(double x, const double *tab)
     return exp_neg_tab64(-__hiloint2double(big ? 0x4085e000 : __double2hiint(x), big ? 0 : __double2loint(x)), tab);
 }
 
+// exp(x) for any x through the 256-entry table (8 FP64 instructions), same cap as exp_cap_tab64
+PIMD_DEV double exp_cap_tab256(double x, const double *tab)
+{
+    const bool big = __double2hiint(x) > 0x4085e000;
+    return exp_neg_tab256(-__hiloint2double(big ? 0x4085e000 : __double2hiint(x), big ? 0 : __double2loint(x)), tab);
+}
+
 // ---------------------------------------------------------------------------------------------
 // double-double helpers.  A dd value is (hi, lo) in a double2 (.x = hi, .y = lo).  The exchange
 // tables a[u], q[l] reach 1e5..1e7 in magnitude while only their DIFFERENCES enter an exp, so
