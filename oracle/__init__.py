@@ -11,17 +11,23 @@ PAPER.md it follows); this file is ctypes marshalling only.
 from .binding import (  # noqa: F401
     OracleError,
     build,
+    conditioning,
     cycle_energies,
     cycle_energies_eq10,
     cycle_energy_eq7,
     eint,
     estimators,
+    estimators_species,
     external_force_on,
     forces,
+    forces_species,
+    pair_histogram,
     philox_normal,
     philox_raw,
     potential,
     pr_matrix,
+    set_pair_potential,
     step,
+    stream_forces_on,
     vb,
 )

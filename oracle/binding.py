@@ -172,3 +172,62 @@ def step(x, v, F, nhc, beta, omega, g, s, xi, dt, thermostat, gamma, seed, step0
                             C.c_double(g), C.c_double(s), C.c_double(xi), C.c_double(dt), int(thermostat),
                             C.c_double(gamma), C.c_uint64(seed), C.c_uint64(step0), int(nsteps)), "orc_step")
     return nhc
+
+
+def set_pair_potential(kind):
+    """0: v = g exp(-r^2/s^2) (default), 1: v = g / sqrt(r^2 + s^2).  Global switch of the oracle library."""
+    _load().orc_set_pair_potential(int(kind))
+
+
+def conditioning(x, beta, xi):
+    """kappa = max sum|terms| / |sum terms| over the signed sums of Eq. 6, 11, 12-14 (1 for xi >= 0)."""
+    x, N, P, d = _x(x)
+    k = C.c_double()
+    _check(_load().orc_conditioning(_dp(x), N, P, d, C.c_double(beta), C.c_double(xi), C.byref(k)), "orc_conditioning")
+    return k.value
+
+
+def forces_species(x, beta, omega, g, s, xi, counts):
+    x, N, P, d = _x(x)
+    F = np.zeros_like(x)
+    v, sg = C.c_double(), C.c_int()
+    cnt = (C.c_int * len(counts))(*[int(c) for c in counts])
+    _check(_load().orc_forces_species(_dp(x), N, P, d, C.c_double(beta), C.c_double(omega), C.c_double(g), C.c_double(s),
+                                      C.c_double(xi), len(counts), cnt, _dp(F), C.byref(v), C.byref(sg)), "orc_forces_species")
+    return F, v.value, sg.value
+
+
+def estimators_species(x, beta, omega, g, s, xi, counts, nbins=0, rmax=1.0):
+    x, N, P, d = _x(x)
+    ep, ev = C.c_double(), C.c_double()
+    hist = np.zeros(max(nbins, 1))
+    cnt = (C.c_int * len(counts))(*[int(c) for c in counts])
+    _check(_load().orc_estimators_species(_dp(x), N, P, d, C.c_double(beta), C.c_double(omega), C.c_double(g), C.c_double(s),
+                                          C.c_double(xi), len(counts), cnt, C.byref(ep), C.byref(ev), _dp(hist), int(nbins),
+                                          C.c_double(rmax)), "orc_estimators_species")
+    return ep.value, ev.value, hist[:nbins].copy()
+
+
+def pair_histogram(x, nbins, rmax):
+    x, N, P, d = _x(x)
+    hist = np.zeros(max(nbins, 1))
+    _check(_load().orc_pair_histogram(_dp(x), N, P, d, _dp(hist), int(nbins), C.c_double(rmax)), "orc_pair_histogram")
+    return hist[:nbins].copy()
+
+
+def stream_forces_on(x, beta, omega, g, s, xi, particles, tables=False):
+    """O(N)-memory evaluation: total force on every bead of the listed particles [k][P][d], V_B, sign
+    (and V^{[1,n]}, V^{[u,N]} with tables=True)."""
+    x, N, P, d = _x(x)
+    ls = np.ascontiguousarray(particles, dtype=np.int32)
+    F = np.zeros((len(ls), P, d))
+    v, sg = C.c_double(), C.c_int()
+    fwd = np.zeros(N + 1) if tables else None
+    bwd = np.zeros(N + 2) if tables else None
+    _check(_load().orc_stream_forces_on(_dp(x), N, P, d, C.c_double(beta), C.c_double(omega), C.c_double(g), C.c_double(s),
+                                        C.c_double(xi), ls.ctypes.data_as(C.POINTER(C.c_int)), len(ls), _dp(F), C.byref(v),
+                                        C.byref(sg), _dp(fwd) if tables else None, _dp(bwd) if tables else None),
+           "orc_stream_forces_on")
+    if tables:
+        return F, v.value, sg.value, fwd, bwd
+    return F, v.value, sg.value

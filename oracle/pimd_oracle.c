@@ -35,6 +35,12 @@
  *                  ensemble energy vs exact.  No reference trajectory
  *                  exists for the thermostat internals:                     PARITY UNPINNED
  *   orc_philox_normal  Philox4x32-10 known-answer vector (Random123 KAT)    PINNED
+ *   orc_stream_*   (O(N) memory) brute-force finite differences at small N,
+ *                  identical-ring closed form at N = 3000                   PINNED
+ *   orc_*_species  product of two composition sums, finite differences      PINNED
+ *   pair potential kind 1: finite differences, two-particle closed form     PINNED
+ *   orc_pair_histogram  numpy histogram of brute-force distances            PINNED
+ *   orc_conditioning    = 1 for xi >= 0; N = 2 closed form for xi < 0       PINNED
  */
 #include <math.h>
 #include <stdint.h>
@@ -301,14 +307,38 @@ int orc_exchange_forces(const double *x, const double *Pr, int N, int P, int d, 
     return ORC_OK;
 }
 
-/* -(1/P) grad U for U = sum_j [ sum_l 1/2 omega^2 |r_l^j|^2 + sum_{i<l} g e^{-|r_l^j-r_i^j|^2/s^2} ]
+/* The pair potential v(r) of Eq. 18 (PAPER.md:142-144 leaves V generic; Eq. 20, is the Gaussian
+ * instance), as a function of r^2:
+ *   kind 0 (default)  v = g exp(-r^2/s^2)
+ *   kind 1            v = g / sqrt(r^2 + s^2)          (soft Coulomb)
+ * *v = v(r), *fw = -(1/r) dv/dr (force on l from i is fw (r_l - r_i)), *vir = v + (r/2) dv/dr (virial estimator term). */
+static int g_pair_kind = 0;
+void orc_set_pair_potential(int kind) { g_pair_kind = kind; }
+
+static void pair_v(double r2, double g, double s, double *v, double *fw, double *vir)
+{
+    if (g_pair_kind == 0) {
+        const double is2 = 1.0 / (s * s);
+        const double e = g * exp(-r2 * is2);
+        *v = e;
+        *fw = 2.0 * is2 * e;
+        *vir = (1.0 - r2 * is2) * e;
+    } else {
+        const double q = r2 + s * s;
+        const double rq = sqrt(q);
+        *v = g / rq;
+        *fw = g / (q * rq);
+        *vir = *v - 0.5 * r2 * *fw;
+    }
+}
+
+/* -(1/P) grad U for U = sum_j [ sum_l 1/2 omega^2 |r_l^j|^2 + sum_{i<l} v(|r_l^j-r_i^j|) ], v = g e^{-r^2/s^2} by default
  * (Eq. 4, Eq. 18 :142, Eq. 19 :158, Eq. 20 :193).  Added into F.
  * Returns Ubar = U/P through *ubar if not NULL. */
 int orc_external_forces(const double *x, int N, int P, int d, double omega, double g, double s,
                         double *F, double *ubar_trap, double *ubar_pair)
 {
     const double invP = 1.0 / (double)P;
-    const double is2 = 1.0 / (s * s);
     long double ut = 0.0L, up = 0.0L;
     for (int j = 0; j < P; ++j) {
         for (int l = 0; l < N; ++l) {
@@ -330,8 +360,9 @@ int orc_external_forces(const double *x, int N, int P, int d, double omega, doub
             for (int i = 0; i < N; ++i) {
                 if (i == l) continue;
                 const double *ri = &x[IDX(j, i, 0)];
-                const double e = g * exp(-sqdist(rl, ri, d) * is2);
-                for (int c = 0; c < d; ++c) acc[c] += 2.0 * is2 * e * (rl[c] - ri[c]);
+                double e, fw, vir;
+                pair_v(sqdist(rl, ri, d), g, s, &e, &fw, &vir);
+                for (int c = 0; c < d; ++c) acc[c] += fw * (rl[c] - ri[c]);
                 if (i < l) up += e;
             }
             for (int c = 0; c < d; ++c) F[IDX(j, l, c)] += invP * acc[c];
@@ -348,14 +379,14 @@ int orc_external_force_on(const double *x, int N, int P, int d, double omega, do
                           int j, int l, double *f)
 {
     const double invP = 1.0 / (double)P;
-    const double is2 = 1.0 / (s * s);
     const double *rl = &x[IDX(j, l, 0)];
     long double acc[3] = {0.0L, 0.0L, 0.0L};
     for (int i = 0; i < N; ++i) {
         if (i == l) continue;
         const double *ri = &x[IDX(j, i, 0)];
-        const double e = g * exp(-sqdist(rl, ri, d) * is2);
-        for (int c = 0; c < d; ++c) acc[c] += 2.0 * is2 * e * (rl[c] - ri[c]);
+        double e, fw, vir;
+        pair_v(sqdist(rl, ri, d), g, s, &e, &fw, &vir);
+        for (int c = 0; c < d; ++c) acc[c] += fw * (rl[c] - ri[c]);
     }
     for (int c = 0; c < d; ++c) f[c] = invP * (double)acc[c] - invP * omega * omega * rl[c];
     return ORC_OK;
@@ -472,7 +503,7 @@ int orc_potential(const double *x, int N, int P, int d, double beta, double omeg
  *      eps^{(n)} = sum_k w_k (eps^{(n-k)} - E^{[n-k+1,n]}) / sum_k w_k,
  *      w_k = xi^{k-1} e^{-beta (E^{[n-k+1,n]} + V^{[1,n-k]})}   (from Eq. 6 with E ~ beta^-2)
  *  E_vir  = Ubar + 1/2 sum r . grad Ubar
- *         = (1/P) sum_j [ sum_l omega^2 |r|^2 + sum_{i<l} (1 - r^2/s^2) g e^{-r^2/s^2} ]
+ *         = (1/P) sum_j [ sum_l omega^2 |r|^2 + sum_{i<l} (v + r v'/2)(r) ],  (1 - r^2/s^2) g e^{-r^2/s^2} for the Gaussian
  *  hist[b] = number of beads with |r| in bin b of [0,rmax) (raw counts, nbins doubles);
  *  the density is hist / (N P shell volume), the harness normalises. */
 int orc_estimators(const double *x, int N, int P, int d, double beta, double omega, double g, double s,
@@ -511,7 +542,6 @@ int orc_estimators(const double *x, int N, int P, int d, double beta, double ome
     free(eps);
     ws_free(&w);
 
-    const double is2 = 1.0 / (s * s);
     long double ut = 0.0L, up = 0.0L, vir_pair = 0.0L;
     for (int b = 0; b < nbins; ++b) hist[b] = 0.0;
     for (int j = 0; j < P; ++j) {
@@ -530,10 +560,10 @@ int orc_estimators(const double *x, int N, int P, int d, double beta, double ome
             }
             if (g != 0.0) {
                 for (int i = 0; i < l; ++i) {
-                    const double rr = sqdist(rl, &x[IDX(j, i, 0)], d);
-                    const double e = g * exp(-rr * is2);
+                    double e, fw, vir;
+                    pair_v(sqdist(rl, &x[IDX(j, i, 0)], d), g, s, &e, &fw, &vir);
                     up += e;
-                    vir_pair += (1.0 - rr * is2) * e;
+                    vir_pair += vir;
                 }
             }
         }
@@ -682,5 +712,315 @@ int orc_cycle_energies_d(const double *x, int N, int P, int d, double beta, doub
         for (int u = 0; u < N; ++u)
             for (int v = 0; v < N; ++v) E[(size_t)u * N + v] = (v >= u) ? (double)El[(size_t)u * N + v] : 0.0;
     free(El);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------
+ * Conditioning of the signed sums (reading R7; xi < 0 lies outside the
+ * paper's stated domain).  kappa = the largest ratio
+ * sum|terms| / |sum terms| met in Eq. 6 (every n), in Eq. 11 (every u), and in
+ * the row and column sums of the quasi-probabilities of Eq. 12-14 (which are 1,
+ * so there it is sum |Pr|).  For xi >= 0 every term is positive and kappa = 1.
+ * The parity tolerance of a signed case is 1e-9 * kappa.
+ * ---------------------------------------------------------------------- */
+int orc_conditioning(const double *x, int N, int P, int d, double beta, double xi, double *kappa)
+{
+    orc_ws w;
+    int rc = ws_alloc(&w, N, 1);
+    if (rc) return rc;
+    rc = orc_cycle_energies(x, N, P, d, beta, w.E);
+    if (!rc) rc = orc_forward(w.E, N, beta, xi, w.L, w.sgL);
+    if (!rc) rc = orc_backward(w.E, N, beta, xi, w.M, w.sgM);
+    if (!rc) rc = orc_probabilities(w.E, w.L, w.sgL, w.M, w.sgM, N, beta, xi, w.Pr);
+    if (rc) { ws_free(&w); return rc; }
+    const long double lam = (xi != 0.0) ? logl(fabsl((long double)xi)) : 0.0L;
+    long double k = 1.0L;
+    for (int n = 1; n <= N; ++n) { /* Eq. 6: sum_k |term_k| / |sum| = sum_k exp(t_k - ln n - L_n) */
+        long double a = 0.0L;
+        for (int kk = 1; kk <= n; ++kk) {
+            if (xi == 0.0 && kk > 1) break;
+            a += expl((long double)(kk - 1) * lam - (long double)beta * w.E[(size_t)(n - kk) * N + (n - 1)] + w.L[n - kk]
+                      - logl((long double)n) - w.L[n]);
+        }
+        if (a > k) k = a;
+    }
+    for (int u = N; u >= 1; --u) { /* Eq. 11 */
+        long double a = 0.0L;
+        for (int l = u; l <= N; ++l) {
+            if (xi == 0.0 && l > u) break;
+            a += expl((long double)(l - u) * lam - logl((long double)l) - (long double)beta * w.E[(size_t)(u - 1) * N + (l - 1)]
+                      + w.M[l + 1] - w.M[u]);
+        }
+        if (a > k) k = a;
+    }
+    for (int l = 0; l < N; ++l) {
+        long double r = 0.0L, c = 0.0L;
+        for (int m = 0; m < N; ++m) {
+            r += fabsl((long double)w.Pr[(size_t)l * N + m]);
+            c += fabsl((long double)w.Pr[(size_t)m * N + l]);
+        }
+        if (r > k) k = r;
+        if (c > k) k = c;
+    }
+    *kappa = (double)k;
+    ws_free(&w);
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------
+ * Several species ("the spin unpolarized case"): particles
+ * [0, counts[0]) are species 0, the next counts[1] species 1, ...  Exchange acts
+ * within a species only, so V_xi = sum_s V_xi^{[range s]} (each by Eq. 6 on that
+ * species' particles alone); the trap and the pair potential act on all
+ * particles (Eq. 4, 18).  vb = sum over species, sign = product.
+ * ---------------------------------------------------------------------- */
+static double *sub_config(const double *x, int N, int P, int d, int l0, int n)
+{
+    double *xs = (double *)malloc(sizeof(double) * (size_t)n * P * d);
+    if (!xs) return NULL;
+    for (int j = 0; j < P; ++j)
+        for (int l = 0; l < n; ++l)
+            for (int c = 0; c < d; ++c) xs[(((size_t)j * n) + l) * d + c] = x[IDX(j, l0 + l, c)];
+    return xs;
+}
+
+int orc_forces_species(const double *x, int N, int P, int d, double beta, double omega, double g, double s, double xi,
+                       int nspecies, const int *counts, double *F, double *vb, int *sign)
+{
+    int l0 = 0, sg = 1;
+    long double v = 0.0L;
+    memset(F, 0, sizeof(double) * (size_t)N * P * d);
+    for (int sp = 0; sp < nspecies; ++sp) {
+        const int n = counts[sp];
+        double *xs = sub_config(x, N, P, d, l0, n);
+        double *Fs = (double *)malloc(sizeof(double) * (size_t)n * P * d);
+        if (!xs || !Fs) { free(xs); free(Fs); return ORC_ENOMEM; }
+        double vs;
+        int ss;
+        int rc = orc_forces(xs, n, P, d, beta, omega, g, s, xi, 0, Fs, &vs, &ss);
+        if (!rc)
+            for (int j = 0; j < P; ++j)
+                for (int l = 0; l < n; ++l)
+                    for (int c = 0; c < d; ++c) F[IDX(j, l0 + l, c)] = Fs[(((size_t)j * n) + l) * d + c];
+        free(xs);
+        free(Fs);
+        if (rc) return rc;
+        v += vs;
+        sg *= ss;
+        l0 += n;
+    }
+    if (l0 != N) return ORC_EINVAL;
+    int rc = orc_external_forces(x, N, P, d, omega, g, s, F, NULL, NULL);
+    if (vb) *vb = (double)v;
+    if (sign) *sign = sg;
+    return rc;
+}
+
+/* estimators with species: eps = d(beta V_xi)/d beta adds over species; the bead sums run over all particles.
+ * orc_estimators(x) = P d N/(2 beta) + eps + Ubar, so eps_s = orc_estimators(species s alone, omega = g = 0) - P d n_s/(2 beta). */
+int orc_estimators_species(const double *x, int N, int P, int d, double beta, double omega, double g, double s, double xi,
+                           int nspecies, const int *counts, double *e_prim, double *e_vir, double *hist, int nbins, double rmax)
+{
+    int l0 = 0;
+    long double eps = 0.0L;
+    for (int sp = 0; sp < nspecies; ++sp) {
+        const int n = counts[sp];
+        double *xs = sub_config(x, N, P, d, l0, n);
+        if (!xs) return ORC_ENOMEM;
+        double ep, ev;
+        int rc = orc_estimators(xs, n, P, d, beta, 0.0, 0.0, s, xi, &ep, &ev, NULL, 0, 1.0);
+        free(xs);
+        if (rc) return rc;
+        eps += (long double)ep - (long double)P * d * n / (2.0L * beta);
+        l0 += n;
+    }
+    if (l0 != N) return ORC_EINVAL;
+    /* the bead sums (Ubar, virial, histogram) of all particles: xi = 0 makes the exchange part of this call trivial and its
+     * eps (distinguishable rings) is taken out again */
+    double ep0, ev0, epd, evd;
+    int rc = orc_estimators(x, N, P, d, beta, omega, g, s, 0.0, &ep0, &ev0, hist, nbins, rmax);
+    if (!rc) rc = orc_estimators(x, N, P, d, beta, 0.0, 0.0, s, 0.0, &epd, &evd, NULL, 0, 1.0);
+    if (rc) return rc;
+    *e_prim = (double)((long double)ep0 - (long double)epd + (long double)P * d * N / (2.0L * beta) + eps);
+    *e_vir = ev0;
+    return ORC_OK;
+}
+
+/* Pair-distance histogram (pair-correlation estimator): counts of |r_l^j - r_i^j|, i < l, over all bead indices j
+ * (the pairs Eq. 18, couples) in nbins equal bins on [0, rmax); raw counts. */
+int orc_pair_histogram(const double *x, int N, int P, int d, double *hist, int nbins, double rmax)
+{
+    for (int b = 0; b < nbins; ++b) hist[b] = 0.0;
+    for (int j = 0; j < P; ++j)
+        for (int l = 0; l < N; ++l)
+            for (int i = 0; i < l; ++i) {
+                const double r = sqrt(sqdist(&x[IDX(j, l, 0)], &x[IDX(j, i, 0)], d));
+                if (r < rmax) {
+                    int b = (int)(r / rmax * nbins);
+                    if (b >= nbins) b = nbins - 1;
+                    hist[b] += 1.0;
+                }
+            }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------
+ * The same definitions with O(N) memory, for sizes whose N x N matrices do not
+ * fit (N = 4e4: 25.6 GB as long double): E^{[u,v]} is regenerated from Eq. 7's
+ * shared partial sums whenever Eq. 6 / Eq. 11 / Eq. 12 ask for it, nothing else
+ * changes.  For fixed v the walk u = v..1 is the one of orc_cycle_energies; for
+ * fixed u the walk v = u..N adds the same terms in the opposite order.
+ * ---------------------------------------------------------------------- */
+static void energies_to_v(const double *x, int N, int P, int d, double ks, const double *Eint, int v, long double *col)
+{
+    long double chain = 0.0L; /* col[u] = E^{[u+1,v+1]} (0-based u <= v) */
+    for (int u = v; u >= 0; --u) {
+        chain += (long double)Eint[u];
+        if (u < v) chain += (long double)closing(x, N, P, d, ks, u, u + 1);
+        col[u] = chain + (long double)closing(x, N, P, d, ks, v, u);
+    }
+}
+
+static void energies_from_u(const double *x, int N, int P, int d, double ks, const double *Eint, int u, long double *row)
+{
+    long double chain = 0.0L; /* row[v] = E^{[u+1,v+1]} (0-based v >= u) */
+    for (int v = u; v < N; ++v) {
+        chain += (long double)Eint[v];
+        if (v > u) chain += (long double)closing(x, N, P, d, ks, v - 1, v);
+        row[v] = chain + (long double)closing(x, N, P, d, ks, v, u);
+    }
+}
+
+/* Eq. 6 and Eq. 11 with regenerated energies: L[0..N], sgL, M[1..N+1] (M[0] unused), sgM; arrays of N+2. */
+int orc_stream_tables(const double *x, int N, int P, int d, double beta, double xi, long double *L, int *sgL,
+                      long double *M, int *sgM)
+{
+    if (N < 1 || P < 2 || d < 1 || !(beta > 0)) return ORC_EINVAL;
+    const double ks = (double)P / (beta * beta);
+    const long double lam = (xi != 0.0) ? logl(fabsl((long double)xi)) : 0.0L;
+    const int sx = xi < 0 ? -1 : 1;
+    double *Eint = (double *)malloc(sizeof(double) * (size_t)N);
+    long double *e = (long double *)malloc(sizeof(long double) * (size_t)N);
+    long double *t = (long double *)malloc(sizeof(long double) * (size_t)N);
+    int *s = (int *)malloc(sizeof(int) * (size_t)N);
+    if (!Eint || !e || !t || !s) { free(Eint); free(e); free(t); free(s); return ORC_ENOMEM; }
+    orc_eint(x, N, P, d, beta, Eint);
+    int rc = ORC_OK;
+    L[0] = 0.0L;
+    sgL[0] = 1;
+    for (int n = 1; n <= N && rc == ORC_OK; ++n) { /* Eq. 6 */
+        energies_to_v(x, N, P, d, ks, Eint, n - 1, e);
+        int cnt = 0;
+        for (int k = 1; k <= n; ++k) {
+            if (xi == 0.0 && k > 1) break;
+            const int u = n - k + 1;
+            t[cnt] = (long double)(k - 1) * lam - (long double)beta * e[u - 1] + L[n - k];
+            s[cnt] = (((k - 1) & 1) ? sx : 1) * sgL[n - k];
+            ++cnt;
+        }
+        long double lse;
+        int sgn;
+        rc = signed_lse(t, s, cnt, &lse, &sgn);
+        if (rc == ORC_OK) { L[n] = -logl((long double)n) + lse; sgL[n] = sgn; }
+    }
+    M[0] = 0.0L; sgM[0] = 1;
+    M[N + 1] = 0.0L; sgM[N + 1] = 1;
+    for (int u = N; u >= 1 && rc == ORC_OK; --u) { /* Eq. 11 */
+        energies_from_u(x, N, P, d, ks, Eint, u - 1, e);
+        int cnt = 0;
+        for (int l = u; l <= N; ++l) {
+            if (xi == 0.0 && l > u) break;
+            t[cnt] = (long double)(l - u) * lam - logl((long double)l) - (long double)beta * e[l - 1] + M[l + 1];
+            s[cnt] = (((l - u) & 1) ? sx : 1) * sgM[l + 1];
+            ++cnt;
+        }
+        long double lse;
+        int sgn;
+        rc = signed_lse(t, s, cnt, &lse, &sgn);
+        if (rc == ORC_OK) { M[u] = lse; sgM[u] = sgn; }
+    }
+    free(Eint); free(e); free(t); free(s);
+    return rc;
+}
+
+/* Total force F = -grad(V_xi + U/P) on every bead of the nl selected particles ls[] (0-based), Fsel[k][j][c], from
+ * Eq. 12-17 with regenerated energies; also V_B, its sign and (if not NULL) the tables V^{[1,n]}, n = 0..N, and
+ * V^{[u,N]}, u = 1..N+1 (index u; N+2 entries). */
+int orc_stream_forces_on(const double *x, int N, int P, int d, double beta, double omega, double g, double s, double xi,
+                         const int *ls, int nl, double *Fsel, double *vb, int *sign, double *vfwd, double *vbwd)
+{
+    if (N < 1 || P < 2 || d < 1 || d > 3 || !(beta > 0) || !(s > 0)) return ORC_EINVAL;
+    const double ks = (double)P / (beta * beta);
+    const long double lam = (xi != 0.0) ? logl(fabsl((long double)xi)) : 0.0L;
+    const int sx = xi < 0 ? -1 : 1;
+    long double *L = (long double *)malloc(sizeof(long double) * (size_t)(N + 2));
+    long double *M = (long double *)malloc(sizeof(long double) * (size_t)(N + 2));
+    int *sgL = (int *)malloc(sizeof(int) * (size_t)(N + 2)), *sgM = (int *)malloc(sizeof(int) * (size_t)(N + 2));
+    double *Eint = (double *)malloc(sizeof(double) * (size_t)N);
+    long double *e = (long double *)malloc(sizeof(long double) * (size_t)N);
+    double *pr = (double *)malloc(sizeof(double) * (size_t)N);
+    int rc = (!L || !M || !sgL || !sgM || !Eint || !e || !pr) ? ORC_ENOMEM : ORC_OK;
+    if (!rc) rc = orc_stream_tables(x, N, P, d, beta, xi, L, sgL, M, sgM);
+    if (!rc) {
+        orc_eint(x, N, P, d, beta, Eint);
+        if (vb) *vb = (double)(-L[N] / (long double)beta);
+        if (sign) *sign = sgL[N];
+        if (vfwd) for (int n = 0; n <= N; ++n) vfwd[n] = (double)(-L[n] / (long double)beta);
+        if (vbwd) { vbwd[0] = 0.0; for (int u = 1; u <= N + 1; ++u) vbwd[u] = (double)(-M[u] / (long double)beta); }
+    }
+    for (int k = 0; k < nl && !rc; ++k) {
+        const int l = ls[k] + 1; /* 1-based, as in the paper */
+        double *F = Fsel + (size_t)k * P * d;
+        memset(F, 0, sizeof(double) * (size_t)P * d);
+        for (int j = 1; j + 1 < P; ++j) /* Eq. 17 */
+            for (int c = 0; c < d; ++c)
+                F[j * d + c] = -ks * (2.0 * x[IDX(j, l - 1, c)] - x[IDX(j + 1, l - 1, c)] - x[IDX(j - 1, l - 1, c)]);
+        /* Eq. 16: bead P of l, weights Pr[G(l) = lp] -- Eq. 12 for lp <= l (energies E^{[lp,l]}), Eq. 13 for lp = l+1 */
+        energies_to_v(x, N, P, d, ks, Eint, l - 1, e);
+        for (int lp = 1; lp <= N; ++lp) {
+            double p = 0.0;
+            if (lp <= l) {
+                if (!(xi == 0.0 && lp < l)) {
+                    long double ex = (long double)(l - lp) * lam - logl((long double)l) + L[lp - 1] - (long double)beta * e[lp - 1] + M[l + 1] - L[N];
+                    p = (double)((((l - lp) & 1) ? sx : 1) * sgL[lp - 1] * sgM[l + 1] * sgL[N]) * exp((double)ex);
+                }
+            } else if (lp == l + 1) {
+                p = 1.0 - (double)(sgL[l] * sgM[l + 1] * sgL[N]) * exp((double)(L[l] + M[l + 1] - L[N]));
+            }
+            pr[lp - 1] = p;
+        }
+        for (int c = 0; c < d; ++c) {
+            long double fP = 0.0L;
+            for (int lp = 0; lp < N; ++lp)
+                fP -= (long double)pr[lp] * ks * (2.0 * x[IDX(P - 1, l - 1, c)] - x[IDX(P - 2, l - 1, c)] - x[IDX(0, lp, c)]);
+            F[(P - 1) * d + c] += (double)fP;
+        }
+        /* Eq. 15: bead 1 of l, weights Pr[G(lp) = l] -- Eq. 12 for lp >= l (energies E^{[l,lp]}), Eq. 13 for lp = l-1 */
+        energies_from_u(x, N, P, d, ks, Eint, l - 1, e);
+        for (int lp = 1; lp <= N; ++lp) {
+            double p = 0.0;
+            if (lp >= l) {
+                if (!(xi == 0.0 && lp > l)) {
+                    long double ex = (long double)(lp - l) * lam - logl((long double)lp) + L[l - 1] - (long double)beta * e[lp - 1] + M[lp + 1] - L[N];
+                    p = (double)((((lp - l) & 1) ? sx : 1) * sgL[l - 1] * sgM[lp + 1] * sgL[N]) * exp((double)ex);
+                }
+            } else if (lp == l - 1) {
+                p = 1.0 - (double)(sgL[lp] * sgM[lp + 1] * sgL[N]) * exp((double)(L[lp] + M[lp + 1] - L[N]));
+            }
+            pr[lp - 1] = p;
+        }
+        for (int c = 0; c < d; ++c) {
+            long double f1 = 0.0L;
+            for (int lp = 0; lp < N; ++lp)
+                f1 -= (long double)pr[lp] * ks * (2.0 * x[IDX(0, l - 1, c)] - x[IDX(1, l - 1, c)] - x[IDX(P - 1, lp, c)]);
+            F[c] += (double)f1;
+        }
+        for (int j = 0; j < P; ++j) { /* -(1/P) grad U */
+            double fe[3];
+            orc_external_force_on(x, N, P, d, omega, g, s, j, l - 1, fe);
+            for (int c = 0; c < d; ++c) F[j * d + c] += fe[c];
+        }
+    }
+    free(L); free(M); free(sgL); free(sgM); free(Eint); free(e); free(pr);
     return rc;
 }
