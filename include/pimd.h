@@ -54,6 +54,10 @@ extern "C" {
 #define PIMD_THERMOSTAT_LANGEVIN 1 /* OBABO, friction gamma (default 1), Philox4x32-10 noise */
 #define PIMD_THERMOSTAT_NHC 2      /* massive Nose-Hoover chains, length 4, Q = beta/P */
 #define PIMD_NHC_LENGTH 4
+#define PIMD_MAX_SPECIES 4
+#define PIMD_MAX_BINS 4096         /* histogram bins (radial density, pair distances) */
+#define PIMD_PAIR_GAUSSIAN 0       /* v(r) = g exp(-r^2/s^2)      (Eq. 20, with g = g_paper/(pi s^2)) */
+#define PIMD_PAIR_SOFT_COULOMB 1   /* v(r) = g / sqrt(r^2 + s^2)  (Eq. 18, leaves the pair potential open) */
 
 typedef struct pimd_s *pimd_t; /* opaque; owns its device workspace unless one is supplied */
 
@@ -65,6 +69,27 @@ typedef struct pimd_s *pimd_t; /* opaque; owns its device workspace unless one i
 int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, double g, double s,
                 double xi, double dt, int thermostat, uint64_t seed);
 int pimd_destroy(pimd_t h);
+
+/* A batch of B replicas of the same system that differ in the exchange parameter xi[b] and the noise seed[b] (HOST
+ * arrays of B entries), advanced by one set of kernel launches (replica = a grid dimension).  This is how the method is
+ * used for fictitious particles: simulate at several xi >= 0 and extrapolate / reweight; it also
+ * fills the GPU at small N.  Either every xi[b] is 0 or none is.  With a batch every state / force array of this header
+ * is [B][P][N][d] and every per-evaluation HOST output (vb, sign, e_prim, e_vir, hist, ...) has B entries (hist: [B][nbins]);
+ * pimd_create() is the batch with B = 1.  B is limited by the co-resident CTAs of the recursion kernel (2 per replica and
+ * direction at small N; 74 replicas at N <= 128 on a B200). */
+int pimd_create_batch(pimd_t *out, int B, int N, int P, int d, double beta, double omega, double g, double s,
+                      const double *xi, double dt, int thermostat, const uint64_t *seed);
+
+/* Several species of identical particles (the spin-unpolarised case): particles [0, counts[0]) are species
+ * 0, the next counts[1] species 1, ...; exchange (Eq. 6, 11-16) acts within a species only, V_xi = sum over species of
+ * V_xi^{[range]}, the trap and pair terms act on all particles alike.  counts: HOST, nspecies <= PIMD_MAX_SPECIES
+ * entries that add up to N.  Must precede the first state / compute call.  vb returned by pimd_forces is the sum over
+ * species, sign the product. */
+int pimd_set_species(pimd_t h, int nspecies, const int *counts);
+
+/* Pair potential between same-index beads (Eq. 18): PIMD_PAIR_GAUSSIAN (default) or PIMD_PAIR_SOFT_COULOMB,
+ * both with the g and s of pimd_create. */
+int pimd_set_pair_potential(pimd_t h, int kind);
 
 /* cuda_stream is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default. */
 int pimd_set_stream(pimd_t h, void *cuda_stream);
@@ -138,9 +163,68 @@ int pimd_step(pimd_t h, int nsteps);
 /* Estimators at the current positions (R9, R15), HOST outputs:
  *   e_prim = P d N/(2 beta) - <E_c> + Ubar   (thermodynamic estimator, -d ln Z/d beta of Eq. 4)
  *   e_vir  = Ubar + 1/2 sum r.grad Ubar       (virial estimator; valid in the trap)
- *   hist[b], b < nbins: number of beads with |r| in [b, b+1) * rmax/nbins (raw counts as doubles;
+ *   hist[b], b < nbins <= PIMD_MAX_BINS: number of beads with |r| in [b, b+1) * rmax/nbins (raw counts as doubles;
  *   beads with |r| >= rmax are dropped).  nbins may be 0 (hist ignored).  Synchronises. */
 int pimd_estimators(pimd_t h, double *e_prim, double *e_vir, double *hist, int nbins, double rmax);
+
+/* pimd_step with sampling: every step whose number (pimd_get_step_count after it) is a multiple of est_every > 0 makes
+ * its force evaluation in estimator mode and adds e_prim, e_vir, the radial histogram (nbins bins on [0, rmax)) and the
+ * pair-distance histogram (if pimd_set_pair_histogram is on) to running sums on the device.  Asynchronous; no extra
+ * force evaluation is made for the estimators.  pimd_read_accumulators() synchronises and returns, per replica, the
+ * number of samples and the sums (HOST; any pointer may be NULL; hist_sum [B][nbins], gr_sum [B][nbins_gr]); reset != 0
+ * clears them afterwards. */
+int pimd_run(pimd_t h, int nsteps, int est_every, int nbins, double rmax);
+int pimd_read_accumulators(pimd_t h, double *nsamples, double *sum_eprim, double *sum_evir, double *hist_sum, int nbins,
+                           double *gr_sum, int nbins_gr, int reset);
+
+/* Pair-correlation estimator: histogram of the distances |r_l^j - r_i^j|, i < l, over all bead indices j (the pairs
+ * Eq. 18, couples), nbins <= PIMD_MAX_BINS equal bins on [0, rmax), raw counts (normalisation by the caller).
+ * Once switched on (nbins > 0) every estimator evaluation (pimd_estimators, sampling steps of pimd_run) fills it;
+ * pimd_pair_histogram() returns the one of the last estimator evaluation (HOST, [B][nbins]). */
+int pimd_set_pair_histogram(pimd_t h, int nbins, double rmax);
+int pimd_pair_histogram(pimd_t h, double *gr_host);
+
+/* Reweighting to a second exchange parameter (R7): the recursion of Eq. 6 is
+ * evaluated at the current positions with xi_obs[b] (HOST, B entries) beside the sampling xi.  HOST outputs, B entries
+ * each, any may be NULL:
+ *   ln_abs_r = ln |W_{xi_obs} / W_{xi}| = -beta (V_{xi_obs} - V_{xi}),  sign = sign of that ratio,
+ *   eps_obs, eps_samp = d(beta V)/d beta = -<E_c> at xi_obs / at the sampling xi,
+ * so that the primitive energy estimator at xi_obs is e_prim (of pimd_estimators) - eps_samp + eps_obs and an observable O
+ * at xi_obs is <O R> / <R> with R = sign exp(ln_abs_r) over a run at the sampling xi.  Synchronises.  PIMD_ENUMERIC if
+ * W_{xi_obs} is exactly zero. */
+int pimd_reweight(pimd_t h, const double *xi_obs, double *ln_abs_r, int *sign, double *eps_obs, double *eps_samp);
+
+/* Bead shards (multi-GPU, one process per GPU).  Rank `rank` of `world` holds the bead slices
+ * [floor(P rank/world), floor(P (rank+1)/world)) of every ring polymer: its state / force arrays are [P_local][N][d].
+ * Springs, trap, pair forces, integrator and the bead sums of the estimators are local; the exchange part (steps 3-6,
+ * O(N^2) against O(P N^2 / world) for the pair part) runs redundantly on every rank.  One exchange step per MD step: the
+ * all-gather (by the caller: NCCL through torch.distributed, or a device copy between shards on one GPU) of every
+ * rank's boundary pack of `pack_doubles` = 2 N d + N doubles:
+ *     [ first local slice : N d ][ last local slice : N d ][ E_int of the springs between local slices : N ].
+ *   pimd_shard_export(h, send_dev)          write this rank's pack (DEVICE out); asynchronous
+ *   pimd_shard_forces(h, gathered_dev)      take the gathered packs (DEVICE, world * pack_doubles, rank-major; copied)
+ *                                           and evaluate the forces of the local slices; asynchronous
+ *   pimd_shard_begin_step(h, send_dev)      thermostat half ; v += dt/2 F ; x += dt v ; export
+ *   pimd_shard_end_step(h, gathered_dev)    import ; forces ; v += dt/2 F ; thermostat half
+ *   pimd_shard_scalars(h, vb, sign)         V_B and sign of the last pimd_shard_forces (HOST; synchronises)
+ * pimd_get_forces / pimd_get_state / pimd_set_state act on the local slices.  pimd_estimators on a shard returns this
+ * rank's share (the bead sums over its slices; the kinetic constant and <E_c> on rank 0 only): the sum over ranks is the
+ * estimator.  The Langevin noise of a degree of freedom is keyed by its global index, so a sharded run reproduces the
+ * single-GPU trajectory.  pimd_forces, pimd_step, pimd_run, pimd_reweight refuse a shard (PIMD_EINVAL). */
+int pimd_create_sharded(pimd_t *out, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
+                        double xi, double dt, int thermostat, uint64_t seed);
+int pimd_shard_layout(pimd_t h, int *j0, int *p_local, size_t *pack_doubles);
+int pimd_shard_export(pimd_t h, double *send_dev);
+int pimd_shard_forces(pimd_t h, const double *gathered_dev);
+int pimd_shard_begin_step(pimd_t h, double *send_dev);
+int pimd_shard_end_step(pimd_t h, const double *gathered_dev);
+int pimd_shard_scalars(pimd_t h, double *vb, int *sign);
+
+/* Diagnostics (HOST out, 4 entries; synchronises): [0] force evaluations since creation in which the recursion with the
+ * previous evaluation's gauge was rejected and redone with a fresh max-plus gauge, [1] PIMD status bits (1 non-finite,
+ * 2 node) seen in any evaluation since the last pimd_set_state, [2] panel worker CTAs per direction, [3] bytes between
+ * replicas in the workspace. */
+int pimd_get_diagnostics(pimd_t h, uint64_t *out);
 
 /* Device time of the kernels of the last pimd_forces()/pimd_step() force evaluation is not
  * recorded here; use CUDA events on the stream.  The number of kernel launches issued by the
@@ -156,14 +240,15 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_CHAIN 2     /* forward + backward recursions (steps 4, 5) */
 #define PIMD_PROF_FORCEPASS 3 /* connection probabilities and their sums (step 6) */
 #define PIMD_PROF_ASSEMBLE 4  /* Eq. 13 and exterior forces (step 6) */
-#define PIMD_PROF_FINALIZE 5  /* V_B, sign, <E_c> */
+#define PIMD_PROF_FINALIZE 5  /* V_B, sign, <E_c>; estimator arithmetic */
 #define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
 #define PIMD_PROF_COMBINE 7   /* force output */
 #define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
-#define PIMD_PROF_CHAIN_FALLBACK 9 /* unused (always 0 launches): the safety net now runs inside the CHAIN launch */
-#define PIMD_PROF_EMAT 10     /* pimd_cycle_energies: the N x N write */
-#define PIMD_PROF_PRMAT 11    /* pimd_connection_probabilities: the N x N write */
-#define PIMD_PROF_NSLOTS 12
+#define PIMD_PROF_EMAT 9      /* pimd_cycle_energies: the N x N write */
+#define PIMD_PROF_PRMAT 10    /* pimd_connection_probabilities: the N x N write */
+#define PIMD_PROF_GR 11       /* pair-distance histogram (estimator steps, pimd_set_pair_histogram) */
+#define PIMD_PROF_SHARD 12    /* bead shards: boundary pack / E_int assembly */
+#define PIMD_PROF_NSLOTS 13
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM

@@ -15,14 +15,34 @@ LIB_PATH = os.path.join(_HERE, "libpimd.so")
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 THERMOSTAT_NVE, THERMOSTAT_LANGEVIN, THERMOSTAT_NHC = 0, 1, 2
 NHC_LENGTH = 4
-PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine", "pair", "chain_fallback", "emat", "prmat")
+PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine", "pair", "emat", "prmat", "gr", "shard")
+MAX_SPECIES, MAX_BINS = 4, 4096
+PAIR_GAUSSIAN, PAIR_SOFT_COULOMB = 0, 1
 
 # every symbol include/pimd.h declares: (restype, argtypes)
 _dp = C.POINTER(C.c_double)
 _SYMBOLS = {
     "pimd_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                               C.c_double, C.c_double, C.c_double, C.c_int, C.c_uint64]),
+    "pimd_create_batch": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                    C.c_double, _dp, C.c_double, C.c_int, C.POINTER(C.c_uint64)]),
+    "pimd_create_sharded": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                      C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, C.c_uint64]),
     "pimd_destroy": (C.c_int, [C.c_void_p]),
+    "pimd_set_species": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int)]),
+    "pimd_set_pair_potential": (C.c_int, [C.c_void_p, C.c_int]),
+    "pimd_set_pair_histogram": (C.c_int, [C.c_void_p, C.c_int, C.c_double]),
+    "pimd_pair_histogram": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_run": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double]),
+    "pimd_read_accumulators": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int]),
+    "pimd_reweight": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_shard_layout": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_size_t)]),
+    "pimd_shard_export": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_shard_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_shard_begin_step": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_shard_end_step": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_shard_scalars": (C.c_int, [C.c_void_p, _dp, C.POINTER(C.c_int)]),
+    "pimd_get_diagnostics": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_stream": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_workspace_bytes": (C.c_size_t, [C.c_void_p]),
     "pimd_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
@@ -36,8 +56,8 @@ _SYMBOLS = {
     "pimd_set_step_count": (C.c_int, [C.c_void_p, C.c_uint64]),
     "pimd_get_nhc": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_nhc": (C.c_int, [C.c_void_p, C.c_void_p]),
-    "pimd_forces": (C.c_int, [C.c_void_p, C.c_void_p, _dp, C.POINTER(C.c_int)]),
-    "pimd_forces_host": (C.c_int, [C.c_void_p, C.c_void_p, _dp, C.POINTER(C.c_int)]),
+    "pimd_forces": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pimd_forces_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_get_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_get_forces_host": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_set_forces": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -46,7 +66,7 @@ _SYMBOLS = {
     "pimd_cycle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_connection_probabilities": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_step": (C.c_int, [C.c_void_p, C.c_int]),
-    "pimd_estimators": (C.c_int, [C.c_void_p, _dp, _dp, C.c_void_p, C.c_int, C.c_double]),
+    "pimd_estimators": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double]),
     "pimd_launch_count": (C.c_uint64, [C.c_void_p]),
     "pimd_set_profiling": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_get_profile": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
@@ -94,15 +114,33 @@ def _ptr(t):
 
 
 class Pimd:
-    """One simulation handle.  Method names mirror the C entry points (pimd_<name>)."""
+    """One simulation handle.  Method names mirror the C entry points (pimd_<name>).
+
+    xi / seed given as sequences make a batch of B replicas (pimd_create_batch): state and force tensors are then
+    [B][P][N][d] and per-evaluation scalars come back as numpy arrays of B entries.  shard=(rank, world) makes a bead
+    shard (pimd_create_sharded) holding P_local slices.  species=(n0, n1, ..) calls pimd_set_species."""
 
     def __init__(self, N, P, d, beta, omega, g, s, xi, dt, thermostat=THERMOSTAT_LANGEVIN, seed=0,
-                 stream=None, use_torch_workspace=True):
+                 stream=None, use_torch_workspace=True, species=None, pair_potential=None, shard=None):
         self._lib = load()
         self._h = C.c_void_p()
         self.N, self.P, self.d = int(N), int(P), int(d)
-        rc = self._lib.pimd_create(C.byref(self._h), int(N), int(P), int(d), float(beta), float(omega), float(g),
-                                   float(s), float(xi), float(dt), int(thermostat), int(seed))
+        self.batched = hasattr(xi, "__len__")
+        if self.batched:
+            xs = [float(v) for v in xi]
+            sd = [int(v) for v in seed] if hasattr(seed, "__len__") else [int(seed) + k for k in range(len(xs))]
+            self.B = len(xs)
+            rc = self._lib.pimd_create_batch(C.byref(self._h), self.B, int(N), int(P), int(d), float(beta), float(omega), float(g),
+                                             float(s), (C.c_double * self.B)(*xs), float(dt), int(thermostat),
+                                             (C.c_uint64 * self.B)(*sd))
+        elif shard is not None:
+            self.B = 1
+            rc = self._lib.pimd_create_sharded(C.byref(self._h), int(shard[0]), int(shard[1]), int(N), int(P), int(d), float(beta),
+                                               float(omega), float(g), float(s), float(xi), float(dt), int(thermostat), int(seed))
+        else:
+            self.B = 1
+            rc = self._lib.pimd_create(C.byref(self._h), int(N), int(P), int(d), float(beta), float(omega), float(g),
+                                       float(s), float(xi), float(dt), int(thermostat), int(seed))
         if rc != OK:
             raise PimdError(rc, self._lib.pimd_last_error(None).decode())
         self._ws = None
@@ -112,6 +150,12 @@ class Pimd:
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
         self._check(self._lib.pimd_set_stream(self._h, C.c_void_p(stream)))
+        if species is not None:
+            cnt = [int(c) for c in species]
+            self._check(self._lib.pimd_set_species(self._h, len(cnt), (C.c_int * len(cnt))(*cnt)))
+        if pair_potential is not None:
+            self._check(self._lib.pimd_set_pair_potential(self._h, int(pair_potential)))
+        self.P_local, self.j0, self.pack_doubles = self.shard_layout()
         if use_torch_workspace:
             nbytes = self._lib.pimd_workspace_bytes(self._h)
             self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
@@ -136,7 +180,12 @@ class Pimd:
             pass
 
     def _empty_state(self):
-        return self._torch.empty((self.P, self.N, self.d), dtype=self._torch.float64, device="cuda")
+        shape = (self.P_local, self.N, self.d)
+        return self._torch.empty(((self.B,) + shape) if self.batched else shape, dtype=self._torch.float64, device="cuda")
+
+    def _scalars(self, arr):
+        """per-replica HOST outputs: a numpy array for a batch, a plain number otherwise"""
+        return arr.copy() if self.batched else arr[0].item()
 
     # -- C ABI mirrors
     def set_stream(self, cuda_stream):
@@ -172,7 +221,8 @@ class Pimd:
         self._check(self._lib.pimd_set_step_count(self._h, int(step)))
 
     def get_nhc(self):
-        t = self._torch.empty((NHC_LENGTH, self.P * self.N * self.d), dtype=self._torch.float64, device="cuda")
+        shape = (NHC_LENGTH, self.P_local * self.N * self.d)
+        t = self._torch.empty(((self.B,) + shape) if self.batched else shape, dtype=self._torch.float64, device="cuda")
         self._check(self._lib.pimd_get_nhc(self._h, _ptr(t)))
         return t
 
@@ -181,17 +231,21 @@ class Pimd:
 
     def forces(self, out=None, want_forces=True):
         """(F [P][N][d] device tensor or None, V_B, sign)."""
+        import numpy as np
+
         f = None
         if want_forces:
             f = out if out is not None else self._empty_state()
-        vb, sg = C.c_double(), C.c_int()
-        self._check(self._lib.pimd_forces(self._h, _ptr(f), C.byref(vb), C.byref(sg)))
-        return f, vb.value, sg.value
+        vb, sg = np.zeros(self.B), np.zeros(self.B, dtype=np.int32)
+        self._check(self._lib.pimd_forces(self._h, _ptr(f), _ptr(vb), _ptr(sg)))
+        return f, self._scalars(vb), self._scalars(sg)
 
     def forces_host(self, f_host):
-        vb, sg = C.c_double(), C.c_int()
-        self._check(self._lib.pimd_forces_host(self._h, _ptr(f_host), C.byref(vb), C.byref(sg)))
-        return vb.value, sg.value
+        import numpy as np
+
+        vb, sg = np.zeros(self.B), np.zeros(self.B, dtype=np.int32)
+        self._check(self._lib.pimd_forces_host(self._h, _ptr(f_host), _ptr(vb), _ptr(sg)))
+        return self._scalars(vb), self._scalars(sg)
 
     def get_forces(self, out=None):
         f = out if out is not None else self._empty_state()
@@ -239,10 +293,78 @@ class Pimd:
     def estimators(self, nbins=0, rmax=1.0):
         import numpy as np
 
-        ep, ev = C.c_double(), C.c_double()
-        hist = np.zeros(max(int(nbins), 1))
-        self._check(self._lib.pimd_estimators(self._h, C.byref(ep), C.byref(ev), _ptr(hist), int(nbins), float(rmax)))
-        return ep.value, ev.value, hist[: int(nbins)].copy()
+        ep, ev = np.zeros(self.B), np.zeros(self.B)
+        hist = np.zeros((self.B, max(int(nbins), 1)))
+        self._check(self._lib.pimd_estimators(self._h, _ptr(ep), _ptr(ev), _ptr(hist), int(nbins), float(rmax)))
+        hist = hist[:, : int(nbins)].copy()
+        return self._scalars(ep), self._scalars(ev), (hist if self.batched else hist[0])
+
+    def run(self, nsteps, est_every=0, nbins=0, rmax=1.0):
+        self._check(self._lib.pimd_run(self._h, int(nsteps), int(est_every), int(nbins), float(rmax)))
+
+    def read_accumulators(self, nbins=0, nbins_gr=0, reset=True):
+        """(number of samples, sum e_prim, sum e_vir, radial histogram sum, pair histogram sum) per replica."""
+        import numpy as np
+
+        n, sp, sv = np.zeros(self.B), np.zeros(self.B), np.zeros(self.B)
+        hs, gs = np.zeros((self.B, max(int(nbins), 1))), np.zeros((self.B, max(int(nbins_gr), 1)))
+        self._check(self._lib.pimd_read_accumulators(self._h, _ptr(n), _ptr(sp), _ptr(sv), _ptr(hs), int(nbins), _ptr(gs),
+                                                     int(nbins_gr), int(bool(reset))))
+        hs, gs = hs[:, : int(nbins)], gs[:, : int(nbins_gr)]
+        if not self.batched:
+            hs, gs = hs[0], gs[0]
+        return self._scalars(n), self._scalars(sp), self._scalars(sv), hs.copy(), gs.copy()
+
+    def set_pair_potential(self, kind):
+        self._check(self._lib.pimd_set_pair_potential(self._h, int(kind)))
+
+    def set_pair_histogram(self, nbins, rmax):
+        self._nbins_gr = int(nbins)
+        self._check(self._lib.pimd_set_pair_histogram(self._h, int(nbins), float(rmax)))
+
+    def pair_histogram(self):
+        import numpy as np
+
+        g = np.zeros((self.B, max(getattr(self, "_nbins_gr", 0), 1)))
+        self._check(self._lib.pimd_pair_histogram(self._h, _ptr(g)))
+        return g.copy() if self.batched else g[0].copy()
+
+    def reweight(self, xi_obs):
+        """(ln|R|, sign, eps_obs, eps_samp) per replica for R = W_{xi_obs} / W_{xi} at the current positions."""
+        import numpy as np
+
+        xo = np.ascontiguousarray(np.broadcast_to(np.asarray(xi_obs, dtype=np.float64), (self.B,)))
+        lr, sg, eo, es = np.zeros(self.B), np.zeros(self.B, dtype=np.int32), np.zeros(self.B), np.zeros(self.B)
+        self._check(self._lib.pimd_reweight(self._h, _ptr(xo), _ptr(lr), _ptr(sg), _ptr(eo), _ptr(es)))
+        return self._scalars(lr), self._scalars(sg), self._scalars(eo), self._scalars(es)
+
+    # -- bead shards
+    def shard_layout(self):
+        j0, pl, n = C.c_int(), C.c_int(), C.c_size_t()
+        self._check(self._lib.pimd_shard_layout(self._h, C.byref(j0), C.byref(pl), C.byref(n)))
+        return pl.value, j0.value, n.value
+
+    def shard_export(self, send_dev):
+        self._check(self._lib.pimd_shard_export(self._h, _ptr(send_dev)))
+
+    def shard_forces(self, gathered_dev):
+        self._check(self._lib.pimd_shard_forces(self._h, _ptr(gathered_dev)))
+
+    def shard_begin_step(self, send_dev):
+        self._check(self._lib.pimd_shard_begin_step(self._h, _ptr(send_dev)))
+
+    def shard_end_step(self, gathered_dev):
+        self._check(self._lib.pimd_shard_end_step(self._h, _ptr(gathered_dev)))
+
+    def shard_scalars(self):
+        vb, sg = C.c_double(), C.c_int()
+        self._check(self._lib.pimd_shard_scalars(self._h, C.byref(vb), C.byref(sg)))
+        return vb.value, sg.value
+
+    def get_diagnostics(self):
+        out = (C.c_uint64 * 4)()
+        self._check(self._lib.pimd_get_diagnostics(self._h, out))
+        return {"fallbacks": int(out[0]), "status_seen": int(out[1]), "workers": int(out[2]), "replica_stride": int(out[3])}
 
     def set_profiling(self, on):
         self._check(self._lib.pimd_set_profiling(self._h, int(bool(on))))

@@ -22,55 +22,82 @@ thread_local char g_create_error[512] = "";
 constexpr int BEAD_TB = 128;
 constexpr int PREP_TB = 64;
 constexpr int ASM_TB = 128;
-constexpr int MAX_BINS = 1 << 16;
+constexpr int MAX_BINS = GR_MAXBINS;
+
+// One exchange problem: the recursion of Eq. 6 / Eq. 11 over the particles [l0, l0 + N) of one species
+// (several species = independent recursions over index ranges) with one parameter set
+// (the sampling xi, or the second xi of pimd_reweight).  Pointers are those of replica 0.
+struct ExchCtx {
+    int N, l0, NB, nprep, nasm, nworkers;
+    ExchPtrs p;
+    Scalars *scal;
+    double *ecpart;
+    RepParams *rp;
+    bool gauge_valid; // p.g / p.gs hold the (T, Zhat) of a completed evaluation of nearby positions
+};
 
 } // namespace
 
 struct pimd_s {
-    int N, P, d;
-    double beta, omega, g, s, xi, dt, gamma;
-    int thermostat;
-    uint64_t seed, step;
+    int B, N, P, d;         // replicas, particles, bead slices held here (= Pg unless sharded), dimensions
+    int Pg, j0, rank, world; // bead shards: global slice count, first local slice, rank of world
+    bool sharded;
+    double beta, omega, g, s, dt, gamma;
+    int thermostat, pot;
+    std::vector<double> *xi, *xi2;
+    std::vector<uint64_t> *seed;
+    bool any_neg[2], all_zero[2]; // per parameter set (0: sampling xi, 1: reweighting xi)
+    uint64_t step;
+    int nspecies, counts[PIMD_MAX_SPECIES];
     // derived
-    double ks, kk, lambda;
+    double ks, kk;
     size_t ndof, slice;
-    int NB, nprep, nasm, look, look_spec, nworkers, sms;
+    int look, look_spec, sms;
     // streams
     cudaStream_t s0, s1;
     cudaEvent_t ev_fork, ev_join;
     bool concurrent;
-    // memory
+    // memory: [global region][replica 0][replica 1]...; pointers below are replica 0's
     unsigned char *ws;
-    size_t ws_bytes;
+    size_t ws_bytes, rstride;
     bool own_ws, carved;
-    double *x, *v, *F, *Fout, *nhc, *Fex1, *FexP, *ecpart, *hist, *Sarr, *Tarr;
-    ExchPtrs ex;
-    Scalars *scal;
+    double *x, *v, *F, *nhc, *Fex1, *FexP, *Fexs1, *FexsP, *hist, *hist_acc, *gr, *gr_acc;
+    ExchCtx ex[2][PIMD_MAX_SPECIES]; // [parameter set][species]
+    RepParams *rp[2];
+    Scalars *scal[2];
     EstAccum *est;
-    int *status;
-    unsigned long long *phase; // chain phase clock (profiling)
-    unsigned long long *dstep; // MD step counter on the device (graph replay)
+    EstSums *sums;
+    int *istatus;
+    // global region
+    double *Fout, *gathered, *eint_tot, *pack, *Sarr, *Tarr;
+    int *gflags;
+    unsigned long long *fallbacks, *phase, *dstep;
     // one MD step (force evaluation, then close + open) captured as a CUDA graph on an internal stream
     cudaStream_t sg;
     cudaEvent_t ev_gin, ev_gout;
-    cudaGraphExec_t gexec;
+    cudaGraphExec_t gexec, gexec_est;
     bool use_graph, graph_failed, graph_conc;
-    uint64_t graph_launches;
+    int graph_nbins, graph_nbins_gr;
+    double graph_rmax, graph_rmax_gr;
+    uint64_t graph_launches, graph_est_launches;
     // pinned host mirrors
-    Scalars *h_scal;
-    EstAccum *h_est;
-    int *h_status;
+    Scalars *h_scal;   // [B * MAX_SPECIES]
+    EstSums *h_sums;   // [B]
+    int *h_status;     // [B * (1 + 2 * MAX_SPECIES)]
+    unsigned long long *h_diag;
     bool forces_valid;
-    bool tables_valid; // the exchange tables (g, gs, pnext, rfin) belong to the current positions
-    bool gauge_valid; // g/gs hold the (T, Zhat) of a completed evaluation of nearby positions
-    bool use_spec;    // PIMD_NOSPEC=1 turns the stale-gauge kernel off
-    size_t spec_smem;
+    bool tables_valid; // the exchange tables of parameter set 0 belong to the current positions
+    bool scalars_valid; // ... and k_finalize has run on them
+    bool shard_imported;
+    bool use_spec;     // PIMD_NOSPEC=1 turns the stale-gauge kernel off
+    size_t spec_smem, chain_smem;
     int coop_max_blocks; // co-resident CTA limit of k_chain
-    size_t chain_smem;
     uint64_t launches;
+    int nbins_gr;
+    double rmax_gr;
     // per-kernel device timing (pimd_set_profiling)
     bool profiling;
-    std::vector<cudaEvent_t> *prof_ev;   // pairs (start, stop)
+    std::vector<cudaEvent_t> *prof_ev; // pairs (start, stop)
     std::vector<int> *prof_slot;
     double prof_ms[PIMD_PROF_NSLOTS];
     uint64_t prof_n[PIMD_PROF_NSLOTS];
@@ -126,7 +153,8 @@ struct ProfScope {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-// carve the workspace; with base == nullptr only the size is computed
+// Carve the workspace; with base == nullptr only the sizes are computed.  Layout: the global region, then B replica
+// regions of h->rstride bytes each with identical layout (kernels reach replica b through blockIdx * rstride).
 size_t carve(pimd_t h, unsigned char *base)
 {
     size_t off = 0;
@@ -135,44 +163,89 @@ size_t carve(pimd_t h, unsigned char *base)
         off = align_up(off + bytes, 256);
         return p;
     };
-    const size_t N = (size_t)h->N, D = (size_t)h->d, nd = h->ndof;
+    const size_t N = (size_t)h->N, D = (size_t)h->d, nd = h->ndof, B = (size_t)h->B;
+    // ---- global region
+    h->Fout = (double *)take(B * nd * 8);
+    h->gflags = (int *)take(4 * 4);
+    h->fallbacks = (unsigned long long *)take(8);
+    h->phase = (unsigned long long *)take(16 * 8);
+    h->dstep = (unsigned long long *)take(8);
+    const size_t packn = 2 * N * D + N;
+    h->pack = (double *)take(h->sharded ? packn * 8 : 8);
+    h->gathered = (double *)take(h->sharded ? (size_t)h->world * packn * 8 : 8);
+    h->eint_tot = (double *)take(h->sharded ? N * 8 : 8);
+    h->Sarr = (double *)take(N * 8);
+    h->Tarr = (double *)take(N * 8);
+    const size_t glob = off;
+    // ---- replica 0
     h->x = (double *)take(nd * 8);
     h->v = (double *)take(nd * 8);
     h->F = (double *)take(nd * 8);
-    h->Fout = (double *)take(nd * 8);
     h->nhc = (double *)take(h->thermostat == PIMD_THERMOSTAT_NHC ? nd * 8 * PIMD_NHC_LENGTH : 8);
     h->Fex1 = (double *)take(N * D * 8);
     h->FexP = (double *)take(N * D * 8);
-    for (int dir = 0; dir < 2; ++dir) {
-        h->ex.rho[dir] = (double *)take(N * D * 8);
-        h->ex.sig[dir] = (double *)take(N * D * 8);
-        h->ex.cc[dir] = (double *)take(N * 8);
-        h->ex.g[dir] = (double2 *)take((N + 1) * 16);
-        h->ex.gs[dir] = (double *)take((N + 1) * 8);
-        h->ex.pan_m[dir] = (double *)take(N * 8);
-        h->ex.pan_s[dir] = (double *)take(N * 8);
-        h->ex.panel_ready[dir] = (int *)take((size_t)h->NB * 4);
-        h->ex.acc[dir] = (double *)take(N * (D + 2) * 8);
+    h->Fexs1 = (double *)take(N * D * 8); // exterior forces of the reweighting xi: computed, never used
+    h->FexsP = (double *)take(N * D * 8);
+    for (int set = 0; set < 2; ++set) {
+        h->rp[set] = (RepParams *)take(sizeof(RepParams));
+        h->scal[set] = (Scalars *)take(sizeof(Scalars) * PIMD_MAX_SPECIES);
+        for (int sp = 0; sp < h->nspecies; ++sp) {
+            ExchCtx &c = h->ex[set][sp];
+            const size_t n = (size_t)c.N;
+            for (int dir = 0; dir < 2; ++dir) {
+                c.p.rho[dir] = (double *)take(n * D * 8);
+                c.p.sig[dir] = (double *)take(n * D * 8);
+                c.p.cc[dir] = (double *)take(n * 8);
+                c.p.g[dir] = (double2 *)take((n + 1) * 16);
+                c.p.gs[dir] = (double *)take((n + 1) * 8);
+                c.p.pan_m[dir] = (double *)take(n * 8);
+                c.p.pan_s[dir] = (double *)take(n * 8);
+                c.p.panel_ready[dir] = (int *)take((size_t)c.NB * 4);
+                c.p.acc[dir] = (double *)take(n * (D + 2) * 8);
+            }
+            c.p.cols_ready = (int *)take(2 * 4);
+            c.p.eint = (double *)take(n * 8);
+            c.p.cnext = (double *)take(n * 8);
+            c.p.cself = (double *)take(n * 8);
+            c.p.pnext = (double *)take(n * 8);
+            c.p.tpart = (double *)take((size_t)c.nprep * 2 * 8);
+            c.p.rfin = (double2 *)take(2 * 16);
+            c.p.rsgn = (double *)take(2 * 8);
+            c.p.status = (int *)take(2 * 4);
+            c.ecpart = (double *)take((size_t)c.nasm * 8);
+            c.scal = h->scal[set] ? h->scal[set] + sp : nullptr;
+            c.rp = h->rp[set];
+        }
     }
-    h->ex.cols_ready = (int *)take(2 * 4);
-    h->ex.eint = (double *)take(N * 8);
-    h->ex.cnext = (double *)take(N * 8);
-    h->ex.cself = (double *)take(N * 8);
-    h->ex.pnext = (double *)take(N * 8);
-    h->ex.tpart = (double *)take((size_t)h->nprep * 2 * 8);
-    h->ex.rfin = (double2 *)take(2 * 16);
-    h->ex.rsgn = (double *)take(2 * 8);
-    h->Sarr = (double *)take(N * 8);
-    h->Tarr = (double *)take(N * 8);
-    h->phase = (unsigned long long *)take(16 * 8);
-    h->dstep = (unsigned long long *)take(8);
-    h->status = (int *)take(4 * 4);
-    h->ex.status = h->status;
-    h->ecpart = (double *)take((size_t)h->nasm * 8);
-    h->scal = (Scalars *)take(sizeof(Scalars));
+    h->istatus = (int *)take(4);
     h->est = (EstAccum *)take(sizeof(EstAccum));
+    h->sums = (EstSums *)take(sizeof(EstSums));
     h->hist = (double *)take((size_t)MAX_BINS * 8);
-    return off;
+    h->hist_acc = (double *)take((size_t)MAX_BINS * 8);
+    h->gr = (double *)take((size_t)MAX_BINS * 8);
+    h->gr_acc = (double *)take((size_t)MAX_BINS * 8);
+    h->rstride = off - glob;
+    return glob + B * h->rstride;
+}
+
+int upload_params(pimd_t h, int set)
+{
+    std::vector<RepParams> rp((size_t)h->B);
+    const std::vector<double> &xi = set ? *h->xi2 : *h->xi;
+    h->any_neg[set] = false;
+    h->all_zero[set] = true;
+    for (int b = 0; b < h->B; ++b) {
+        rp[b].xi = xi[b];
+        rp[b].lambda = xi[b] != 0.0 ? std::log(std::fabs(xi[b])) : 0.0;
+        rp[b].sx = xi[b] < 0.0 ? -1.0 : 1.0;
+        rp[b].seed = (*h->seed)[b];
+        if (xi[b] < 0.0) h->any_neg[set] = true;
+        if (xi[b] != 0.0) h->all_zero[set] = false;
+    }
+    CU(cudaMemcpy2DAsync(h->rp[set], h->rstride, rp.data(), sizeof(RepParams), sizeof(RepParams), (size_t)h->B,
+                         cudaMemcpyHostToDevice, h->s0));
+    CU(cudaStreamSynchronize(h->s0)); // rp is a stack vector
+    return PIMD_OK;
 }
 
 int ensure_ws(pimd_t h)
@@ -192,7 +265,40 @@ int ensure_ws(pimd_t h)
     carve(h, h->ws);
     CU(cudaMemsetAsync(h->ws, 0, need, h->s0));
     h->carved = true;
-    return PIMD_OK;
+    int rc = upload_params(h, 0);
+    if (rc) return rc;
+    return upload_params(h, 1);
+}
+
+// species ranges -> exchange problems (both parameter sets); worker counts need the co-residency limit
+void setup_species(pimd_t h)
+{
+    int l0 = 0;
+    for (int sp = 0; sp < h->nspecies; ++sp) {
+        for (int set = 0; set < 2; ++set) {
+            ExchCtx &c = h->ex[set][sp];
+            c.N = h->counts[sp];
+            c.l0 = l0;
+            c.NB = (c.N + 31) / 32;
+            c.nprep = (c.N + PREP_TB - 1) / PREP_TB;
+            c.nasm = (c.N + ASM_TB - 1) / ASM_TB;
+            c.gauge_valid = false;
+            // Panel workers per direction.  A worker spins while it waits for columns and owns a whole SM, so only as many
+            // as the panel work needs are launched: a worker needs about 480 NB cycles for its last row blocks and gets
+            // nworkers x (one chain block, about 3000 cycles) for each, so NB/5 workers keep the panels ahead of the chain;
+            // when the pair kernel dominates the step (g != 0 and P N large) the SMs are worth more there and NB/8 is enough.
+            const int want = c.NB - h->look - 1;
+            int cap = h->coop_max_blocks / (2 * h->B) - 1; // all replicas' CTAs must be co-resident
+            int need = (h->g != 0.0 && (long long)h->P * h->N > 80000) ? (c.NB + 7) / 8 : (c.NB + 4) / 5;
+            if (const char *e = std::getenv("PIMD_WORKERS")) {
+                const int v = std::atoi(e);
+                if (v >= 1) need = v;
+            }
+            if (need > cap) need = cap;
+            c.nworkers = want <= 0 ? 0 : std::max(0, std::min(want, need));
+        }
+        l0 += h->counts[sp];
+    }
 }
 
 template <int D> int setup_chain_attr(pimd_t h)
@@ -211,23 +317,29 @@ template <int D> int setup_chain_attr(pimd_t h)
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     h->coop_max_blocks = nb * sms;
     h->sms = sms;
-    if (h->coop_max_blocks < 2) return fail(h, PIMD_ECUDA, "k_chain cannot be made co-resident (%d blocks)", h->coop_max_blocks);
+    if (h->coop_max_blocks < 2 * h->B)
+        return fail(h, PIMD_EINVAL, "a batch of %d replicas needs %d co-resident recursion CTAs, the device holds %d", h->B, 2 * h->B,
+                    h->coop_max_blocks);
     return PIMD_OK;
 }
 
 template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins, double rmax)
 {
-    const dim3 grid((h->N + BEAD_TB - 1) / BEAD_TB, h->P), block(BEAD_TB);
-    const double om2P = h->omega * h->omega / h->P, is2 = 1.0 / (h->s * h->s);
+    const dim3 grid((h->N + BEAD_TB - 1) / BEAD_TB, h->P, h->B), block(BEAD_TB);
+    const double om2P = h->omega * h->omega / h->Pg;
+    const size_t sl = h->slice, packn = 2 * sl + (size_t)h->N;
+    // bead shards: the ring neighbours' boundary slices come out of the gathered packs
+    const double *halo_lo = (h->sharded && h->j0 > 0) ? h->gathered + (size_t)(h->rank - 1) * packn + sl : nullptr;
+    const double *halo_hi = (h->sharded && h->j0 + h->P < h->Pg) ? h->gathered + (size_t)(h->rank + 1) * packn : nullptr;
     {
         // spring + trap forces (and the trap energy / histogram on estimator calls): F is written here
         ProfScope ps(h, PIMD_PROF_BEAD, st);
-        if (est) k_bead<D, false, true, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, 0.0, h->g, h->est, h->hist, nbins, rmax);
-        else k_bead<D, false, false, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, is2, 0.0, h->g, h->est, h->hist, nbins, rmax);
+        if (est) k_bead<D, true, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, h->est, h->hist, nbins, rmax, halo_lo, halo_hi, h->rstride);
+        else k_bead<D, false, BEAD_TB><<<grid, block, 0, st>>>(h->x, h->F, h->N, h->P, h->ks, om2P, h->est, h->hist, nbins, rmax, halo_lo, halo_hi, h->rstride);
     }
     CU(cudaGetLastError());
     if (h->g != 0.0) {
-        // pair forces, added to F (Newton's third law, one Gaussian per unordered pair)
+        // pair forces, added to F (Newton's third law, one potential evaluation per unordered pair)
         const int NT = (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
         // offsets per task: small tasks balance small grids (measured: 1 is best up to N = 2500, 4 at N = 10000; tuning knob PIMD_PAIR_CH)
@@ -236,90 +348,148 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         const int nchunk = hmax > 0 ? std::max(1, (hmax + target / 2) / target) : 0;
         const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
         const long long tasks = (long long)NT * (nchunk + 1);
-        const dim3 pgrid((unsigned)((tasks + PAIR_WARPS - 1) / PAIR_WARPS), h->P);
-        const double coef = 2.0 * h->g / (h->s * h->P);
+        const dim3 pgrid((unsigned)((tasks + PAIR_WARPS - 1) / PAIR_WARPS), h->P, h->B);
+        // constant factors of the potential (pair_weight): force coefficient and energy prefactor
+        const double coef = h->pot == 0 ? 2.0 * h->g / (h->s * h->Pg) : h->g / (h->s * h->s * h->Pg);
+        const double gE = h->pot == 0 ? h->g : h->g / h->s;
         ProfScope ps(h, PIMD_PROF_PAIR, st);
-        if (est) k_pair<D, true><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, h->g, h->est);
-        else k_pair<D, false><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, h->g, h->est);
+#define LP(E, POT) k_pair<D, E, POT><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, gE, h->est, h->rstride)
+        if (h->pot == 0) { if (est) LP(true, 0); else LP(false, 0); }
+        else { if (est) LP(true, 1); else LP(false, 1); }
+#undef LP
     }
     CU(cudaGetLastError());
+    if (est && h->nbins_gr > 0) {
+        const dim3 ggrid((h->N + GR_TB - 1) / GR_TB, h->P, h->B);
+        ProfScope ps(h, PIMD_PROF_GR, st);
+        k_gr<D><<<ggrid, GR_TB, 0, st>>>(h->x, h->N, h->gr, h->nbins_gr, h->rmax_gr, h->rstride);
+        CU(cudaGetLastError());
+    }
     return PIMD_OK;
 }
 
-template <int D> int launch_prep(pimd_t h, cudaStream_t st)
+template <int D> int launch_prep(pimd_t h, ExchCtx &c, cudaStream_t st)
 {
+    const size_t sl = h->slice, packn = 2 * sl + (size_t)h->N, lo = (size_t)c.l0 * D;
+    const double *x = h->x + lo, *x1 = h->x + lo, *xP = h->x + (size_t)(h->P - 1) * sl + lo, *ein = nullptr;
+    if (h->sharded) { // bead 1 = first slice of rank 0, bead P = last slice of the last rank, E_int summed over the ranks
+        x = nullptr;
+        x1 = h->gathered + lo;
+        xP = h->gathered + (size_t)(h->world - 1) * packn + sl + lo;
+        ein = h->eint_tot + c.l0;
+    }
     {
         ProfScope ps(h, PIMD_PROF_PREP, st);
-        k_prep<D, PREP_TB><<<h->nprep, PREP_TB * PREP_SPLIT, 0, st>>>(h->x, h->N, h->P, h->NB, h->ks, h->kk, h->lambda, h->ex);
+        k_prep<D, PREP_TB><<<dim3(c.nprep, h->B), PREP_TB * PREP_SPLIT, 0, st>>>(x, x1, xP, ein, sl, c.N, h->P, c.NB, h->ks, h->kk, c.p, c.rp,
+                                                                               h->gflags, h->rstride);
     }
     CU(cudaGetLastError());
     return PIMD_OK;
 }
 
-template <int D> int launch_exchange(pimd_t h, cudaStream_t st, bool scalars)
+template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t st, bool scalars)
 {
-    const bool sgn = h->xi < 0.0;
-    if (h->xi == 0.0) {
+    const bool sgn = h->any_neg[set];
+    const size_t lo = (size_t)c.l0 * D;
+    double *const Fex1 = set ? h->Fexs1 : h->Fex1, *const FexP = set ? h->FexsP : h->FexP;
+    if (h->all_zero[set]) {
         {
             ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
-            k_exch_xi0<D, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->ex, h->Fex1, h->FexP, h->ecpart);
+            k_exch_xi0<D, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, Fex1 + lo, FexP + lo, c.ecpart, h->rstride);
         }
         CU(cudaGetLastError());
     } else {
         ChainArgs a;
-        a.N = h->N; a.NB = h->NB; a.look = h->look; a.nworkers = h->nworkers;
-        a.kk = h->kk; a.sx = sgn ? -1.0 : 1.0; a.p = h->ex;
+        a.N = c.N; a.NB = c.NB; a.look = h->look; a.nworkers = c.nworkers;
+        a.kk = h->kk; a.p = c.p; a.rp = c.rp; a.rs = h->rstride;
         a.phase = h->profiling ? h->phase : nullptr;
         a.look_fb = h->look;
-        const int look_spec = h->look_spec;
+        a.gauge_misfit = h->gflags;
+        a.fallbacks = h->fallbacks;
         void *args[] = {&a};
-        const dim3 grid(1 + h->nworkers, 2), block(CH_THREADS);
-        const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
-        if (h->gauge_valid && h->use_spec) {
+        const dim3 grid(1 + c.nworkers, 2, h->B), block(CH_THREADS);
+        if (c.gauge_valid && h->use_spec) {
             // the previous evaluation's gauge is at hand: linear pass only; the kernel redoes the recursion with a
             // fresh max-plus gauge itself (after a grid barrier) if the gauge turned out not to fit
             const void *fs = sgn ? (const void *)k_chain_spec<D, true> : (const void *)k_chain_spec<D, false>;
-            a.look = look_spec; // the workers need one more block of head start when the chain runs this fast
+            a.look = h->look_spec; // the workers need one more block of head start when the chain runs this fast
             ProfScope ps(h, PIMD_PROF_CHAIN, st);
             CU(cudaLaunchCooperativeKernel(fs, grid, block, args, h->spec_smem, st));
         } else {
+            const void *fn = sgn ? (const void *)k_chain<D, true> : (const void *)k_chain<D, false>;
             ProfScope ps(h, PIMD_PROF_CHAIN, st);
             CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
         }
-        h->gauge_valid = true;
-        const int NT = (h->N + FP_TB - 1) / FP_TB;
+        c.gauge_valid = true;
+        const int NT = (c.N + FP_TB - 1) / FP_TB;
         // NT (NT+1) tiles at or below the diagonal (both directions); with fewer than 8 per SM one thread per row leaves
-        // the kernel latency bound, so four threads share a row (measured at cfg3: 0.023 -> 0.017 ms with the columns cut
-        // into four CTAs, less again with the partial sums combined inside one CTA)
-        const long long tiles = (long long)NT * (NT + 1);
+        // the kernel latency bound, so four threads share a row (measured at cfg3: 0.023 -> 0.017 ms)
+        const long long tiles = (long long)NT * (NT + 1) * h->B;
         const bool wide = tiles < 8LL * h->sms;
-        const dim3 fgrid(wide ? (h->N + FP_TB / 4 - 1) / (FP_TB / 4) : NT, NT, 2);
+        const dim3 fgrid(wide ? (c.N + FP_TB / 4 - 1) / (FP_TB / 4) : NT, NT, 2 * h->B);
         {
             ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
             if (wide) {
-                if (sgn) k_forcepass<D, true, 4><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
-                else k_forcepass<D, false, 4><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+                if (sgn) k_forcepass<D, true, 4><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
+                else k_forcepass<D, false, 4><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
             } else {
-                if (sgn) k_forcepass<D, true, 1><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
-                else k_forcepass<D, false, 1><<<fgrid, FP_TB, 0, st>>>(h->N, h->kk, h->ex);
+                if (sgn) k_forcepass<D, true, 1><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
+                else k_forcepass<D, false, 1><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
             }
         }
         CU(cudaGetLastError());
         {
             ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
-            if (sgn) k_assemble<D, true, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
-            else k_assemble<D, false, ASM_TB><<<h->nasm, ASM_TB, 0, st>>>(h->N, h->ks, h->xi, h->ex, h->Fex1, h->FexP, h->ecpart);
+            if (sgn) k_assemble<D, true, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->rstride);
+            else k_assemble<D, false, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->rstride);
         }
         CU(cudaGetLastError());
     }
     if (scalars) {
         {
             ProfScope ps(h, PIMD_PROF_FINALIZE, st);
-            k_finalize<256><<<1, 256, 0, st>>>(h->N, h->nprep, h->nasm, h->beta, h->lambda, h->xi, std::lgamma((double)h->N + 1.0),
-                                               h->ex, h->ecpart, h->scal);
+            k_finalize<256><<<h->B, 256, 0, st>>>(c.N, c.nprep, c.nasm, h->beta, c.rp, std::lgamma((double)c.N + 1.0), c.p, c.ecpart, c.scal,
+                                                  h->rstride);
         }
         CU(cudaGetLastError());
     }
+    return PIMD_OK;
+}
+
+int prep_d(pimd_t h, ExchCtx &c, cudaStream_t st)
+{
+    switch (h->d) {
+    case 1: return launch_prep<1>(h, c, st);
+    case 2: return launch_prep<2>(h, c, st);
+    default: return launch_prep<3>(h, c, st);
+    }
+}
+int exchange_d(pimd_t h, ExchCtx &c, int set, cudaStream_t st, bool scalars)
+{
+    switch (h->d) {
+    case 1: return launch_exchange<1>(h, c, set, st, scalars);
+    case 2: return launch_exchange<2>(h, c, set, st, scalars);
+    default: return launch_exchange<3>(h, c, set, st, scalars);
+    }
+}
+int bead_d(pimd_t h, cudaStream_t st, bool est, int nbins, double rmax)
+{
+    switch (h->d) {
+    case 1: return launch_bead<1>(h, st, est, nbins, rmax);
+    case 2: return launch_bead<2>(h, st, est, nbins, rmax);
+    default: return launch_bead<3>(h, st, est, nbins, rmax);
+    }
+}
+
+// the estimators of the evaluation just made (k_estimate), optionally added to the running sums
+int launch_estimate(pimd_t h, int nbins, bool accumulate)
+{
+    const double kin = (double)h->Pg * h->d * h->N / (2.0 * h->beta);
+    const double ecw = (!h->sharded || h->rank == 0) ? 1.0 : 0.0;
+    ProfScope ps(h, PIMD_PROF_FINALIZE, h->s0);
+    k_estimate<<<h->B, 256, 0, h->s0>>>(h->nspecies, h->scal[0], h->est, h->sums, h->hist, h->hist_acc, nbins, h->gr, h->gr_acc,
+                                        h->nbins_gr, kin, ecw, 1.0 / h->Pg, accumulate ? 1 : 0, h->rstride);
+    CU(cudaGetLastError());
     return PIMD_OK;
 }
 
@@ -330,32 +500,26 @@ int eval_forces(pimd_t h, bool scalars, bool est, int nbins, double rmax)
 {
     int rc = ensure_ws(h);
     if (rc) return rc;
+    if (h->sharded && !h->shard_imported) return fail(h, PIMD_EINVAL, "bead shard: no boundary data imported for the current positions");
     if (est) {
-        CU(cudaMemsetAsync(h->est, 0, sizeof(EstAccum), h->s0));
-        if (nbins > 0) CU(cudaMemsetAsync(h->hist, 0, (size_t)nbins * 8, h->s0));
+        CU(cudaMemset2DAsync(h->est, h->rstride, 0, sizeof(EstAccum), (size_t)h->B, h->s0));
+        if (nbins > 0) CU(cudaMemset2DAsync(h->hist, h->rstride, 0, (size_t)nbins * 8, (size_t)h->B, h->s0));
+        if (h->nbins_gr > 0) CU(cudaMemset2DAsync(h->gr, h->rstride, 0, (size_t)h->nbins_gr * 8, (size_t)h->B, h->s0));
     }
     cudaStream_t sb = h->concurrent ? h->s1 : h->s0;
-    switch (h->d) {
-    case 1: rc = launch_prep<1>(h, h->s0); break;
-    case 2: rc = launch_prep<2>(h, h->s0); break;
-    default: rc = launch_prep<3>(h, h->s0); break;
+    for (int sp = 0; sp < h->nspecies; ++sp) {
+        rc = prep_d(h, h->ex[0][sp], h->s0);
+        if (rc) return rc;
     }
-    if (rc) return rc;
     if (h->concurrent) {
         CU(cudaEventRecord(h->ev_fork, h->s0));
         CU(cudaStreamWaitEvent(h->s1, h->ev_fork, 0));
     }
-    switch (h->d) {
-    case 1: rc = launch_exchange<1>(h, h->s0, scalars); break;
-    case 2: rc = launch_exchange<2>(h, h->s0, scalars); break;
-    default: rc = launch_exchange<3>(h, h->s0, scalars); break;
+    for (int sp = 0; sp < h->nspecies; ++sp) {
+        rc = exchange_d(h, h->ex[0][sp], 0, h->s0, scalars || est);
+        if (rc) return rc;
     }
-    if (rc) return rc;
-    switch (h->d) {
-    case 1: rc = launch_bead<1>(h, sb, est, nbins, rmax); break;
-    case 2: rc = launch_bead<2>(h, sb, est, nbins, rmax); break;
-    default: rc = launch_bead<3>(h, sb, est, nbins, rmax); break;
-    }
+    rc = bead_d(h, sb, est, nbins, rmax);
     if (rc) return rc;
     if (h->concurrent) {
         CU(cudaEventRecord(h->ev_join, h->s1));
@@ -363,6 +527,7 @@ int eval_forces(pimd_t h, bool scalars, bool est, int nbins, double rmax)
     }
     h->forces_valid = true;
     h->tables_valid = true;
+    h->scalars_valid = scalars || est;
     return PIMD_OK;
 }
 
@@ -371,11 +536,14 @@ int launch_integrate(pimd_t h, bool do_close, bool do_open, uint64_t step_close,
     const unsigned long long *dstep = device_counter ? h->dstep : nullptr;
     const double c1 = std::exp(-h->gamma * h->dt * 0.5);
     const double c2 = std::sqrt((1.0 - c1 * c1) / h->beta);
-    const double Q = h->beta / (double)h->P;
-    const unsigned grid = (unsigned)((h->ndof + 255) / 256);
+    const double Q = h->beta / (double)h->Pg;
+    const dim3 grid((unsigned)((h->ndof + 255) / 256), h->B);
+    const int own_first = (!h->sharded || h->j0 == 0) ? 1 : 0, own_last = (!h->sharded || h->j0 + h->P == h->Pg) ? 1 : 0;
+    const size_t dof0 = (size_t)h->j0 * h->slice;
 #define LI(T) \
     k_integrate<T><<<grid, 256, 0, h->s0>>>(h->x, h->v, h->F, h->Fex1, h->FexP, h->nhc, h->ndof, h->slice, h->P, h->dt, c1, c2, \
-                                            h->beta, Q, h->seed, step_close, step_open, do_close ? 1 : 0, do_open ? 1 : 0, h->status, dstep)
+                                            h->beta, Q, h->rp[0], step_close, step_open, do_close ? 1 : 0, do_open ? 1 : 0,     \
+                                            h->istatus, dstep, own_first, own_last, dof0, h->rstride)
     {
         ProfScope ps(h, PIMD_PROF_INTEGRATE, h->s0);
         if (h->thermostat == PIMD_THERMOSTAT_LANGEVIN) LI(1);
@@ -384,14 +552,20 @@ int launch_integrate(pimd_t h, bool do_close, bool do_open, uint64_t step_close,
     }
 #undef LI
     CU(cudaGetLastError());
+    if (do_open) h->shard_imported = false; // positions moved: the boundary data is stale
     return PIMD_OK;
 }
 
+// status words of the last evaluation (every replica, every species) and of the integrator; synchronises
 int read_status(pimd_t h)
 {
-    CU(cudaMemcpyAsync(h->h_status, h->status, 4 * sizeof(int), cudaMemcpyDeviceToHost, h->s0));
+    const int B = h->B, S = h->nspecies;
+    CU(cudaMemcpy2DAsync(h->h_status, 4, h->istatus, h->rstride, 4, (size_t)B, cudaMemcpyDeviceToHost, h->s0));
+    for (int sp = 0; sp < S; ++sp)
+        CU(cudaMemcpy2DAsync(h->h_status + (size_t)B * (1 + sp), 4, h->ex[0][sp].p.status, h->rstride, 4, (size_t)B, cudaMemcpyDeviceToHost, h->s0));
     CU(cudaStreamSynchronize(h->s0));
-    const int st = h->h_status[0] | h->h_status[1];
+    int st = 0;
+    for (int k = 0; k < B * (1 + S); ++k) st |= h->h_status[k];
     if (st & ST_NONFINITE) return fail(h, PIMD_ENUMERIC, "non-finite state or potential");
     if (st & ST_NODE) return fail(h, PIMD_ENUMERIC, "e^{-beta V} summed to zero (node of the xi<0 weight)");
     return PIMD_OK;
@@ -404,25 +578,28 @@ bool finite_all(std::initializer_list<double> v)
     return true;
 }
 
-} // namespace
-
-// Capture "force evaluation ; close step s + open step s+1 ; counter += 1" once, on an internal stream (the caller's
-// stream may be the legacy default stream, which cannot be captured).  Any failure (e.g. a driver that cannot put a
-// cooperative launch into a graph) switches the feature off for this handle; nothing else depends on it.
-static int ensure_graph(pimd_t h)
+void drop_graphs(pimd_t h)
 {
-    if (h->gexec && h->graph_conc == h->concurrent) return PIMD_OK;
-    if (h->graph_failed) return PIMD_ECUDA;
     if (h->gexec) { cudaGraphExecDestroy(h->gexec); h->gexec = nullptr; }
+    if (h->gexec_est) { cudaGraphExecDestroy(h->gexec_est); h->gexec_est = nullptr; }
+}
+
+// Capture "force evaluation ; [estimators] ; close step s + open step s+1 ; counter += 1" once, on an internal stream
+// (the caller's stream may be the legacy default stream, which cannot be captured).  Any failure (e.g. a driver that
+// cannot put a cooperative launch into a graph) switches the feature off for this handle; nothing else depends on it.
+int capture_step(pimd_t h, bool est, int nbins, double rmax, cudaGraphExec_t *out, uint64_t *nlaunch)
+{
+    if (h->graph_failed) return PIMD_ECUDA;
     cudaStream_t user = h->s0;
     const uint64_t l0 = h->launches;
-    const bool fv = h->forces_valid, tv = h->tables_valid;
+    const bool fv = h->forces_valid, tv = h->tables_valid, sv = h->scalars_valid;
     cudaGraph_t graph = nullptr;
     int rc = PIMD_OK;
     if (cudaStreamBeginCapture(h->sg, cudaStreamCaptureModeRelaxed) != cudaSuccess) rc = PIMD_ECUDA;
     if (rc == PIMD_OK) {
         h->s0 = h->sg;
-        rc = eval_forces(h, false, false, 0, 0.0);
+        rc = eval_forces(h, false, est, nbins, rmax);
+        if (rc == PIMD_OK && est) rc = launch_estimate(h, nbins, true);
         if (rc == PIMD_OK) rc = launch_integrate(h, true, true, 0, 0, true);
         if (rc == PIMD_OK) {
             k_step_counter<<<1, 32, 0, h->sg>>>(h->dstep, 0ull, 1);
@@ -432,63 +609,140 @@ static int ensure_graph(pimd_t h)
         h->s0 = user;
         if (cudaStreamEndCapture(h->sg, &graph) != cudaSuccess || !graph) rc = PIMD_ECUDA;
     }
-    if (rc == PIMD_OK && cudaGraphInstantiate(&h->gexec, graph, 0) != cudaSuccess) rc = PIMD_ECUDA;
+    if (rc == PIMD_OK && cudaGraphInstantiate(out, graph, 0) != cudaSuccess) rc = PIMD_ECUDA;
     if (graph) cudaGraphDestroy(graph);
-    h->graph_launches = h->launches - l0;
+    *nlaunch = h->launches - l0;
     h->launches = l0;
     h->forces_valid = fv;
     h->tables_valid = tv;
+    h->scalars_valid = sv;
     if (rc != PIMD_OK) {
         cudaGetLastError();
-        h->gexec = nullptr;
+        *out = nullptr;
         h->graph_failed = true;
         return PIMD_ECUDA;
     }
-    h->graph_conc = h->concurrent;
     return PIMD_OK;
 }
 
+int ensure_graphs(pimd_t h, bool need_est, int nbins, double rmax)
+{
+    if (h->graph_conc != h->concurrent) drop_graphs(h);
+    if (h->gexec_est && (h->graph_nbins != nbins || h->graph_rmax != rmax || h->graph_nbins_gr != h->nbins_gr || h->graph_rmax_gr != h->rmax_gr)) {
+        cudaGraphExecDestroy(h->gexec_est);
+        h->gexec_est = nullptr;
+    }
+    h->graph_conc = h->concurrent;
+    if (!h->gexec) {
+        int rc = capture_step(h, false, 0, 0.0, &h->gexec, &h->graph_launches);
+        if (rc) return rc;
+    }
+    if (need_est && !h->gexec_est) {
+        int rc = capture_step(h, true, nbins, rmax, &h->gexec_est, &h->graph_est_launches);
+        if (rc) return rc;
+        h->graph_nbins = nbins; h->graph_rmax = rmax; h->graph_nbins_gr = h->nbins_gr; h->graph_rmax_gr = h->rmax_gr;
+    }
+    return PIMD_OK;
+}
+
+// nsteps MD steps; with est_every > 0 the force evaluation of every step whose (absolute) number is a multiple of
+// est_every runs in estimator mode and its estimators are added to the running sums
+int run_steps(pimd_t h, int nsteps, int est_every, int nbins, double rmax)
+{
+    if (nsteps == 0) return PIMD_OK;
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    if (h->sharded) return fail(h, PIMD_EINVAL, "bead shard: advance with pimd_shard_begin_step / pimd_shard_end_step");
+    if (!h->forces_valid) {
+        rc = eval_forces(h, false, false, 0, 0.0);
+        if (rc) return rc;
+    }
+    auto is_est = [&](uint64_t step_done) { return est_every > 0 && step_done % (uint64_t)est_every == 0; };
+    // open step s ; forces ; [close s + open s+1] ; forces ; ... ; close last
+    rc = launch_integrate(h, false, true, 0, h->step);
+    if (rc) return rc;
+    int it = 0;
+    bool gauge_ok = true;
+    for (int sp = 0; sp < h->nspecies; ++sp) gauge_ok = gauge_ok && (h->ex[0][sp].gauge_valid || h->all_zero[0]);
+    if (h->use_graph && !h->profiling && gauge_ok && nsteps >= 3 && ensure_graphs(h, est_every > 0, nbins, rmax) == PIMD_OK) {
+        // all but the last step replay the captured graphs; the step counter of the noise lives on the device meanwhile
+        k_step_counter<<<1, 32, 0, h->s0>>>(h->dstep, (unsigned long long)h->step, 0);
+        CU(cudaGetLastError());
+        CU(cudaEventRecord(h->ev_gin, h->s0));
+        CU(cudaStreamWaitEvent(h->sg, h->ev_gin, 0));
+        for (; it < nsteps - 1; ++it) {
+            const bool e = is_est(h->step + 1);
+            CU(cudaGraphLaunch(e ? h->gexec_est : h->gexec, h->sg));
+            h->launches += e ? h->graph_est_launches : h->graph_launches;
+            h->step++;
+        }
+        CU(cudaEventRecord(h->ev_gout, h->sg));
+        CU(cudaStreamWaitEvent(h->s0, h->ev_gout, 0));
+    }
+    for (; it < nsteps; ++it) {
+        const bool e = is_est(h->step + 1);
+        rc = eval_forces(h, false, e, nbins, rmax);
+        if (rc == PIMD_OK && e) rc = launch_estimate(h, nbins, true);
+        if (rc) return rc;
+        const bool last = it == nsteps - 1;
+        rc = launch_integrate(h, true, !last, h->step, h->step + 1);
+        if (rc) return rc;
+        h->step++;
+    }
+    return PIMD_OK; // the flags eval_forces set for the last step hold: F, the tables belong to the final positions
+}
+
+} // namespace
+
 template <int D> static int cycle_energies_impl(pimd_t h, double *e_dev)
 {
-    int rc = launch_prep<D>(h, h->s0); // E_int, C(l,l+1), bead-1 / bead-P slices of the current positions
+    ExchCtx &c = h->ex[0][0];
+    int rc = launch_prep<D>(h, c, h->s0); // E_int, C(l,l+1), bead-1 / bead-P slices of the current positions
     if (rc) return rc;
-    k_prefix_st<<<1, 1024, 0, h->s0>>>(h->N, h->beta, h->ex.eint, h->ex.cnext, h->Sarr, h->Tarr);
+    k_prefix_st<<<1, 1024, 0, h->s0>>>(c.N, h->beta, c.p.eint, c.p.cnext, h->Sarr, h->Tarr);
     CU(cudaGetLastError());
-    const dim3 grid((h->N + 1023) / 1024, h->N);
+    const dim3 grid((c.N + 1023) / 1024, c.N);
     {
         ProfScope ps(h, PIMD_PROF_EMAT, h->s0);
-        k_emat<D><<<grid, 256, 0, h->s0>>>(h->N, h->ks, h->ex.rho[0], h->ex.sig[0], h->Sarr, h->Tarr, e_dev);
+        k_emat<D><<<grid, 256, 0, h->s0>>>(c.N, h->ks, c.p.rho[0], c.p.sig[0], h->Sarr, h->Tarr, e_dev);
     }
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(h->s0));
+    h->tables_valid = false; // k_prep cleared the accumulators of the last evaluation
+    h->scalars_valid = false;
     return PIMD_OK;
 }
 
 template <int D> static int prmat_impl(pimd_t h, double *pr_dev)
 {
-    const dim3 grid((h->N + 1023) / 1024, h->N), gridp((h->N + 256 * PRMAT_COLS - 1) / (256 * PRMAT_COLS), (h->N + PRMAT_ROWS - 1) / PRMAT_ROWS);
+    ExchCtx &c = h->ex[0][0];
+    const int N = c.N;
+    const dim3 grid((N + 1023) / 1024, N), gridp((N + 256 * PRMAT_COLS - 1) / (256 * PRMAT_COLS), (N + PRMAT_ROWS - 1) / PRMAT_ROWS);
     ProfScope ps(h, PIMD_PROF_PRMAT, h->s0);
-    if (h->xi == 0.0) k_identity<<<grid, 256, 0, h->s0>>>(h->N, pr_dev);
-    else if (h->xi < 0.0) k_prmat<D, true><<<gridp, 256, 0, h->s0>>>(h->N, h->kk, h->ex, pr_dev);
-    else k_prmat<D, false><<<gridp, 256, 0, h->s0>>>(h->N, h->kk, h->ex, pr_dev);
+    if (h->all_zero[0]) k_identity<<<grid, 256, 0, h->s0>>>(N, pr_dev);
+    else if (h->any_neg[0]) k_prmat<D, true><<<gridp, 256, 0, h->s0>>>(N, h->kk, c.p, pr_dev);
+    else k_prmat<D, false><<<gridp, 256, 0, h->s0>>>(N, h->kk, c.p, pr_dev);
     return PIMD_OK;
 }
 
-extern "C" {
-
-const char *pimd_version(void) { return "pimd-b200 0.1 (sm_100a)"; }
-
-const char *pimd_last_error(pimd_t h) { return h ? h->err : g_create_error; }
-
-int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, double g, double s, double xi, double dt,
-                int thermostat, uint64_t seed)
+static int create_impl(pimd_t *out, int B, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
+                       const double *xi, double dt, int thermostat, const uint64_t *seed)
 {
     pimd_t h = nullptr;
     if (!out) return fail(nullptr, PIMD_EINVAL, "out is NULL");
     *out = nullptr;
     if (N < 1 || P < 2 || d < 1 || d > 3) return fail(nullptr, PIMD_EINVAL, "need N >= 1, P >= 2, d in {1,2,3} (got N=%d P=%d d=%d)", N, P, d);
-    if (!finite_all({beta, omega, g, s, xi, dt}) || !(beta > 0) || !(s > 0) || !(dt > 0) || omega < 0)
+    if (B < 1 || !xi || !seed) return fail(nullptr, PIMD_EINVAL, "need B >= 1 replicas with xi[B] and seed[B]");
+    if (world < 1 || rank < 0 || rank >= world || world > P) return fail(nullptr, PIMD_EINVAL, "need 0 <= rank < world <= P (got rank=%d world=%d P=%d)", rank, world, P);
+    if (world > 1 && B != 1) return fail(nullptr, PIMD_EINVAL, "bead shards hold one replica");
+    if (!finite_all({beta, omega, g, s, dt}) || !(beta > 0) || !(s > 0) || !(dt > 0) || omega < 0)
         return fail(nullptr, PIMD_EINVAL, "need finite arguments with beta > 0, s > 0, dt > 0, omega >= 0");
+    bool any0 = false, anynz = false;
+    for (int b = 0; b < B; ++b) {
+        if (!std::isfinite(xi[b])) return fail(nullptr, PIMD_EINVAL, "xi must be finite");
+        if (xi[b] == 0.0) any0 = true; else anynz = true;
+    }
+    if (any0 && anynz) return fail(nullptr, PIMD_EINVAL, "a batch is either all xi = 0 (distinguishable particles) or all xi != 0");
     if (thermostat < 0 || thermostat > 2) return fail(nullptr, PIMD_EINVAL, "thermostat must be 0, 1 or 2");
     if ((double)N * P * d > 2.0e9) return fail(nullptr, PIMD_EINVAL, "N*P*d too large");
     int ndev = 0;
@@ -498,26 +752,30 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     h = new (std::nothrow) pimd_s();
     if (!h) return fail(nullptr, PIMD_ENOMEM, "host allocation failed");
     std::memset(h, 0, sizeof(*h));
-    h->N = N; h->P = P; h->d = d;
-    h->beta = beta; h->omega = omega; h->g = g; h->s = s; h->xi = xi; h->dt = dt; h->gamma = 1.0;
-    h->thermostat = thermostat; h->seed = seed; h->step = 0;
+    h->B = B; h->N = N; h->d = d;
+    h->Pg = P; h->rank = rank; h->world = world; h->sharded = world > 1;
+    // bead shards: rank r holds the slices [floor(P r / world), floor(P (r+1) / world))
+    h->j0 = (int)((long long)P * rank / world);
+    h->P = (int)((long long)P * (rank + 1) / world) - h->j0;
+    h->beta = beta; h->omega = omega; h->g = g; h->s = s; h->dt = dt; h->gamma = 1.0;
+    h->thermostat = thermostat; h->step = 0; h->pot = PIMD_PAIR_GAUSSIAN;
+    h->xi = new std::vector<double>(xi, xi + B);
+    h->xi2 = new std::vector<double>(xi, xi + B);
+    h->seed = new std::vector<uint64_t>(seed, seed + B);
     h->ks = (double)P / (beta * beta);          // m omega_P^2, omega_P = sqrt(P)/(beta hbar)
     h->kk = (double)P / (2.0 * beta);           // beta k_s / 2
-    h->lambda = (xi != 0.0) ? std::log(std::fabs(xi)) : 0.0;
     h->slice = (size_t)N * d;
-    h->ndof = h->slice * P;
-    h->NB = (N + 31) / 32;
-    h->nprep = (N + PREP_TB - 1) / PREP_TB;
-    h->nasm = (N + ASM_TB - 1) / ASM_TB;
+    h->ndof = h->slice * h->P;
+    h->nspecies = 1;
+    h->counts[0] = N;
     h->look = 2;
     h->look_spec = 3;
-    if (const char *e = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
-        const int v = std::atoi(e);
+    if (const char *e2 = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
+        const int v = std::atoi(e2);
         if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;
     }
     h->concurrent = true;
     h->use_graph = !(std::getenv("PIMD_GRAPH") && std::atoi(std::getenv("PIMD_GRAPH")) == 0);
-    h->gauge_valid = false;
     h->use_spec = !(std::getenv("PIMD_NOSPEC") && std::atoi(std::getenv("PIMD_NOSPEC")) != 0);
     h->prof_ev = new std::vector<cudaEvent_t>();
     h->prof_slot = new std::vector<int>();
@@ -529,35 +787,45 @@ int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, dou
     default: rc = setup_chain_attr<3>(h); break;
     }
     if (rc) return bail(rc);
-    {
-        // Panel workers per direction.  A worker spins while it waits for columns and owns a whole SM,
-        // so only as many as the panel work needs are launched.
-        const int want = h->NB - h->look - 1;
-        int cap = h->coop_max_blocks / 2 - 1;
-        // A worker needs about 480 NB cycles for its last row blocks and gets nworkers x (one chain block, about 3000
-        // cycles) for each, so NB/5 workers keep the panels ahead of the chain; when the pair kernel dominates the step
-        // (g != 0 and P N large: its work over the chain's grows like P N) the SMs are worth more there and NB/8 is enough.
-        int need = (h->g != 0.0 && (long long)h->P * h->N > 80000) ? (h->NB + 7) / 8 : (h->NB + 4) / 5;
-        if (const char *e = std::getenv("PIMD_WORKERS")) {
-            const int v = std::atoi(e);
-            if (v >= 1) need = v;
-        }
-        if (need > cap) need = cap;
-        h->nworkers = want <= 0 ? 0 : (want < need ? want : need);
-        if (want > 0 && h->nworkers < 1) return bail(fail(h, PIMD_ECUDA, "not enough co-resident CTAs for the recursion"));
-    }
+    setup_species(h);
+    const size_t nst = (size_t)B * (1 + 2 * PIMD_MAX_SPECIES);
     if (cudaStreamCreateWithFlags(&h->s1, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&h->sg, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_gin, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_gout, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess ||
-        cudaMallocHost((void **)&h->h_scal, sizeof(Scalars)) != cudaSuccess ||
-        cudaMallocHost((void **)&h->h_est, sizeof(EstAccum)) != cudaSuccess ||
-        cudaMallocHost((void **)&h->h_status, 4 * sizeof(int)) != cudaSuccess)
+        cudaMallocHost((void **)&h->h_scal, sizeof(Scalars) * (size_t)B * PIMD_MAX_SPECIES) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_sums, sizeof(EstSums) * (size_t)B) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_diag, 16) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_status, nst * sizeof(int)) != cudaSuccess)
         return bail(fail(h, PIMD_ECUDA, "stream/event/pinned allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
     *out = h;
     return PIMD_OK;
+}
+
+extern "C" {
+
+const char *pimd_version(void) { return "pimd-b200 0.2 (sm_100a)"; }
+
+const char *pimd_last_error(pimd_t h) { return h ? h->err : g_create_error; }
+
+int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, double g, double s, double xi, double dt,
+                int thermostat, uint64_t seed)
+{
+    return create_impl(out, 1, 0, 1, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
+}
+
+int pimd_create_batch(pimd_t *out, int B, int N, int P, int d, double beta, double omega, double g, double s, const double *xi,
+                      double dt, int thermostat, const uint64_t *seed)
+{
+    return create_impl(out, B, 0, 1, N, P, d, beta, omega, g, s, xi, dt, thermostat, seed);
+}
+
+int pimd_create_sharded(pimd_t *out, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
+                        double xi, double dt, int thermostat, uint64_t seed)
+{
+    return create_impl(out, 1, rank, world, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
 }
 
 int pimd_destroy(pimd_t h)
@@ -565,7 +833,7 @@ int pimd_destroy(pimd_t h)
     if (!h) return PIMD_OK;
     if (h->s0 || h->s1) cudaDeviceSynchronize();
     if (h->own_ws && h->ws) cudaFree(h->ws);
-    if (h->gexec) cudaGraphExecDestroy(h->gexec);
+    drop_graphs(h);
     if (h->sg) cudaStreamDestroy(h->sg);
     if (h->ev_gin) cudaEventDestroy(h->ev_gin);
     if (h->ev_gout) cudaEventDestroy(h->ev_gout);
@@ -573,13 +841,17 @@ int pimd_destroy(pimd_t h)
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
     if (h->h_scal) cudaFreeHost(h->h_scal);
-    if (h->h_est) cudaFreeHost(h->h_est);
+    if (h->h_sums) cudaFreeHost(h->h_sums);
+    if (h->h_diag) cudaFreeHost(h->h_diag);
     if (h->h_status) cudaFreeHost(h->h_status);
     if (h->prof_ev) {
         for (cudaEvent_t e : *h->prof_ev) cudaEventDestroy(e);
         delete h->prof_ev;
         delete h->prof_slot;
     }
+    delete h->xi;
+    delete h->xi2;
+    delete h->seed;
     delete h;
     return PIMD_OK;
 }
@@ -614,6 +886,7 @@ int pimd_set_gamma(pimd_t h, double gamma)
 {
     if (!h) return PIMD_EINVAL;
     if (!(gamma > 0) || !std::isfinite(gamma)) return fail(h, PIMD_EINVAL, "gamma must be positive");
+    if (gamma != h->gamma) drop_graphs(h); // the captured integrator nodes carry the friction as kernel arguments
     h->gamma = gamma;
     return PIMD_OK;
 }
@@ -625,21 +898,74 @@ int pimd_set_concurrency(pimd_t h, int on)
     return PIMD_OK;
 }
 
+int pimd_set_species(pimd_t h, int nspecies, const int *counts)
+{
+    if (!h) return PIMD_EINVAL;
+    if (h->carved) return fail(h, PIMD_EINVAL, "pimd_set_species must precede the first state / compute call");
+    if (nspecies < 1 || nspecies > PIMD_MAX_SPECIES || !counts) return fail(h, PIMD_EINVAL, "need 1 <= nspecies <= %d", PIMD_MAX_SPECIES);
+    long long tot = 0;
+    for (int k = 0; k < nspecies; ++k) {
+        if (counts[k] < 1) return fail(h, PIMD_EINVAL, "every species needs at least one particle");
+        tot += counts[k];
+    }
+    if (tot != h->N) return fail(h, PIMD_EINVAL, "species counts add up to %lld, not N = %d", tot, h->N);
+    h->nspecies = nspecies;
+    for (int k = 0; k < nspecies; ++k) h->counts[k] = counts[k];
+    setup_species(h);
+    return PIMD_OK;
+}
+
+int pimd_set_pair_potential(pimd_t h, int kind)
+{
+    if (!h) return PIMD_EINVAL;
+    if (kind != PIMD_PAIR_GAUSSIAN && kind != PIMD_PAIR_SOFT_COULOMB) return fail(h, PIMD_EINVAL, "unknown pair potential %d", kind);
+    if (kind != h->pot) { drop_graphs(h); h->forces_valid = false; }
+    h->pot = kind;
+    return PIMD_OK;
+}
+
+int pimd_set_pair_histogram(pimd_t h, int nbins, double rmax)
+{
+    if (!h) return PIMD_EINVAL;
+    if (nbins < 0 || nbins > MAX_BINS || (nbins > 0 && !(rmax > 0))) return fail(h, PIMD_EINVAL, "need 0 <= nbins <= %d and rmax > 0", MAX_BINS);
+    h->nbins_gr = nbins;
+    h->rmax_gr = rmax;
+    return PIMD_OK;
+}
+
+// copies between the caller's contiguous [B][n] doubles and the replica regions (rstride apart)
+static int copy_in(pimd_t h, double *dst, const double *src, size_t n, cudaMemcpyKind kind)
+{
+    CU(cudaMemcpy2DAsync(dst, h->rstride, src, n * 8, n * 8, (size_t)h->B, kind, h->s0));
+    return PIMD_OK;
+}
+static int copy_out(pimd_t h, double *dst, const double *src, size_t n, cudaMemcpyKind kind)
+{
+    CU(cudaMemcpy2DAsync(dst, n * 8, src, h->rstride, n * 8, (size_t)h->B, kind, h->s0));
+    return PIMD_OK;
+}
+
 static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpyKind kind)
 {
     if (!h) return PIMD_EINVAL;
     if (!x) return fail(h, PIMD_EINVAL, "x is NULL");
     int rc = ensure_ws(h);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->x, x, h->ndof * 8, kind, h->s0));
-    if (v) CU(cudaMemcpyAsync(h->v, v, h->ndof * 8, kind, h->s0));
-    else CU(cudaMemsetAsync(h->v, 0, h->ndof * 8, h->s0));
-    if (h->thermostat == PIMD_THERMOSTAT_NHC) CU(cudaMemsetAsync(h->nhc, 0, h->ndof * 8 * PIMD_NHC_LENGTH, h->s0));
-    CU(cudaMemsetAsync(h->status, 0, 4 * sizeof(int), h->s0));
+    rc = copy_in(h, h->x, x, h->ndof, kind);
+    if (rc) return rc;
+    if (v) rc = copy_in(h, h->v, v, h->ndof, kind);
+    else CU(cudaMemset2DAsync(h->v, h->rstride, 0, h->ndof * 8, (size_t)h->B, h->s0));
+    if (rc) return rc;
+    if (h->thermostat == PIMD_THERMOSTAT_NHC) CU(cudaMemset2DAsync(h->nhc, h->rstride, 0, h->ndof * 8 * PIMD_NHC_LENGTH, (size_t)h->B, h->s0));
+    CU(cudaMemset2DAsync(h->istatus, h->rstride, 0, 4, (size_t)h->B, h->s0));
+    for (int set = 0; set < 2; ++set)
+        for (int sp = 0; sp < h->nspecies; ++sp) CU(cudaMemset2DAsync(h->ex[set][sp].p.status, h->rstride, 0, 8, (size_t)h->B, h->s0));
     h->forces_valid = false;
     h->tables_valid = false;
-    // the exchange gauge of the last evaluation is kept: if the new positions are far from the old ones the
-    // stale-gauge kernel notices and redoes the recursion with a fresh max-plus gauge
+    h->scalars_valid = false;
+    h->shard_imported = false;
+    // The exchange gauge of the last evaluation is kept: the stale-gauge kernel accepts it only if every row sum stays
+    // within 2^+-8 of it (chain_cta_spec) and otherwise redoes the recursion with a fresh max-plus gauge.
     return PIMD_OK;
 }
 
@@ -648,8 +974,8 @@ static int get_state_impl(pimd_t h, double *x, double *v, cudaMemcpyKind kind)
     if (!h) return PIMD_EINVAL;
     int rc = ensure_ws(h);
     if (rc) return rc;
-    if (x) CU(cudaMemcpyAsync(x, h->x, h->ndof * 8, kind, h->s0));
-    if (v) CU(cudaMemcpyAsync(v, h->v, h->ndof * 8, kind, h->s0));
+    if (x && (rc = copy_out(h, x, h->x, h->ndof, kind))) return rc;
+    if (v && (rc = copy_out(h, v, h->v, h->ndof, kind))) return rc;
     CU(cudaStreamSynchronize(h->s0));
     return PIMD_OK;
 }
@@ -677,7 +1003,8 @@ int pimd_get_nhc(pimd_t h, double *nhc_dev)
     if (h->thermostat != PIMD_THERMOSTAT_NHC) return fail(h, PIMD_EINVAL, "thermostat is not Nose-Hoover");
     int rc = ensure_ws(h);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(nhc_dev, h->nhc, h->ndof * 8 * PIMD_NHC_LENGTH, cudaMemcpyDeviceToDevice, h->s0));
+    rc = copy_out(h, nhc_dev, h->nhc, h->ndof * PIMD_NHC_LENGTH, cudaMemcpyDeviceToDevice);
+    if (rc) return rc;
     CU(cudaStreamSynchronize(h->s0));
     return PIMD_OK;
 }
@@ -687,44 +1014,63 @@ int pimd_set_nhc(pimd_t h, const double *nhc_dev)
     if (h->thermostat != PIMD_THERMOSTAT_NHC) return fail(h, PIMD_EINVAL, "thermostat is not Nose-Hoover");
     int rc = ensure_ws(h);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->nhc, nhc_dev, h->ndof * 8 * PIMD_NHC_LENGTH, cudaMemcpyDeviceToDevice, h->s0));
+    return copy_in(h, h->nhc, nhc_dev, h->ndof * PIMD_NHC_LENGTH, cudaMemcpyDeviceToDevice);
+}
+
+static int launch_combine(pimd_t h, double *dst)
+{
+    const int own_first = (!h->sharded || h->j0 == 0) ? 1 : 0, own_last = (!h->sharded || h->j0 + h->P == h->Pg) ? 1 : 0;
+    {
+        ProfScope ps(h, PIMD_PROF_COMBINE, h->s0);
+        k_combine<<<dim3((unsigned)((h->ndof + 255) / 256), h->B), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P,
+                                                                                   own_first, own_last, h->rstride);
+    }
+    CU(cudaGetLastError());
+    return PIMD_OK;
+}
+
+// V_B and sign per replica from the species' scalars: V = sum over species, sign = product
+static int fetch_scalars(pimd_t h, double *vb, int *sign)
+{
+    const size_t B = (size_t)h->B;
+    CU(cudaMemcpy2DAsync(h->h_scal, sizeof(Scalars) * PIMD_MAX_SPECIES, h->scal[0], h->rstride, sizeof(Scalars) * PIMD_MAX_SPECIES, B,
+                         cudaMemcpyDeviceToHost, h->s0));
+    int rc = read_status(h);
+    if (rc) return rc;
+    for (size_t b = 0; b < B; ++b) {
+        double v = 0.0, sg = 1.0;
+        for (int sp = 0; sp < h->nspecies; ++sp) {
+            v += h->h_scal[b * PIMD_MAX_SPECIES + sp].vb;
+            sg *= h->h_scal[b * PIMD_MAX_SPECIES + sp].sign;
+        }
+        if (!std::isfinite(v)) return fail(h, PIMD_ENUMERIC, "V_B is not finite");
+        if (vb) vb[b] = v;
+        if (sign) sign[b] = sg < 0 ? -1 : 1;
+    }
     return PIMD_OK;
 }
 
 static int forces_impl(pimd_t h, double *f, bool host, double *vb, int *sign)
 {
     if (!h) return PIMD_EINVAL;
+    if (h->sharded) return fail(h, PIMD_EINVAL, "bead shard: use pimd_shard_forces");
     int rc = eval_forces(h, true, false, 0, 0.0);
     if (rc) return rc;
     if (f) {
-        double *dst = host ? h->Fout : f;
-        {
-            ProfScope ps(h, PIMD_PROF_COMBINE, h->s0);
-            k_combine<<<(unsigned)((h->ndof + 255) / 256), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P);
-        }
-        CU(cudaGetLastError());
-        if (host) CU(cudaMemcpyAsync(f, h->Fout, h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
+        rc = launch_combine(h, host ? h->Fout : f);
+        if (rc) return rc;
+        if (host) CU(cudaMemcpyAsync(f, h->Fout, (size_t)h->B * h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
     }
-    CU(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scalars), cudaMemcpyDeviceToHost, h->s0));
-    rc = read_status(h);
-    if (rc) return rc;
-    if (!std::isfinite(h->h_scal->vb)) return fail(h, PIMD_ENUMERIC, "V_B is not finite");
-    if (vb) *vb = h->h_scal->vb;
-    if (sign) *sign = h->h_scal->sign < 0 ? -1 : 1;
-    return PIMD_OK;
+    return fetch_scalars(h, vb, sign);
 }
 
 static int get_forces_impl(pimd_t h, double *f, bool host)
 {
     if (!h || !f) return PIMD_EINVAL;
     if (!h->forces_valid) return fail(h, PIMD_EINVAL, "no forces cached for the current positions");
-    double *dst = host ? h->Fout : f;
-    {
-        ProfScope ps(h, PIMD_PROF_COMBINE, h->s0);
-        k_combine<<<(unsigned)((h->ndof + 255) / 256), 256, 0, h->s0>>>(dst, h->F, h->Fex1, h->FexP, h->ndof, h->slice, h->P);
-    }
-    CU(cudaGetLastError());
-    if (host) CU(cudaMemcpyAsync(f, h->Fout, h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
+    int rc = launch_combine(h, host ? h->Fout : f);
+    if (rc) return rc;
+    if (host) CU(cudaMemcpyAsync(f, h->Fout, (size_t)h->B * h->ndof * 8, cudaMemcpyDeviceToHost, h->s0));
     CU(cudaStreamSynchronize(h->s0));
     return PIMD_OK;
 }
@@ -734,9 +1080,10 @@ static int set_forces_impl(pimd_t h, const double *f, cudaMemcpyKind kind)
     if (!h || !f) return PIMD_EINVAL;
     int rc = ensure_ws(h);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->F, f, h->ndof * 8, kind, h->s0));
-    CU(cudaMemsetAsync(h->Fex1, 0, h->slice * 8, h->s0));
-    CU(cudaMemsetAsync(h->FexP, 0, h->slice * 8, h->s0));
+    rc = copy_in(h, h->F, f, h->ndof, kind);
+    if (rc) return rc;
+    CU(cudaMemset2DAsync(h->Fex1, h->rstride, 0, h->slice * 8, (size_t)h->B, h->s0));
+    CU(cudaMemset2DAsync(h->FexP, h->rstride, 0, h->slice * 8, (size_t)h->B, h->s0));
     h->forces_valid = true;
     return PIMD_OK;
 }
@@ -752,24 +1099,27 @@ int pimd_forces_host(pimd_t h, double *f_host, double *vb, int *sign) { return f
 int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
 {
     if (!h) return PIMD_EINVAL;
+    if (h->B != 1 || h->nspecies != 1) return fail(h, PIMD_EINVAL, "tables are reported for one replica and one species");
     if (!h->tables_valid) return fail(h, PIMD_EINVAL, "no force evaluation to report");
+    if ((vfwd || vbwd) && h->all_zero[0]) return fail(h, PIMD_EINVAL, "tables are not formed for xi = 0");
+    const ExchPtrs &ex = h->ex[0][0].p;
     const int N = h->N;
-    if (pnext) CU(cudaMemcpyAsync(pnext, h->ex.pnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
+    const double lambda = (*h->xi)[0] != 0.0 ? std::log(std::fabs((*h->xi)[0])) : 0.0;
+    if (pnext) CU(cudaMemcpyAsync(pnext, ex.pnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
     if (vfwd || vbwd) {
         // V^{[1,n]} and V^{[u,N]} from the de-trended tables g: prefix sums of E_int and C(l,l+1)
         // are diagnostics of the evaluation, formed here in long double.
         std::vector<double> gf(2 * (size_t)(N + 1)), gb(2 * (size_t)(N + 1)), zf(N + 1), zb(N + 1), eint(N), cnext(N);
         double rf[4];
-        CU(cudaMemcpyAsync(gf.data(), h->ex.g[0], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(gb.data(), h->ex.g[1], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(zf.data(), h->ex.gs[0], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(zb.data(), h->ex.gs[1], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(eint.data(), h->ex.eint, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(cnext.data(), h->ex.cnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
-        CU(cudaMemcpyAsync(rf, h->ex.rfin, 32, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(gf.data(), ex.g[0], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(gb.data(), ex.g[1], (size_t)(N + 1) * 16, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(zf.data(), ex.gs[0], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(zb.data(), ex.gs[1], (size_t)(N + 1) * 8, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(eint.data(), ex.eint, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(cnext.data(), ex.cnext, (size_t)N * 8, cudaMemcpyDeviceToHost, h->s0));
+        CU(cudaMemcpyAsync(rf, ex.rfin, 32, cudaMemcpyDeviceToHost, h->s0));
         CU(cudaStreamSynchronize(h->s0));
-        if (h->xi == 0.0) return fail(h, PIMD_EINVAL, "tables are not formed for xi = 0");
-        const long double beta = h->beta, lam = h->lambda;
+        const long double beta = h->beta, lam = lambda;
         std::vector<long double> S(N + 1), T(N + 1); // 1-based: S[0] = 0, T[v] = S[v-1] + E_int[v], S[v] = T[v] + C[v][v+1]
         S[0] = 0;
         for (int v = 1; v <= N; ++v) {
@@ -808,11 +1158,17 @@ int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext)
     return PIMD_OK;
 }
 
+static int nxn_check(pimd_t h, const void *out)
+{
+    if (!h || !out) return PIMD_EINVAL;
+    if (h->B != 1 || h->nspecies != 1 || h->sharded) return fail(h, PIMD_EINVAL, "N x N output: one replica, one species, no bead shards");
+    if (h->N > 65535) return fail(h, PIMD_EINVAL, "N x N output supported up to N = 65535");
+    return ensure_ws(h);
+}
+
 int pimd_cycle_energies(pimd_t h, double *e_dev)
 {
-    if (!h || !e_dev) return PIMD_EINVAL;
-    if (h->N > 65535) return fail(h, PIMD_EINVAL, "N x N output supported up to N = 65535");
-    int rc = ensure_ws(h);
+    int rc = nxn_check(h, e_dev);
     if (rc) return rc;
     switch (h->d) {
     case 1: return cycle_energies_impl<1>(h, e_dev);
@@ -823,9 +1179,7 @@ int pimd_cycle_energies(pimd_t h, double *e_dev)
 
 int pimd_connection_probabilities(pimd_t h, double *pr_dev)
 {
-    if (!h || !pr_dev) return PIMD_EINVAL;
-    if (h->N > 65535) return fail(h, PIMD_EINVAL, "N x N output supported up to N = 65535");
-    int rc = ensure_ws(h);
+    int rc = nxn_check(h, pr_dev);
     if (rc) return rc;
     if (!h->tables_valid) {
         rc = eval_forces(h, false, false, 0, 0.0);
@@ -845,44 +1199,39 @@ int pimd_step(pimd_t h, int nsteps)
 {
     if (!h) return PIMD_EINVAL;
     if (nsteps < 0) return fail(h, PIMD_EINVAL, "nsteps < 0");
-    if (nsteps == 0) return PIMD_OK;
+    return run_steps(h, nsteps, 0, 0, 0.0);
+}
+
+int pimd_run(pimd_t h, int nsteps, int est_every, int nbins, double rmax)
+{
+    if (!h) return PIMD_EINVAL;
+    if (nsteps < 0 || est_every < 0) return fail(h, PIMD_EINVAL, "nsteps < 0 or est_every < 0");
+    if (nbins < 0 || nbins > MAX_BINS || (nbins > 0 && !(rmax > 0))) return fail(h, PIMD_EINVAL, "nbins must be in [0, %d] with rmax > 0", MAX_BINS);
+    return run_steps(h, nsteps, est_every, nbins, rmax);
+}
+
+int pimd_read_accumulators(pimd_t h, double *nsamples, double *sum_eprim, double *sum_evir, double *hist_sum, int nbins,
+                           double *gr_sum, int nbins_gr, int reset)
+{
+    if (!h) return PIMD_EINVAL;
+    if (nbins < 0 || nbins > MAX_BINS || nbins_gr < 0 || nbins_gr > MAX_BINS) return fail(h, PIMD_EINVAL, "bad bin count");
     int rc = ensure_ws(h);
     if (rc) return rc;
-    if (!h->forces_valid) {
-        rc = eval_forces(h, false, false, 0, 0.0);
-        if (rc) return rc;
+    const size_t B = (size_t)h->B;
+    CU(cudaMemcpy2DAsync(h->h_sums, sizeof(EstSums), h->sums, h->rstride, sizeof(EstSums), B, cudaMemcpyDeviceToHost, h->s0));
+    if (hist_sum && nbins > 0) CU(cudaMemcpy2DAsync(hist_sum, (size_t)nbins * 8, h->hist_acc, h->rstride, (size_t)nbins * 8, B, cudaMemcpyDeviceToHost, h->s0));
+    if (gr_sum && nbins_gr > 0) CU(cudaMemcpy2DAsync(gr_sum, (size_t)nbins_gr * 8, h->gr_acc, h->rstride, (size_t)nbins_gr * 8, B, cudaMemcpyDeviceToHost, h->s0));
+    if (reset) {
+        CU(cudaMemset2DAsync(h->sums, h->rstride, 0, sizeof(EstSums), B, h->s0));
+        CU(cudaMemset2DAsync(h->hist_acc, h->rstride, 0, (size_t)MAX_BINS * 8, B, h->s0));
+        CU(cudaMemset2DAsync(h->gr_acc, h->rstride, 0, (size_t)MAX_BINS * 8, B, h->s0));
     }
-    // open step s ; forces ; [close s + open s+1] ; forces ; ... ; close last
-    rc = launch_integrate(h, false, true, 0, h->step);
+    rc = read_status(h); // synchronises
     if (rc) return rc;
-    int it = 0;
-    const bool gauge_ok = h->gauge_valid || h->xi == 0.0;
-    if (h->use_graph && !h->profiling && gauge_ok && nsteps >= 3 && ensure_graph(h) == PIMD_OK) {
-        // all but the last step replay the captured graph; the step counter of the noise lives on the device meanwhile
-        k_step_counter<<<1, 32, 0, h->s0>>>(h->dstep, (unsigned long long)h->step, 0);
-        CU(cudaGetLastError());
-        CU(cudaEventRecord(h->ev_gin, h->s0));
-        CU(cudaStreamWaitEvent(h->sg, h->ev_gin, 0));
-        for (; it < nsteps - 1; ++it) {
-            CU(cudaGraphLaunch(h->gexec, h->sg));
-            h->launches += h->graph_launches;
-            h->step++;
-        }
-        CU(cudaEventRecord(h->ev_gout, h->sg));
-        CU(cudaStreamWaitEvent(h->s0, h->ev_gout, 0));
-        h->forces_valid = false; // set again below
-    }
-    for (; it < nsteps; ++it) {
-        rc = eval_forces(h, false, false, 0, 0.0);
-        if (rc) return rc;
-        const bool last = it == nsteps - 1;
-        rc = launch_integrate(h, true, !last, h->step, h->step + 1);
-        if (rc) return rc;
-        h->step++;
-    }
-    if (nsteps > 0) {
-        // forces in F belong to the final positions: still valid
-        h->forces_valid = true;
+    for (size_t b = 0; b < B; ++b) {
+        if (nsamples) nsamples[b] = h->h_sums[b].n;
+        if (sum_eprim) sum_eprim[b] = h->h_sums[b].sum_ep;
+        if (sum_evir) sum_evir[b] = h->h_sums[b].sum_ev;
     }
     return PIMD_OK;
 }
@@ -893,16 +1242,199 @@ int pimd_estimators(pimd_t h, double *e_prim, double *e_vir, double *hist, int n
     if (nbins < 0 || nbins > MAX_BINS) return fail(h, PIMD_EINVAL, "nbins must be in [0, %d]", MAX_BINS);
     if (nbins > 0 && (!hist || !(rmax > 0))) return fail(h, PIMD_EINVAL, "hist is NULL or rmax <= 0");
     int rc = eval_forces(h, true, true, nbins, rmax);
+    if (rc == PIMD_OK) rc = launch_estimate(h, nbins, false);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(h->h_scal, h->scal, sizeof(Scalars), cudaMemcpyDeviceToHost, h->s0));
-    CU(cudaMemcpyAsync(h->h_est, h->est, sizeof(EstAccum), cudaMemcpyDeviceToHost, h->s0));
-    if (nbins > 0) CU(cudaMemcpyAsync(hist, h->hist, (size_t)nbins * 8, cudaMemcpyDeviceToHost, h->s0));
+    const size_t B = (size_t)h->B;
+    CU(cudaMemcpy2DAsync(h->h_sums, sizeof(EstSums), h->sums, h->rstride, sizeof(EstSums), B, cudaMemcpyDeviceToHost, h->s0));
+    if (nbins > 0) CU(cudaMemcpy2DAsync(hist, (size_t)nbins * 8, h->hist, h->rstride, (size_t)nbins * 8, B, cudaMemcpyDeviceToHost, h->s0));
     rc = read_status(h);
     if (rc) return rc;
-    // Ubar = U/P: the trap term is accumulated already divided by P, the pair terms are not
-    const double ubar = h->h_est->utrap + h->h_est->upair / h->P;
-    if (e_prim) *e_prim = (double)h->P * h->d * h->N / (2.0 * h->beta) - h->h_scal->ec + ubar;
-    if (e_vir) *e_vir = 2.0 * h->h_est->utrap + h->h_est->virpair / h->P;
+    for (size_t b = 0; b < B; ++b) {
+        if (e_prim) e_prim[b] = h->h_sums[b].last_ep;
+        if (e_vir) e_vir[b] = h->h_sums[b].last_ev;
+    }
+    return PIMD_OK;
+}
+
+int pimd_pair_histogram(pimd_t h, double *gr_host)
+{
+    if (!h || !gr_host) return PIMD_EINVAL;
+    if (h->nbins_gr <= 0) return fail(h, PIMD_EINVAL, "pimd_set_pair_histogram first");
+    if (!h->carved) return fail(h, PIMD_EINVAL, "no estimator evaluation yet");
+    CU(cudaMemcpy2DAsync(gr_host, (size_t)h->nbins_gr * 8, h->gr, h->rstride, (size_t)h->nbins_gr * 8, (size_t)h->B, cudaMemcpyDeviceToHost, h->s0));
+    CU(cudaStreamSynchronize(h->s0));
+    return PIMD_OK;
+}
+
+int pimd_reweight(pimd_t h, const double *xi_obs, double *ln_abs_r, int *sign, double *eps_obs, double *eps_samp)
+{
+    if (!h || !xi_obs) return PIMD_EINVAL;
+    if (h->sharded) return fail(h, PIMD_EINVAL, "pimd_reweight is not available on a bead shard");
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    bool any0 = false, anynz = false, same = true;
+    for (int b = 0; b < h->B; ++b) {
+        if (!std::isfinite(xi_obs[b])) return fail(h, PIMD_EINVAL, "xi_obs must be finite");
+        if (xi_obs[b] == 0.0) any0 = true; else anynz = true;
+        same = same && xi_obs[b] == (*h->xi2)[b];
+    }
+    if (any0 && anynz) return fail(h, PIMD_EINVAL, "xi_obs is either all 0 or all != 0");
+    if (!same) {
+        h->xi2->assign(xi_obs, xi_obs + h->B);
+        rc = upload_params(h, 1);
+        if (rc) return rc;
+        for (int sp = 0; sp < h->nspecies; ++sp) h->ex[1][sp].gauge_valid = false;
+    }
+    // the sampling xi's tables and scalars at the current positions
+    if (!h->tables_valid) {
+        rc = eval_forces(h, true, false, 0, 0.0);
+        if (rc) return rc;
+    } else if (!h->scalars_valid) {
+        for (int sp = 0; sp < h->nspecies; ++sp) {
+            ExchCtx &c = h->ex[0][sp];
+            ProfScope ps(h, PIMD_PROF_FINALIZE, h->s0);
+            k_finalize<256><<<h->B, 256, 0, h->s0>>>(c.N, c.nprep, c.nasm, h->beta, c.rp, std::lgamma((double)c.N + 1.0), c.p, c.ecpart, c.scal, h->rstride);
+        }
+        CU(cudaGetLastError());
+        h->scalars_valid = true;
+    }
+    // the same recursion with xi_obs (second set of exchange tables; its exterior forces go to a scratch buffer)
+    for (int sp = 0; sp < h->nspecies; ++sp) {
+        rc = prep_d(h, h->ex[1][sp], h->s0);
+        if (rc == PIMD_OK) rc = exchange_d(h, h->ex[1][sp], 1, h->s0, true);
+        if (rc) return rc;
+    }
+    const size_t B = (size_t)h->B, row = sizeof(Scalars) * PIMD_MAX_SPECIES;
+    std::vector<Scalars> obs(B * PIMD_MAX_SPECIES);
+    CU(cudaMemcpy2DAsync(obs.data(), row, h->scal[1], h->rstride, row, B, cudaMemcpyDeviceToHost, h->s0));
+    CU(cudaMemcpy2DAsync(h->h_scal, row, h->scal[0], h->rstride, row, B, cudaMemcpyDeviceToHost, h->s0));
+    for (int sp = 0; sp < h->nspecies; ++sp)
+        CU(cudaMemcpy2DAsync(h->h_status + B * (1 + PIMD_MAX_SPECIES + sp), 4, h->ex[1][sp].p.status, h->rstride, 4, B, cudaMemcpyDeviceToHost, h->s0));
+    rc = read_status(h);
+    if (rc) return rc;
+    for (size_t b = 0; b < B; ++b) {
+        double vo = 0.0, vs = 0.0, so = 1.0, ss = 1.0, eo = 0.0, es = 0.0;
+        int st = 0;
+        for (int sp = 0; sp < h->nspecies; ++sp) {
+            const Scalars &o = obs[b * PIMD_MAX_SPECIES + sp], &q = h->h_scal[b * PIMD_MAX_SPECIES + sp];
+            vo += o.vb; so *= o.sign; eo += o.ec;
+            vs += q.vb; ss *= q.sign; es += q.ec;
+            st |= h->h_status[B * (1 + PIMD_MAX_SPECIES + sp) + b];
+        }
+        if (st & ST_NODE) return fail(h, PIMD_ENUMERIC, "W(xi_obs) summed to zero (a node)");
+        if (!std::isfinite(vo) || !std::isfinite(vs)) return fail(h, PIMD_ENUMERIC, "V_B is not finite");
+        if (ln_abs_r) ln_abs_r[b] = -h->beta * (vo - vs);
+        if (sign) sign[b] = (so * ss < 0) ? -1 : 1;
+        if (eps_obs) eps_obs[b] = -eo;
+        if (eps_samp) eps_samp[b] = -es;
+    }
+    return PIMD_OK;
+}
+
+// ---- bead shards ------------------------------------------------------------------------------------
+int pimd_shard_layout(pimd_t h, int *j0, int *p_local, size_t *pack_doubles)
+{
+    if (!h) return PIMD_EINVAL;
+    if (j0) *j0 = h->j0;
+    if (p_local) *p_local = h->P;
+    if (pack_doubles) *pack_doubles = 2 * h->slice + (size_t)h->N;
+    return PIMD_OK;
+}
+
+int pimd_shard_export(pimd_t h, double *send_dev)
+{
+    if (!h || !send_dev) return PIMD_EINVAL;
+    if (!h->sharded) return fail(h, PIMD_EINVAL, "not a bead shard (pimd_create_sharded)");
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    const unsigned grid = (unsigned)((h->N + 127) / 128);
+    ProfScope ps(h, PIMD_PROF_SHARD, h->s0);
+    switch (h->d) {
+    case 1: k_shard_pack<1><<<grid, 128, 0, h->s0>>>(h->x, h->N, h->P, h->ks, send_dev); break;
+    case 2: k_shard_pack<2><<<grid, 128, 0, h->s0>>>(h->x, h->N, h->P, h->ks, send_dev); break;
+    default: k_shard_pack<3><<<grid, 128, 0, h->s0>>>(h->x, h->N, h->P, h->ks, send_dev); break;
+    }
+    CU(cudaGetLastError());
+    return PIMD_OK;
+}
+
+static int shard_import(pimd_t h, const double *gathered_dev)
+{
+    const size_t packn = 2 * h->slice + (size_t)h->N;
+    CU(cudaMemcpyAsync(h->gathered, gathered_dev, (size_t)h->world * packn * 8, cudaMemcpyDeviceToDevice, h->s0));
+    const unsigned grid = (unsigned)((h->N + 127) / 128);
+    {
+        ProfScope ps(h, PIMD_PROF_SHARD, h->s0);
+        switch (h->d) {
+        case 1: k_shard_eint<1><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
+        case 2: k_shard_eint<2><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
+        default: k_shard_eint<3><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
+        }
+    }
+    CU(cudaGetLastError());
+    h->shard_imported = true;
+    return PIMD_OK;
+}
+
+int pimd_shard_forces(pimd_t h, const double *gathered_dev)
+{
+    if (!h || !gathered_dev) return PIMD_EINVAL;
+    if (!h->sharded) return fail(h, PIMD_EINVAL, "not a bead shard (pimd_create_sharded)");
+    int rc = ensure_ws(h);
+    if (rc == PIMD_OK) rc = shard_import(h, gathered_dev);
+    if (rc == PIMD_OK) rc = eval_forces(h, true, false, 0, 0.0);
+    return rc;
+}
+
+int pimd_shard_scalars(pimd_t h, double *vb, int *sign)
+{
+    if (!h) return PIMD_EINVAL;
+    if (!h->scalars_valid) return fail(h, PIMD_EINVAL, "no evaluation with scalars to report");
+    return fetch_scalars(h, vb, sign);
+}
+
+int pimd_shard_begin_step(pimd_t h, double *send_dev)
+{
+    if (!h || !send_dev) return PIMD_EINVAL;
+    if (!h->sharded) return fail(h, PIMD_EINVAL, "not a bead shard (pimd_create_sharded)");
+    if (!h->forces_valid) return fail(h, PIMD_EINVAL, "bead shard: evaluate the forces of the starting state first (pimd_shard_export + pimd_shard_forces)");
+    int rc = launch_integrate(h, false, true, 0, h->step);
+    if (rc) return rc;
+    h->forces_valid = false;
+    h->tables_valid = false;
+    h->scalars_valid = false;
+    return pimd_shard_export(h, send_dev);
+}
+
+int pimd_shard_end_step(pimd_t h, const double *gathered_dev)
+{
+    if (!h || !gathered_dev) return PIMD_EINVAL;
+    if (!h->sharded) return fail(h, PIMD_EINVAL, "not a bead shard (pimd_create_sharded)");
+    int rc = shard_import(h, gathered_dev);
+    if (rc == PIMD_OK) rc = eval_forces(h, false, false, 0, 0.0);
+    if (rc == PIMD_OK) rc = launch_integrate(h, true, false, h->step, 0);
+    if (rc) return rc;
+    h->shard_imported = true; // close does not move the positions
+    h->step++;
+    return PIMD_OK;
+}
+
+int pimd_get_diagnostics(pimd_t h, uint64_t *out)
+{
+    if (!h || !out) return PIMD_EINVAL;
+    int rc = ensure_ws(h);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h->h_diag, h->fallbacks, 8, cudaMemcpyDeviceToHost, h->s0));
+    const int B = h->B, S = h->nspecies;
+    for (int sp = 0; sp < S; ++sp)
+        CU(cudaMemcpy2DAsync(h->h_status + (size_t)B * (1 + sp), 4, h->ex[0][sp].p.status + 1, h->rstride, 4, (size_t)B, cudaMemcpyDeviceToHost, h->s0));
+    CU(cudaStreamSynchronize(h->s0));
+    int sticky = 0;
+    for (int k = B; k < B * (1 + S); ++k) sticky |= h->h_status[k];
+    out[0] = h->h_diag[0];
+    out[1] = (uint64_t)sticky;
+    out[2] = (uint64_t)h->ex[0][0].nworkers;
+    out[3] = (uint64_t)h->rstride;
     return PIMD_OK;
 }
 

@@ -75,6 +75,10 @@ PIMD_DEV void st_relaxed_f64(double *p, double v)
     asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 
+// Replica b of a batch lives `rs` bytes behind replica b-1 with the same layout: a kernel is handed the pointers of
+// replica 0 and shifts them by blockIdx.{y,z} * rs.
+template <class T> PIMD_DEV T *rshift(T *p, size_t off) { return (T *)((size_t)p + off); }
+
 // status word bits (device -> host)
 enum { ST_NONFINITE = 1, ST_NODE = 2 };
 
@@ -97,28 +101,27 @@ template <int NT> PIMD_DEV double block_sum(double v, double *sh /* NT/32 double
 }
 
 // ==========================================================================================
-// Step 1+2 of the hot path: spring + trap + pair forces of every bead.
+// Step 1 of the hot path: spring + trap forces of every bead.
 //   F[j][l] = intra-ring springs (Eq. 17; for j = 1, P the intra-ring half of
-//             Eq. 15/16) - (1/P) omega^2 r (Eq. 4/19) + (1/P) sum_{i != l} (2g/s^2) e^{-r^2/s^2} (r_l - r_i)
-//             (Eq. 18 :142 with v(r) = g e^{-r^2/s^2})
-// grid (ceil(N/TB), P), block TB.  One thread owns one bead (j,l); the slice x[j][.][.] is
-// staged through shared memory in tiles of TB particles, read back as broadcasts.
-// Padding particles sit at +1e150 so that their Gaussian is exactly 0; the i == l term has
-// r = 0 and contributes no force (its energy g is subtracted analytically).
-// EST: also accumulate U_trap, U_pair and the pair virial sum_{i<l} (1 - r^2/s^2) g e^{-r^2/s^2},
-// and the radial histogram.
+//             Eq. 15/16) - (1/P) omega^2 r (Eq. 4/19)
+// grid (ceil(N/TB), P, B), block TB.  One thread owns one bead (j,l).  F is written (the pair kernel adds to it).
+// EST: also accumulate U_trap and the radial histogram.
 // ==========================================================================================
 struct EstAccum {
     double utrap, upair, virpair, ec, pad[4];
 };
 
-template <int D, bool PAIR, bool EST, int TB>
+template <int D, bool EST, int TB>
 __global__ void __launch_bounds__(TB) k_bead(const double *__restrict__ x, double *__restrict__ F, int N, int P,
-                                            double ks, double om2_over_P, double is2, double pair_coef /* 2g/(s^2 P) */,
-                                            double g, EstAccum *est, double *hist, int nbins, double rmax)
+                                            double ks, double om2_over_P, EstAccum *est, double *hist, int nbins, double rmax,
+                                            const double *__restrict__ halo_lo, const double *__restrict__ halo_hi, size_t rs)
 {
-    __shared__ double tile[TB * D];
+    // P = number of bead slices held here.  A bead shard holds a contiguous range of the ring's slices and
+    // gets the neighbouring ranks' boundary slices as halo_lo (the slice below local slice 0) / halo_hi (above local slice
+    // P-1); NULL where the ring polymer itself ends (global bead 1 / bead P) and for an unsharded handle.
     __shared__ double red[TB / 32];
+    const size_t off = (size_t)blockIdx.z * rs;
+    x = rshift(x, off); F = rshift(F, off);
     const int j = blockIdx.y;
     const int l = blockIdx.x * TB + threadIdx.x;
     const bool valid = l < N;
@@ -134,77 +137,25 @@ __global__ void __launch_bounds__(TB) k_bead(const double *__restrict__ x, doubl
         // the exchange kernels (Eq. 15, 16).
 #pragma unroll
         for (int c = 0; c < D; ++c) f.v[c] = -om2_over_P * r.v[c];
-        if (j > 0) {
-            Vec<D> a = ldvec<D>(xs - (size_t)N * D, l);
+        if (j > 0 || halo_lo != nullptr) {
+            Vec<D> a = (j > 0) ? ldvec<D>(xs - (size_t)N * D, l) : ldvec<D>(rshift(halo_lo, off), l);
 #pragma unroll
             for (int c = 0; c < D; ++c) f.v[c] -= ks * (r.v[c] - a.v[c]);
         }
-        if (j < P - 1) {
-            Vec<D> a = ldvec<D>(xs + (size_t)N * D, l);
+        if (j < P - 1 || halo_hi != nullptr) {
+            Vec<D> a = (j < P - 1) ? ldvec<D>(xs + (size_t)N * D, l) : ldvec<D>(rshift(halo_hi, off), l);
 #pragma unroll
             for (int c = 0; c < D; ++c) f.v[c] -= ks * (r.v[c] - a.v[c]);
         }
 #pragma unroll
         for (int c = 0; c < D; ++c) r2self = fma(r.v[c], r.v[c], r2self);
     }
-    double up = 0.0, vir = 0.0;
-    if constexpr (PAIR) {
-        Vec<D> acc;
-#pragma unroll
-        for (int c = 0; c < D; ++c) acc.v[c] = 0.0;
-        const double nis2 = -is2;
-        for (int t0 = 0; t0 < N; t0 += TB) {
-            __syncthreads();
-            {
-                const int i = t0 + threadIdx.x;
-                Vec<D> p;
-                if (i < N) p = ldvec<D>(xs, i);
-                else {
-#pragma unroll
-                    for (int c = 0; c < D; ++c) p.v[c] = -1e150;
-                }
-#pragma unroll
-                for (int c = 0; c < D; ++c) tile[threadIdx.x * D + c] = p.v[c];
-            }
-            __syncthreads();
-#pragma unroll 4
-            for (int k = 0; k < TB; ++k) {
-                Vec<D> dlt;
-#pragma unroll
-                for (int c = 0; c < D; ++c) dlt.v[c] = r.v[c] - tile[k * D + c];
-                double r2 = dlt.v[0] * dlt.v[0];
-#pragma unroll
-                for (int c = 1; c < D; ++c) r2 = fma(dlt.v[c], dlt.v[c], r2);
-                const double arg = r2 * nis2;
-                const double e = exp_fast(arg);
-#pragma unroll
-                for (int c = 0; c < D; ++c) acc.v[c] = fma(e, dlt.v[c], acc.v[c]);
-                if constexpr (EST) {
-                    up += e;
-                    vir = fma(e, arg, vir); // sum e * (-r^2/s^2)
-                }
-            }
-        }
-#pragma unroll
-        for (int c = 0; c < D; ++c) f.v[c] = fma(pair_coef, acc.v[c], f.v[c]);
-    }
     if (valid) stvec<D>(F + (size_t)j * N * D, l, f);
     if constexpr (EST) {
-        // ordered pairs were summed, including i == l (e = 1, arg = 0): remove it, halve the rest
+        est = rshift(est, off); hist = rshift(hist, off);
         double utr = valid ? 0.5 * om2_over_P * r2self : 0.0; // (1/P) 1/2 omega^2 r^2
-        double upl = 0.0, virl = 0.0;
-        if (PAIR && valid) {
-            upl = 0.5 * g * (up - 1.0);
-            virl = 0.5 * g * (up - 1.0 + vir);
-        }
         double s1 = block_sum<TB>(utr, red);
-        double s2 = block_sum<TB>(upl, red);
-        double s3 = block_sum<TB>(virl, red);
-        if (threadIdx.x == 0) {
-            atomicAdd(&est->utrap, s1);
-            atomicAdd(&est->upair, s2);
-            atomicAdd(&est->virpair, s3);
-        }
+        if (threadIdx.x == 0) atomicAdd(&est->utrap, s1);
         if (nbins > 0 && valid) {
             const double rr = sqrt(r2self);
             if (rr < rmax) {
@@ -232,22 +183,55 @@ struct ExchPtrs {
     double *tpart;        // [2*nprepblocks] per-block partial sums of E_int, cnext
     double2 *rfin;        // [2]
     double *rsgn;         // [2]
-    int *status;
+    int *status;          // [2]: [0] ST_* bits of the current evaluation, [1] the same, sticky since pimd_set_state
 };
+
+// Per-replica parameters, kept in the replica's workspace region (a batch advances B replicas that differ in xi and
+// in the noise seed with one set of launches).
+struct RepParams {
+    double xi, lambda /* ln|xi|, 0 for xi = 0 */, sx /* sgn xi */;
+    unsigned long long seed;
+};
+
+PIMD_DEV ExchPtrs rshift(ExchPtrs p, size_t off)
+{
+    if (off == 0) return p;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        p.rho[k] = rshift(p.rho[k], off); p.sig[k] = rshift(p.sig[k], off); p.cc[k] = rshift(p.cc[k], off);
+        p.g[k] = rshift(p.g[k], off); p.gs[k] = rshift(p.gs[k], off);
+        p.pan_m[k] = rshift(p.pan_m[k], off); p.pan_s[k] = rshift(p.pan_s[k], off);
+        p.panel_ready[k] = rshift(p.panel_ready[k], off); p.acc[k] = rshift(p.acc[k], off);
+    }
+    p.cols_ready = rshift(p.cols_ready, off);
+    p.eint = rshift(p.eint, off); p.cnext = rshift(p.cnext, off); p.cself = rshift(p.cself, off); p.pnext = rshift(p.pnext, off);
+    p.tpart = rshift(p.tpart, off); p.rfin = rshift(p.rfin, off); p.rsgn = rshift(p.rsgn, off); p.status = rshift(p.status, off);
+    return p;
+}
 
 constexpr int PREP_SPLIT = 4; // thread groups that share the bead loop of a particle
 
+// x: bead-major coordinates already offset to the first particle of this exchange problem (a species, SURVEY 8(f4),
+// the recursion of Eq. 6 runs over that index range alone), `sl` doubles between consecutive bead slices,
+// P slices; x1 / xP: the bead-1 and bead-P slices (same offset).  eint_in != NULL (bead shards): E_int comes
+// summed over the ranks' slices instead of from the bead loop (x may be NULL).  grid (nprep, B).
 template <int D, int TB>
-__global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restrict__ x, int N, int P, int NB, double ks, double kk,
-                                                        double lambda, ExchPtrs p)
+__global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restrict__ x, const double *__restrict__ x1s,
+                                                        const double *__restrict__ xPs, const double *__restrict__ eint_in,
+                                                        size_t sl, int N, int P, int NB, double ks, double kk, ExchPtrs p,
+                                                        const RepParams *rp, int *gauge_misfit, size_t rs)
 {
     __shared__ double red[TB * PREP_SPLIT / 32];
     __shared__ double part_s[PREP_SPLIT][TB];
+    const size_t off = (size_t)blockIdx.y * rs;
+    p = rshift(p, off);
+    x1s = rshift(x1s, off); xPs = rshift(xPs, off);
+    const double lambda = rshift(rp, off)->lambda;
     const int lt = threadIdx.x % TB, part = threadIdx.x / TB;
     const int l = blockIdx.x * TB + lt;
-    const size_t sl = (size_t)N * D;
-    {
+    if (eint_in == nullptr) {
         // the P-1 bead differences of particle l, in PREP_SPLIT contiguous segments
+        x = rshift(x, off);
         const int per = (P - 1 + PREP_SPLIT - 1) / PREP_SPLIT, j0 = 1 + part * per, j1 = min(P, j0 + per);
         double accp = 0.0;
         if (l < N && j0 < j1) {
@@ -263,13 +247,16 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
     __syncthreads();
     double e_int = 0.0, cn = 0.0;
     if (part == 0 && l < N) {
-        double acc = 0.0;
+        if (eint_in == nullptr) {
+            double acc = 0.0;
 #pragma unroll
-        for (int q = 0; q < PREP_SPLIT; ++q) acc += part_s[q][lt];
-        const Vec<D> x1 = ldvec<D>(x, l);
-        const Vec<D> prev = ldvec<D>(x + (size_t)(P - 1) * sl, l);
-        const Vec<D> xP = prev;
-        e_int = 0.5 * ks * acc;
+            for (int q = 0; q < PREP_SPLIT; ++q) acc += part_s[q][lt];
+            e_int = 0.5 * ks * acc;
+        } else {
+            e_int = rshift(eint_in, off)[l];
+        }
+        const Vec<D> x1 = ldvec<D>(x1s, l);
+        const Vec<D> xP = ldvec<D>(xPs, l);
         stvec<D>(p.rho[0], l, xP);
         stvec<D>(p.sig[0], l, x1);
         stvec<D>(p.rho[1], N - 1 - l, x1);
@@ -277,7 +264,7 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
         p.eint[l] = e_int;
         p.cself[l] = kk * dist2<D>(xP, x1);
         if (l < N - 1) {
-            Vec<D> x1n = ldvec<D>(x, l + 1);
+            Vec<D> x1n = ldvec<D>(x1s, l + 1);
             cn = kk * dist2<D>(xP, x1n);
             const double c = cn - lambda - log((double)(l + 1));
             p.cc[0][l] = c;
@@ -314,8 +301,10 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
             p.gs[1][0] = 1.0;
             p.cols_ready[0] = 1;
             p.cols_ready[1] = 1;
-            *p.status = 0;
-            p.status[2] = 0;
+            // status[0]: bits of the evaluation that starts here; status[1]: every bit seen since pimd_set_state
+            p.status[1] |= p.status[0];
+            p.status[0] = 0;
+            if (blockIdx.y == 0) *gauge_misfit = 0;
         }
     }
     double s1 = block_sum<TB * PREP_SPLIT>(e_int, red);
@@ -345,9 +334,13 @@ constexpr int CH_MAXLOOK = 3; // (4 L + 1) * 32 part entries are scaled by one p
 
 struct ChainArgs {
     int N, NB, look, nworkers;
-    double kk, sx;
-    ExchPtrs p;
+    double kk;
+    ExchPtrs p;                // replica 0; replica b of a batch is rs bytes further on (grid.z = replica)
+    const RepParams *rp;       // likewise: sgn xi of the replica
+    size_t rs;
     int look_fb;               // k_chain_spec: look-ahead of the max-plus recursion it falls back to
+    int *gauge_misfit;         // k_chain_spec: one flag for the whole launch (all replicas fall back together)
+    unsigned long long *fallbacks; // counts the launches that fell back
     unsigned long long *phase; // optional [16]: cycles of the forward chain CTA per phase (profiling), or NULL
 };
 
@@ -413,8 +406,11 @@ PIMD_DEV double approx_log_abs(double s)
 // the SM's load/store pipe, and helper traffic placed beside the passes delayed them one for one.
 // ==========================================================================================
 template <int D, bool SGN>
-__device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, const double *etab)
+__device__ void chain_cta(const ChainArgs &a, int dir, size_t roff, unsigned char *smem_raw, const double *etab)
 {
+    unsigned long long *const phase = (roff == 0) ? a.phase : nullptr;
+    [[maybe_unused]] double sx = rshift(a.rp, roff)->sx; // this replica's sgn xi
+    asm volatile("" : "+d"(sx));
     int N = a.N, L = a.look;
     // keep the two in registers: re-reading kernel parameters from the constant bank inside the block loop
     // was measured to stall the dependent warp for hundreds of cycles
@@ -431,9 +427,9 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     float *part_g = reinterpret_cast<float *>(sm + lay.partG);
     double *part_m = sm + lay.partM, *part_s = sm + lay.partS, *apart_s = sm + lay.apart, *sh_s = sm + lay.sh;
 
-    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
-    double2 *g = a.p.g[dir];
-    double *gs = a.p.gs[dir];
+    const double *rho = rshift(a.p.rho[dir], roff), *sig = rshift(a.p.sig[dir], roff), *cc = rshift(a.p.cc[dir], roff);
+    double2 *g = rshift(a.p.g[dir], roff);
+    double *gs = rshift(a.p.gs[dir], roff);
     const double kk = a.kk;
     const bool is_io = (warp == CH_WARPS - 1); // the warp that talks to global memory
 
@@ -529,7 +525,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     // optional phase clock of the forward chain CTA: slot 2k-1 = warp 0's own time in phase k, slot 2k = its
     // wait at the barrier that ends phase k, slot 0 = loop overhead
     __shared__ long long ph_s[16];
-    const bool tim = a.phase != nullptr && dir == 0 && tid == 0;
+    const bool tim = phase != nullptr && dir == 0 && tid == 0;
     if (tid < 16) ph_s[tid] = 0;
     long long tprev = clock64();
 #define PH(k) do { if (tim) { const long long c__ = clock64(); ph_s[k] += c__ - tprev; tprev = c__; } } while (0)
@@ -558,15 +554,15 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             if (jrec0n > 0) {
                 int ready = 0;
                 if (lane == 0) {
-                    ready = ld_acquire(&a.p.panel_ready[dir][K + 1]);
-                    while (wait && ready == 0) ready = ld_acquire(&a.p.panel_ready[dir][K + 1]);
+                    ready = ld_acquire(&rshift(a.p.panel_ready[dir], roff)[K + 1]);
+                    while (wait && ready == 0) ready = ld_acquire(&rshift(a.p.panel_ready[dir], roff)[K + 1]);
                 }
                 ready = __shfl_sync(0xffffffffu, ready, 0);
                 if (!ready) return;
                 const int i = i0 + 32 + lane;
                 if (i < N) {
-                    m = ldcg1(&a.p.pan_m[dir][i]) + dd_diff(ring_T[jrec0n & (RB - 1)], Tref);
-                    s = ldcg1(&a.p.pan_s[dir][i]);
+                    m = ldcg1(&rshift(a.p.pan_m[dir], roff)[i]) + dd_diff(ring_T[jrec0n & (RB - 1)], Tref);
+                    s = ldcg1(&rshift(a.p.pan_s[dir], roff)[i]);
                 }
             }
             pmN[lane] = m;
@@ -614,7 +610,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
                 // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
                 __syncwarp();
-                if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
+                if (lane == 0) st_release(&rshift(a.p.cols_ready, roff)[dir], min(N, i0 + 1));
                 pend_ready = 0;
             }
             panel_done = 0;
@@ -661,7 +657,7 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
             const double a0 = (((double)ts_s[p0] - Gr) + dgK[tid]) + dlt_s[p0];
             const double a1 = (((double)ts_s[p1] - Gr) + dgK[tid + 512]) + dlt_s[p1];
             double m0 = exp_tab(a0, etab), m1 = exp_tab(a1, etab);
-            if constexpr (SGN) { if (p0 >= 1) m0 *= a.sx; m1 *= a.sx; }
+            if constexpr (SGN) { if (p0 >= 1) m0 *= sx; m1 *= sx; }
             dgK[tid] = m0;
             dgK[tid + 512] = m1;
             const int ai = tid - (CH_THREADS - NP * 32); // the last warps also scale the earlier-column parts
@@ -693,8 +689,8 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
                 if (lane == p + 1) zmine = zc;
             }
             accr = acc;
-            if (lane >= 1) zK[lane] = SGN ? a.sx * zmine : zmine;
-            if (lane == 0) { zK[32] = SGN ? a.sx * zc : zc; zN[0] = SGN ? a.sx * zc : zc; }
+            if (lane >= 1) zK[lane] = SGN ? sx * zmine : zmine;
+            if (lane == 0) { zK[32] = SGN ? sx * zc : zc; zN[0] = SGN ? sx * zc : zc; }
         } else if (is_io) {
             if (has_next) {
                 if (!panel_done) fetch_panel(true);
@@ -779,21 +775,21 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
     }
 #undef PH
     if (tim) {
-        for (int k = 0; k < 16; ++k) a.phase[k] += (unsigned long long)ph_s[k];
+        for (int k = 0; k < 16; ++k) phase[k] += (unsigned long long)ph_s[k];
     }
     if (warp == 0) {
         // R_{N-1} = T + G + log|X^| of the last row, its sign, and the status of all rows
         if (lane == (N - 1) % 32) {
-            a.p.rfin[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
-            a.p.rsgn[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
+            rshift(a.p.rfin, roff)[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
+            rshift(a.p.rsgn, roff)[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
         }
-        if (bad) atomicOr(a.p.status, bad);
+        if (bad) atomicOr(rshift(a.p.status, roff), bad);
     }
     if (is_io && pend_ready) {
         if (pend_j >= 0) { g[pend_j] = pend_T; gs[pend_j] = pend_Z; }
         // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
         __syncwarp();
-        if (lane == 0) st_release(&a.p.cols_ready[dir], N);
+        if (lane == 0) st_release(&rshift(a.p.cols_ready, roff)[dir], N);
     }
 }
 
@@ -816,8 +812,8 @@ __device__ void chain_cta(const ChainArgs &a, int dir, unsigned char *smem_raw, 
 //   frame (exact powers of two), so a systematic drift of the solution along the chain cannot overflow.
 //   warp 0 folds E'(K+1) Zhat into the next block's start value inside its own loop (one more DFMA per
 //   step, off the dependent path), so one block-wide barrier per block is all the synchronisation.
-// A row sum outside [1e-270, 1e270] (the gauge no longer fits: first evaluation, state replaced, a jump)
-// raises status[2]; k_chain_spec then redoes the recursion with the max-plus code after a grid barrier.
+// A row sum outside 2^+-8 of its gauge (the gauge no longer fits: state replaced, a jump) raises the misfit flag;
+// k_chain_spec then redoes the recursion with the max-plus code after a grid barrier.
 // ==========================================================================================
 #ifndef PIMD_SPEC_NHW
 #define PIMD_SPEC_NHW 9
@@ -854,8 +850,11 @@ template <int D> struct SpecSmem {
 };
 
 template <int D, bool SGN>
-__device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_raw, const double *etab64)
+__device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigned char *smem_raw, const double *etab64)
 {
+    unsigned long long *const phase = (roff == 0) ? a.phase : nullptr;
+    [[maybe_unused]] double sx = rshift(a.rp, roff)->sx; // this replica's sgn xi
+    asm volatile("" : "+d"(sx));
     int N = a.N, L = a.look, NBk = a.NB;
     asm volatile("" : "+r"(N), "+r"(L), "+r"(NBk));
     const SpecSmem<D> lay;
@@ -873,9 +872,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     int *kacc_s = reinterpret_cast<int *>(sm + lay.kacc);
     double *ctab_s = sm + lay.ctab, *rtab_s = sm + lay.rtab;
 
-    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir], *cc = a.p.cc[dir];
-    double2 *g = a.p.g[dir];
-    double *gs = a.p.gs[dir];
+    const double *rho = rshift(a.p.rho[dir], roff), *sig = rshift(a.p.sig[dir], roff), *cc = rshift(a.p.cc[dir], roff);
+    double2 *g = rshift(a.p.g[dir], roff);
+    double *gs = rshift(a.p.gs[dir], roff);
     const double kk = a.kk;
 
     // ---- pieces of the preparation, written for a group of `nt` threads with index `t`
@@ -993,7 +992,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         return __any_sync(0xffffffffu, live) != 0;
     };
     auto helper_tasks = [&](int K, int hw) {
-        const bool tht = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
+        const bool tht = phase != nullptr && dir == 0 && lane == 0 && hw == 0;
         const long long ht0 = clock64();
         {   // ---- M(K+1): only p <= r is needed, so columns pp and 31-pp share one pass of 32 lanes (33 entries; the
             // odd one, row 31 of column 31-pp, goes to a 17th pass); above the diagonal the tile stays 0 from the start.
@@ -1020,7 +1019,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 if (idx[k] >= 0) {
-                    if constexpr (SGN) { if (idx[k] >= 32) arg[k] *= a.sx; }
+                    if constexpr (SGN) { if (idx[k] >= 32) arg[k] *= sx; }
                     mB[idx[k]] = arg[k];
                 }
             }
@@ -1097,7 +1096,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             for (int k = 0; k < SPEC_NCOL; ++k) {
                 const int p = hw + SPEC_NHW * k;
                 if (p < 32) {
-                    if constexpr (SGN) { if (p >= 1) arg[k] *= a.sx; }
+                    if constexpr (SGN) { if (p >= 1) arg[k] *= sx; }
                     uB[p * 32 + lane] = arg[k];
                 }
             }
@@ -1115,11 +1114,11 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 unsigned long long um, us;
                 int npoll = 0;
                 do { // each lane waits for its own row (k_prep emptied the words, the worker fills them)
-                    um = ld_relaxed_u64(&a.p.pan_m[dir][i]);
-                    us = ld_relaxed_u64(&a.p.pan_s[dir][i]);
+                    um = ld_relaxed_u64(&rshift(a.p.pan_m[dir], roff)[i]);
+                    us = ld_relaxed_u64(&rshift(a.p.pan_s[dir], roff)[i]);
                     ++npoll;
                 } while (um == PAN_EMPTY || us == PAN_EMPTY);
-                if (lane == 0 && a.phase != nullptr && dir == 0) ph_s[10] += npoll; // 1 per block = never waited
+                if (lane == 0 && phase != nullptr && dir == 0) ph_s[10] += npoll; // 1 per block = never waited
                 v = __longlong_as_double((long long)us) * exp_cap_tab64(__longlong_as_double((long long)um) + shift, etab64);
             }
         }
@@ -1150,7 +1149,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     __syncthreads();
     if (warp < SPEC_NHW) helper_tasks(-1, warp);
 
-    int bad = 0;                     // warp 0: status of its rows
+    int bad = 0;                     // warp 0: a row sum of its rows left the acceptance band of the stale gauge
     int kacc = 0;                    // warp 0: power of two taken out of Zhat up to the start of block K
     int kh1 = 0, kh2 = 0, kh3 = 0, kh4 = 0; // warp 0: the same for blocks K-1 .. K-4
     double z0 = 1.0, acc_next = 0.0; // warp 0: Zhat of the block's first column; start value of the next block
@@ -1158,7 +1157,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
     double fin_G = 0.0, fin_acc = 1.0;
     const double2 LN2 = make_double2(0.6931471805599453, 2.3190468138462996e-17);
 
-    const bool tim = a.phase != nullptr && dir == 0 && tid == 0;
+    const bool tim = phase != nullptr && dir == 0 && tid == 0;
     if (tid < 16) ph_s[tid] = 0;
     long long tprev = clock64();
 #define PH(k) do { if (tim) { const long long c__ = clock64(); ph_s[k] += c__ - tprev; tprev = c__; } } while (0)
@@ -1204,8 +1203,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             PH(2);
             // Zhat of the columns this block produced (frame of block K); the next block's frame takes the
             // exponent of its first column out, so that Zhat stays O(1) however far the solution has drifted
-            const double zmine = SGN ? a.sx * acc : acc;
-            const double z32 = SGN ? a.sx * zc : zc;
+            const double zmine = SGN ? sx * acc : acc;
+            const double z32 = SGN ? sx * zc : zc;
             const int ex = (__double2hiint(z32) >> 20) & 0x7ff;
             const int kstep = (ex != 0 && ex != 0x7ff) ? ex - 1023 : 0;
             z0 = z32 * pow2i(-kstep);
@@ -1213,16 +1212,12 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             const int jn = i0 + lane + 1;
             if (jn < N) ring_Z[jn & (RB - 1)] = (lane == 31) ? z0 : zmine;
             if (lane == 0) kacc_s[K & 7] = kacc;
-            if (lane < nrows) {
-                if (acc == 0.0) bad |= ST_NODE;
-                else if (!(fabs(acc) > 1e-270 && fabs(acc) < 1e270)) {
-#ifdef PIMD_DEBUG_GAUGE
-                    if (!(bad & 4) && a.phase) { a.phase[8 + 4 * dir] = i0 + lane; a.phase[9 + 4 * dir] = (unsigned long long)__double_as_longlong(acc);
-                        a.phase[10 + 4 * dir] = (unsigned long long)__double_as_longlong(z0); a.phase[11 + 4 * dir] = (unsigned long long)(long long)kacc; }
-#endif
-                    bad |= 4;
-                }
-            }
+            // Acceptance band of the stale gauge (DESIGN.md 5.1 "error budget"): every row sum, taken in its block's frame,
+            // must lie within 2^+-8 of the gauge (0, NaN and inf fail too; a zero under a stale gauge is a misfit, the
+            // max-plus pass decides whether it is a node).  The helpers drop entries below e^-64 of the row's gauge; with
+            // |Zhat| <= 2^8, frames of the three blocks behind at most 2^24 apart and the row sum itself >= 2^-8 a dropped
+            // entry is below e^-64 2^40 = 1.7e-16 of the row sum.
+            if (lane < nrows && !(fabs(acc) > 0x1p-8 && fabs(acc) < 0x1p8)) bad = 1;
             if (K + 1 == NBk) {
                 fin_T = dd_add_d(dd_add_d(trefn_s[K & 7], (double)kacc * LN2.x), (double)kacc * LN2.y);
                 fin_G = G_s[(K & 7) * 32 + lane];
@@ -1244,9 +1239,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
             }
             if (K > 0) {
                 __syncwarp();
-                if (lane == 0) st_release(&a.p.cols_ready[dir], min(N, i0 + 1));
+                if (lane == 0) st_release(&rshift(a.p.cols_ready, roff)[dir], min(N, i0 + 1));
             }
-            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[7] += clock64() - hcp;
+            if (phase != nullptr && dir == 0 && lane == 0) ph_s[7] += clock64() - hcp;
         } else if (warp == CH_WARPS - 3) {
             // gauges of block K+3 (its raw data arrived during the previous window), then the raw data of block K+4
             const long long hcg = clock64();
@@ -1274,34 +1269,33 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
                 ring_sig[(i & (RB - 1)) * D + c] = pc.v[c];
             }
             cc_s[b3 * 32 + lane] = c0;
-            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[15] += clock64() - hcg;
+            if (phase != nullptr && dir == 0 && lane == 0) ph_s[15] += clock64() - hcg;
         } else if (warp == CH_WARPS - 2) {
             long long hc0 = clock64();
             fetch_panel(K + 1);
-            if (a.phase != nullptr && dir == 0 && lane == 0) ph_s[9] += clock64() - hc0;
+            if (phase != nullptr && dir == 0 && lane == 0) ph_s[9] += clock64() - hc0;
         } else if (SPEC_NHW == 12 || (warp & 3) != 0) {
             // helper warps: with SPEC_NHW = 9 the three that share warp 0's scheduler partition (4, 8, 12) stay idle
             const int hw = (SPEC_NHW == 12) ? warp - 1 : warp - 1 - (warp >> 2);
-            const bool th = a.phase != nullptr && dir == 0 && lane == 0 && hw == 0;
+            const bool th = phase != nullptr && dir == 0 && lane == 0 && hw == 0;
             const long long hc0 = clock64();
             helper_tasks(K, hw);
             if (th) ph_s[8] += clock64() - hc0;
-            if (a.phase != nullptr && dir == 0 && lane == 0 && hw == 4) ph_s[13] += clock64() - hc0;
-            if (a.phase != nullptr && dir == 0 && lane == 0 && hw == 8) ph_s[14] += clock64() - hc0;
+            if (phase != nullptr && dir == 0 && lane == 0 && hw == 4) ph_s[13] += clock64() - hc0;
+            if (phase != nullptr && dir == 0 && lane == 0 && hw == 8) ph_s[14] += clock64() - hc0;
         }
     }
     __syncthreads();
 #undef PH
     if (tim) {
-        for (int k = 0; k < 16; ++k) a.phase[k] += (unsigned long long)ph_s[k];
+        for (int k = 0; k < 16; ++k) phase[k] += (unsigned long long)ph_s[k];
     }
     if (warp == 0) {
         if (lane == (N - 1) % 32) {
-            a.p.rfin[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
-            a.p.rsgn[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
+            rshift(a.p.rfin, roff)[dir] = dd_add_d(dd_add_d(fin_T, fin_G), log(fabs(fin_acc)));
+            rshift(a.p.rsgn, roff)[dir] = (fin_acc < 0.0) ? -1.0 : 1.0;
         }
-        if (bad & 3) atomicOr(a.p.status, bad & 3);
-        if (bad & 4) atomicOr(a.p.status + 2, 1);
+        if (bad) atomicOr(a.gauge_misfit, 1);
     }
     if (warp == CH_WARPS - 1) {
         const int jn = (NBk - 1) * 32 + lane + 1;
@@ -1312,12 +1306,12 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, unsigned char *smem_
         }
         // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
         __syncwarp();
-        if (lane == 0) st_release(&a.p.cols_ready[dir], N);
+        if (lane == 0) st_release(&rshift(a.p.cols_ready, roff)[dir], N);
     }
 }
 
 template <int D, bool SGN>
-__device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char *smem_raw, const double *etab64)
+__device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, unsigned char *smem_raw, const double *etab64)
 {
     const int N = a.N, LOOK = a.look;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -1328,10 +1322,10 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
     double *mg_m = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + CH_WARPS * 32 + CH_WARPS * 32 * D;
     double *mg_s = mg_m + CH_WARPS * 32;
 
-    const double *rho = a.p.rho[dir], *sig = a.p.sig[dir];
-    const double2 *g = a.p.g[dir];
-    const double *gs = a.p.gs[dir];
-    const int *cols_ready = &a.p.cols_ready[dir];
+    const double *rho = rshift(a.p.rho[dir], roff), *sig = rshift(a.p.sig[dir], roff);
+    const double2 *g = rshift(a.p.g[dir], roff);
+    const double *gs = rshift(a.p.gs[dir], roff);
+    const int *cols_ready = &rshift(a.p.cols_ready, roff)[dir];
     const double kk = a.kk;
     int known_ready = 0;
 
@@ -1477,12 +1471,12 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, unsigned char 
                 for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_neg_tab64(-(mg_m[w * 32 + lane] - t.m), etab64), t.s);
             }
             if (i < N) {
-                st_relaxed_f64(&a.p.pan_m[dir][i], t.m);
-                st_relaxed_f64(&a.p.pan_s[dir][i], t.s);
+                st_relaxed_f64(&rshift(a.p.pan_m[dir], roff)[i], t.m);
+                st_relaxed_f64(&rshift(a.p.pan_s[dir], roff)[i], t.s);
             }
             // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
             __syncwarp();
-            if (lane == 0) st_release(&a.p.panel_ready[dir][K], 1);
+            if (lane == 0) st_release(&rshift(a.p.panel_ready[dir], roff)[K], 1);
         }
         __syncthreads();
     }
@@ -1497,8 +1491,9 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int dir = blockIdx.y;
-    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, smem_raw, etab);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
+    const size_t roff = (size_t)blockIdx.z * a.rs; // replica of a batch
+    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, roff, smem_raw, etab);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
 }
 
 // the recursion with the previous evaluation's gauge (see chain_cta_spec); same grid, same workers
@@ -1511,26 +1506,30 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
     if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
     __syncthreads();
     const int dir = blockIdx.y;
-    if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, smem_raw, etab64);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, smem_raw, etab64);
+    const size_t roff = (size_t)blockIdx.z * a.rs;
+    if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, roff, smem_raw, etab64);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
     // Safety net in the same launch (a second, conditional cooperative launch cost 7 us per evaluation): if a row sum
-    // left the range the stale gauge covers, every CTA sees status[2] after the grid barrier and the whole grid redoes
-    // the recursion with a fresh max-plus gauge (chain_cta), which overwrites everything this pass published.
+    // left the band the stale gauge covers (in any replica of the batch), every CTA sees the misfit flag after the grid
+    // barrier and the whole grid redoes the recursion with a fresh max-plus gauge (chain_cta), which overwrites everything
+    // this pass published.
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     __threadfence();
     grid.sync();
-    if (ld_acquire(a.p.status + 2) == 0) return; // the same answer in every CTA
+    if (ld_acquire(a.gauge_misfit) == 0) return; // the same answer in every CTA
     if (blockIdx.x == 0 && blockIdx.y == 0) {
-        for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { a.p.panel_ready[0][k] = 0; a.p.panel_ready[1][k] = 0; }
-        if (threadIdx.x < 2) a.p.cols_ready[threadIdx.x] = 1;
+        int *pr0 = rshift(a.p.panel_ready[0], roff), *pr1 = rshift(a.p.panel_ready[1], roff);
+        for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { pr0[k] = 0; pr1[k] = 0; }
+        if (threadIdx.x < 2) rshift(a.p.cols_ready, roff)[threadIdx.x] = 1;
+        if (threadIdx.x == 0 && blockIdx.z == 0) atomicAdd(a.fallbacks, 1ull);
     }
     __threadfence();
     grid.sync();
     ChainArgs b = a;
     b.look = a.look_fb;
     b.phase = nullptr;
-    if (blockIdx.x == 0) chain_cta<D, SGN>(b, dir, smem_raw, etab);
-    else worker_cta<D, SGN>(b, dir, blockIdx.x - 1, smem_raw, etab64);
+    if (blockIdx.x == 0) chain_cta<D, SGN>(b, dir, roff, smem_raw, etab);
+    else worker_cta<D, SGN>(b, dir, blockIdx.x - 1, roff, smem_raw, etab64);
 }
 
 template <int D> size_t chain_spec_smem_bytes_host()
@@ -1548,12 +1547,12 @@ template <int D> size_t chain_spec_smem_bytes_host()
 //   w_ij = exp( g^{other}[N-1-i] + g^{dir}[j] - kk |rho_i - sig_j|^2 - R_N ),  j <= i
 //   acc[dir][i] = ( sum_j w, sum_j w sig_j, sum_j w kk r^2 )
 // dir 0 gives the row sums (bead P, Eq. 16), dir 1 the column sums (bead 1, Eq. 15).
-// grid (NT, NT, 2) over 128 x 128 tiles of the lower triangle; block 128.
+// grid (NT, NT, 2 B) over 128 x 128 tiles of the lower triangle; block 128.
 // ==========================================================================================
 constexpr int FP_TB = 128;
 
 template <int D, bool SGN, int NQ>
-__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p)
+__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, size_t rs)
 {
     // a CTA of FP_TB threads takes RT rows x FP_TB columns at or below the diagonal.  NQ = 1: RT = FP_TB, one thread per
     // row walks the tile's columns (large N: enough tiles to fill the GPU).  NQ = 4: RT = 32, four threads per row with 32
@@ -1561,9 +1560,10 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
     // the SMs with a warp or two each and the kernel latency bound; four times as many, smaller CTAs also spread evenly
     // over the SMs).
     constexpr int CW = FP_TB / NQ, RT = FP_TB / NQ;
-    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z;
+    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z & 1; // grid.z = 2 * replica + direction
     const int j0 = ct * FP_TB;
     if (j0 > rt * RT + RT - 1) return; // above the diagonal
+    p = rshift(p, (size_t)(blockIdx.z >> 1) * rs);
     // one thread per row (large N): 256-entry table, 8 FP64 instructions per exponential (N=10000 0.202 -> 0.195 ms);
     // four threads per row (small N, many small CTAs): the 64-entry table, whose fill per CTA is four times cheaper
     // (cfg3 0.0170 against 0.0173 ms with the large table)
@@ -1656,10 +1656,13 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 // One thread per particle.  ecpart: per-block partial sums of sum_{l'} Pr[l->l'] beta C(l,l').
 // ==========================================================================================
 template <int D, bool SGN, int TB>
-__global__ void __launch_bounds__(TB) k_assemble(int N, double ks, double xi, ExchPtrs p, double *Fex1, double *FexP,
-                                                double *ecpart)
+__global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, const RepParams *rp, double *Fex1, double *FexP,
+                                                double *ecpart, size_t rs)
 {
     __shared__ double red[TB / 32];
+    const size_t off = (size_t)blockIdx.y * rs;
+    p = rshift(p, off); Fex1 = rshift(Fex1, off); FexP = rshift(FexP, off); ecpart = rshift(ecpart, off);
+    const double xi = rshift(rp, off)->xi;
     const int l = blockIdx.x * TB + threadIdx.x;
     double ec = 0.0;
     if (l < N) {
@@ -1819,9 +1822,11 @@ __global__ void __launch_bounds__(256, PRMAT_MINB) k_prmat(int N, double kk, Exc
 // xi = 0 (0^0 = 1): only k = 1 survives in Eq. 6, Pr is the identity, every ring closes
 // on itself.  V = sum_l E^{[l,l]} + (1/beta) ln N!.
 template <int D, int TB>
-__global__ void __launch_bounds__(TB) k_exch_xi0(int N, double ks, ExchPtrs p, double *Fex1, double *FexP, double *ecpart)
+__global__ void __launch_bounds__(TB) k_exch_xi0(int N, double ks, ExchPtrs p, double *Fex1, double *FexP, double *ecpart, size_t rs)
 {
     __shared__ double red[TB / 32];
+    const size_t off = (size_t)blockIdx.y * rs;
+    p = rshift(p, off); Fex1 = rshift(Fex1, off); FexP = rshift(FexP, off); ecpart = rshift(ecpart, off);
     const int l = blockIdx.x * TB + threadIdx.x;
     double ec = 0.0;
     if (l < N) {
@@ -1850,10 +1855,13 @@ struct Scalars {
 };
 
 template <int TB>
-__global__ void __launch_bounds__(TB) k_finalize(int N, int nprep, int nasm, double beta, double lambda, double xi,
-                                                double lgammaN1, ExchPtrs p, const double *ecpart, Scalars *out)
+__global__ void __launch_bounds__(TB) k_finalize(int N, int nprep, int nasm, double beta, const RepParams *rp,
+                                                double lgammaN1, ExchPtrs p, const double *ecpart, Scalars *out, size_t rs)
 {
     __shared__ double red[TB / 32];
+    const size_t off = (size_t)blockIdx.x * rs; // one block per replica
+    p = rshift(p, off); ecpart = rshift(ecpart, off); out = rshift(out, off);
+    const double lambda = rshift(rp, off)->lambda, xi = rshift(rp, off)->xi;
     double a = 0.0, b = 0.0, c = 0.0;
     for (int i = threadIdx.x; i < nprep; i += TB) { a += p.tpart[2 * i]; b += p.tpart[2 * i + 1]; }
     for (int i = threadIdx.x; i < nasm; i += TB) c += ecpart[i];
@@ -1906,26 +1914,34 @@ PIMD_DEV void nhc_half(double &vi, double *vx, double h, double kT, double Q)
     vx[M - 1] += 0.5 * h * G;
 }
 
+// Bead shards: P = local slices; own_first / own_last say whether local slice 0 / P-1 is the ring's bead 1 /
+// bead P (only those take the exterior exchange forces); dof0 = global index of local degree of freedom 0, so that the
+// noise of a degree of freedom does not depend on how the beads are sharded.  grid (ceil(ndof/256), B).
 template <int THERMO>
 __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, double *__restrict__ v, const double *__restrict__ F,
                                                   const double *__restrict__ Fex1, const double *__restrict__ FexP,
                                                   double *__restrict__ nhc, size_t ndof, size_t slice /* N*d */, int P,
-                                                  double dt, double c1, double c2, double beta, double Q, uint64_t seed,
+                                                  double dt, double c1, double c2, double beta, double Q, const RepParams *rp,
                                                   uint64_t step_close, uint64_t step_open, int do_close, int do_open,
-                                                  int *status, const unsigned long long *dstep)
+                                                  int *istatus, const unsigned long long *dstep, int own_first, int own_last,
+                                                  size_t dof0, size_t rs)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= ndof) return;
+    const size_t off = (size_t)blockIdx.y * rs;
+    x = rshift(x, off); v = rshift(v, off); F = rshift(F, off); Fex1 = rshift(Fex1, off); FexP = rshift(FexP, off);
+    [[maybe_unused]] const uint64_t seed = rshift(rp, off)->seed;
     // step counter kept on the device when launches are replayed from a CUDA graph (no per-step arguments there)
     [[maybe_unused]] const uint64_t s_close = dstep ? *dstep : step_close;
     [[maybe_unused]] const uint64_t s_open = dstep ? *dstep + (do_close ? 1 : 0) : step_open;
     const size_t j = idx / slice, rem = idx - j * slice;
     double f = F[idx];
-    if (j == 0) f += Fex1[rem];
-    if (j == (size_t)(P - 1)) f += FexP[rem];
+    if (j == 0 && own_first) f += Fex1[rem];
+    if (j == (size_t)(P - 1) && own_last) f += FexP[rem];
     double vi = v[idx];
     double vx[4];
     if constexpr (THERMO == 2) {
+        nhc = rshift(nhc, off);
 #pragma unroll
         for (int k = 0; k < 4; ++k) vx[k] = nhc[(size_t)k * ndof + idx];
     }
@@ -1934,7 +1950,7 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
         vi = fma(hdt, f, vi);
         if constexpr (THERMO == 1) {
             double z0, z1;
-            philox_normal(seed, idx, s_close, z0, z1);
+            philox_normal(seed, dof0 + idx, s_close, z0, z1);
             vi = c1 * vi + c2 * z1;
         } else if constexpr (THERMO == 2) {
             nhc_half(vi, vx, hdt, 1.0 / beta, Q);
@@ -1943,7 +1959,7 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
     if (do_open) {
         if constexpr (THERMO == 1) {
             double z0, z1;
-            philox_normal(seed, idx, s_open, z0, z1);
+            philox_normal(seed, dof0 + idx, s_open, z0, z1);
             vi = c1 * vi + c2 * z0;
         } else if constexpr (THERMO == 2) {
             nhc_half(vi, vx, hdt, 1.0 / beta, Q);
@@ -1951,7 +1967,7 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
         vi = fma(hdt, f, vi);
         const double xn = fma(dt, vi, x[idx]);
         x[idx] = xn;
-        if (!(fabs(xn) < INFINITY)) atomicOr(status + 1, ST_NONFINITE);
+        if (!(fabs(xn) < INFINITY)) atomicOr(rshift(istatus, off), ST_NONFINITE);
     }
     v[idx] = vi;
     if constexpr (THERMO == 2) {
@@ -1962,15 +1978,17 @@ __global__ void __launch_bounds__(256) k_integrate(double *__restrict__ x, doubl
 
 __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const double *__restrict__ F,
                                                 const double *__restrict__ Fex1, const double *__restrict__ FexP, size_t ndof,
-                                                size_t slice, int P)
+                                                size_t slice, int P, int own_first, int own_last, size_t rs)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= ndof) return;
+    const size_t off = (size_t)blockIdx.y * rs;
+    F = rshift(F, off); Fex1 = rshift(Fex1, off); FexP = rshift(FexP, off);
     const size_t j = idx / slice, rem = idx - j * slice;
     double f = F[idx];
-    if (j == 0) f += Fex1[rem];
-    if (j == (size_t)(P - 1)) f += FexP[rem];
-    out[idx] = f;
+    if (j == 0 && own_first) f += Fex1[rem];
+    if (j == (size_t)(P - 1) && own_last) f += FexP[rem];
+    out[(size_t)blockIdx.y * ndof + idx] = f; // out: [B][P][N][d], contiguous
 }
 
 // ==========================================================================================
@@ -1988,12 +2006,32 @@ __global__ void __launch_bounds__(256) k_combine(double *__restrict__ out, const
 // The Gaussian is exp_neg_tab256 (8 FP64 instructions; the 64-entry form with one more FMA measured 0.0811 against
 // 0.0783 ms at cfg3).  Coordinates are pre-scaled by 1/s so that the exponent is -|dx'|^2; padding particles sit at
 // +-1e150 and give e^-708 ~ 3e-308 (their forces are never written).
-// grid (ceil(tasks/PAIR_WARPS), P), block PAIR_WARPS * 32; tasks = NT (nchunk + 1).
+// grid (ceil(tasks/PAIR_WARPS), P, B), block PAIR_WARPS * 32; tasks = NT (nchunk + 1).
 // ==========================================================================================
 constexpr int PAIR_WARPS = 8;
-constexpr int PAIR_CH = 8;
 
-template <int D, bool EST>
+// The pair potential v(r) of Eq. 18 (PAPER.md:142-144: "V" is generic; Eq. 20, :193, is the Gaussian instance) as a
+// compile-time choice.  With r2 = |dx|^2 / s^2 (coordinates pre-scaled by 1/s) a potential gives
+//   w  : force weight, F_i += coef * w * dx',  F_j -= the same     (coef carries the potential's constant factors)
+//   u  : v(r) in units of the energy prefactor gE,   du : (v + r v'/2)(r) - v(r) in the same units (virial estimator)
+//   POT 0  Gaussian       v = g exp(-r^2/s^2)      : w = u = e^{-r2},        du = -r2 e^{-r2};   coef = 2 g/(s P), gE = g
+//   POT 1  soft Coulomb   v = g / sqrt(r^2 + s^2)  : w = (1+r2)^{-3/2}, u = (1+r2)^{-1/2}, du = -r2 w/2; coef = g/(s^2 P), gE = g/s
+// Both are smooth at r = 0 with u(0) = 1, du(0) = 0 (the diagonal tile removes the self term analytically).
+template <int POT> PIMD_DEV void pair_weight(double r2, const double *tab, double &w, double &u, double &du)
+{
+    if constexpr (POT == 0) {
+        w = exp_neg_tab256(r2, tab);
+        u = w;
+        du = -w * fmin(r2, 708.0); // padding pairs have r2 ~ 1e300 and e = e^-708, not 0
+    } else {
+        const double rs = rsqrt(1.0 + r2);
+        w = rs * rs * rs;
+        u = rs;
+        du = -0.5 * fmin(r2, 1e100) * w; // padding pairs: w = 0
+    }
+}
+
+template <int D, bool EST, int POT>
 PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, Vec<D> &fi, Vec<D> &fj, double &se, double &sea)
 {
     Vec<D> dl;
@@ -2002,28 +2040,30 @@ PIMD_DEV void pair_term(const Vec<D> &ri, const double *sj, const double *tab, V
     double r2 = dl.v[0] * dl.v[0];
 #pragma unroll
     for (int c = 1; c < D; ++c) r2 = fma(dl.v[c], dl.v[c], r2);
-    const double e = exp_neg_tab256(r2, tab);
+    double e, u, du;
+    if constexpr (POT == 0 && !EST) e = exp_neg_tab256(r2, tab);
+    else pair_weight<POT>(r2, tab, e, u, du);
 #pragma unroll
     for (int c = 0; c < D; ++c) {
         fi.v[c] = fma(e, dl.v[c], fi.v[c]);
         fj.v[c] = fma(-e, dl.v[c], fj.v[c]);
     }
     if constexpr (EST) {
-        se += e;
-        sea = fma(-e, fmin(r2, 708.0), sea); // padding pairs have r2 ~ 1e300 and e = e^-708, not 0
+        se += u;
+        sea += du;
     }
 }
 
 // 32 steps of lane t against NJ column tiles held twice over in shared memory (tl = tile + t*D, so
 // that column (t + k) mod 32 is at the compile-time offset k*D); the column accumulators rotate.
-template <int D, int NJ, bool EST>
+template <int D, int NJ, bool EST, int POT>
 PIMD_DEV void pair_sweep(const Vec<D> &ri, const double *tlA, const double *tlB, const double *tab, Vec<D> &fi, Vec<D> &fA,
                          Vec<D> &fB, double &se, double &sea, int nxt)
 {
 #pragma unroll
     for (int k = 0; k < 32; ++k) {
-        pair_term<D, EST>(ri, tlA + k * D, tab, fi, fA, se, sea);
-        if constexpr (NJ == 2) pair_term<D, EST>(ri, tlB + k * D, tab, fi, fB, se, sea);
+        pair_term<D, EST, POT>(ri, tlA + k * D, tab, fi, fA, se, sea);
+        if constexpr (NJ == 2) pair_term<D, EST, POT>(ri, tlB + k * D, tab, fi, fB, se, sea);
         if (k < 31) {
 #pragma unroll
             for (int q = 0; q < D; ++q) {
@@ -2034,11 +2074,13 @@ PIMD_DEV void pair_sweep(const Vec<D> &ri, const double *tlA, const double *tlB,
     }
 }
 
-template <int D, bool EST>
+template <int D, bool EST, int POT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restrict__ x, double *__restrict__ F, int N, int NT,
                                                          int nchunk, int ch, double inv_s, double coef /* 2 g / (s P) */,
-                                                         double g, EstAccum *est)
+                                                         double g, EstAccum *est, size_t rs)
 {
+    x = rshift(x, (size_t)blockIdx.z * rs); F = rshift(F, (size_t)blockIdx.z * rs);
+    if constexpr (EST) est = rshift(est, (size_t)blockIdx.z * rs);
     __shared__ double tiles[PAIR_WARPS][2][64 * D];
     __shared__ double tab[256];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -2095,7 +2137,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
 #pragma unroll
         for (int k = 0; k < D; ++k) dummy.v[k] = 0.0;
 #pragma unroll 8
-        for (int k = 0; k < 32; ++k) pair_term<D, EST>(ri, tlA + k * D, tab, fi, dummy, se, sea);
+        for (int k = 0; k < 32; ++k) pair_term<D, EST, POT>(ri, tlA + k * D, tab, fi, dummy, se, sea);
         if constexpr (EST) {
             se = vi ? 0.5 * (se - 1.0) : 0.0;
             sea = vi ? 0.5 * sea : 0.0;
@@ -2115,7 +2157,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
             Vec<D> fA, fB;
 #pragma unroll
             for (int k = 0; k < D; ++k) { fA.v[k] = 0.0; fB.v[k] = 0.0; }
-            pair_sweep<D, 2, EST>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
+            pair_sweep<D, 2, EST, POT>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
             flush(JA, lastcol, fA);
             flush(JB, lastcol, fB);
         }
@@ -2128,7 +2170,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
             Vec<D> fA, fB;
 #pragma unroll
             for (int k = 0; k < D; ++k) { fA.v[k] = 0.0; fB.v[k] = 0.0; }
-            pair_sweep<D, 1, EST>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
+            pair_sweep<D, 1, EST, POT>(ri, tlA, tlB, tab, fi, fA, fB, se, sea, nxt);
             flush(JA, lastcol, fA);
         }
     }
@@ -2146,6 +2188,136 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
     }
 }
 
+// ==========================================================================================
+// Step 8: the estimators of one configuration from the sums the force kernels left behind (R9)
+//   e_prim = P d N/(2 beta) - <E_c> + Ubar,  e_vir = Ubar + 1/2 sum r . grad Ubar,  Ubar = U/P
+// and, when `accumulate` is set (pimd_run), their running sums and the running histograms.  One block per replica.
+// Bead shards: `kin` and <E_c> are counted on rank 0 only, Ubar over the local slices, so the ranks' values add up.
+// ==========================================================================================
+struct EstSums {
+    double n, sum_ep, sum_ev, last_ep, last_ev, pad[3];
+};
+
+__global__ void __launch_bounds__(256) k_estimate(int nspecies, const Scalars *scal, const EstAccum *est, EstSums *sums,
+                                                 const double *hist, double *hist_acc, int nbins, const double *gr,
+                                                 double *gr_acc, int nbins_gr, double kin, double ec_weight, double invP,
+                                                 int accumulate, size_t rs)
+{
+    const size_t off = (size_t)blockIdx.x * rs;
+    scal = rshift(scal, off); est = rshift(est, off); sums = rshift(sums, off);
+    if (threadIdx.x == 0) {
+        double ec = 0.0;
+        for (int s = 0; s < nspecies; ++s) ec += scal[s].ec;
+        const double ubar = est->utrap + est->upair * invP; // the trap term is accumulated already divided by P
+        const double ep = ec_weight * (kin - ec) + ubar;
+        const double ev = 2.0 * est->utrap + est->virpair * invP;
+        sums->last_ep = ep;
+        sums->last_ev = ev;
+        if (accumulate) { sums->n += 1.0; sums->sum_ep += ep; sums->sum_ev += ev; }
+    }
+    if (accumulate) {
+        hist = rshift(hist, off); hist_acc = rshift(hist_acc, off); gr = rshift(gr, off); gr_acc = rshift(gr_acc, off);
+        for (int b = threadIdx.x; b < nbins; b += blockDim.x) hist_acc[b] += hist[b];
+        for (int b = threadIdx.x; b < nbins_gr; b += blockDim.x) gr_acc[b] += gr[b];
+    }
+}
+
+// ==========================================================================================
+// Pair-distance histogram (pair-correlation estimator): counts of |r_l^j - r_i^j|, i < l, same bead
+// index j (the pairs Eq. 18, couples), in nbins equal bins on [0, rmax); raw counts, normalisation by the
+// caller.  Estimator steps only.  The distance is formed with separately rounded multiplies and adds (no FMA
+// contraction), the order a plain C loop takes, so that the bin decision is the oracle's to the bit.
+// grid (ceil(N/GR_TB), P, B), block GR_TB: thread = particle l, tiles of GR_TB partners through shared memory.
+// ==========================================================================================
+constexpr int GR_TB = 128;
+constexpr int GR_MAXBINS = 4096;
+
+template <int D>
+__global__ void __launch_bounds__(GR_TB) k_gr(const double *__restrict__ x, int N, double *hist, int nbins, double rmax, size_t rs)
+{
+    __shared__ double tile[GR_TB * D];
+    __shared__ unsigned int cnt[GR_MAXBINS];
+    x = rshift(x, (size_t)blockIdx.z * rs); hist = rshift(hist, (size_t)blockIdx.z * rs);
+    const double *xs = x + (size_t)blockIdx.y * N * D;
+    for (int b = threadIdx.x; b < nbins; b += GR_TB) cnt[b] = 0u;
+    const int l = blockIdx.x * GR_TB + threadIdx.x;
+    Vec<D> r;
+#pragma unroll
+    for (int c = 0; c < D; ++c) r.v[c] = 0.0;
+    if (l < N) r = ldvec<D>(xs, l);
+    const int lmax = min(N, (blockIdx.x + 1) * GR_TB); // partners i < l only
+    for (int t0 = 0; t0 < lmax; t0 += GR_TB) {
+        __syncthreads();
+        if (t0 + threadIdx.x < N) {
+            const Vec<D> q = ldvec<D>(xs, t0 + threadIdx.x);
+#pragma unroll
+            for (int c = 0; c < D; ++c) tile[threadIdx.x * D + c] = q.v[c];
+        }
+        __syncthreads();
+        const int kend = min(GR_TB, l - t0);
+        for (int k = 0; k < kend; ++k) {
+            double r2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < D; ++c) {
+                const double t = __dsub_rn(r.v[c], tile[k * D + c]);
+                r2 = __dadd_rn(r2, __dmul_rn(t, t));
+            }
+            const double rr = sqrt(r2);
+            if (l < N && rr < rmax) {
+                int b = (int)(__dmul_rn(__ddiv_rn(rr, rmax), (double)nbins));
+                if (b >= nbins) b = nbins - 1;
+                atomicAdd(&cnt[b], 1u);
+            }
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += GR_TB)
+        if (cnt[b]) atomicAdd(&hist[b], (double)cnt[b]);
+}
+
+// ==========================================================================================
+// Bead shards ("parallel computing ... with a large number of ... GPUs"; the
+// per-slice pair term parallelises like classical MD).  A rank holds the contiguous slices [j0, j0 + Pl) of every ring.
+// What leaves a rank per MD step is its boundary pack
+//     [ first local slice : N d ][ last local slice : N d ][ partial E_int : N ]      (2 N d + N doubles)
+// (partial E_int = the springs between two local slices, Eq. 9); the all-gather of the packs gives every rank the halo
+// slices of its ring neighbours, bead 1 (first slice of rank 0), bead P (last slice of the last rank) and, with the springs
+// that cross a rank boundary added, E_int -- everything the exchange part (steps 3-6, run redundantly on every rank)
+// and the local spring forces need.
+// ==========================================================================================
+template <int D>
+__global__ void __launch_bounds__(128) k_shard_pack(const double *__restrict__ x, int N, int Pl, double ks, double *__restrict__ pack)
+{
+    const int l = blockIdx.x * 128 + threadIdx.x;
+    if (l >= N) return;
+    const size_t sl = (size_t)N * D;
+    Vec<D> prev = ldvec<D>(x, l);
+    stvec<D>(pack, l, prev);
+    double acc = 0.0;
+    for (int j = 1; j < Pl; ++j) {
+        const Vec<D> cur = ldvec<D>(x + (size_t)j * sl, l);
+        acc += dist2<D>(cur, prev);
+        prev = cur;
+    }
+    stvec<D>(pack + sl, l, prev);
+    pack[2 * sl + l] = 0.5 * ks * acc;
+}
+
+template <int D>
+__global__ void __launch_bounds__(128) k_shard_eint(const double *__restrict__ gathered, int N, int world, double ks,
+                                                   double *__restrict__ eint)
+{
+    const int l = blockIdx.x * 128 + threadIdx.x;
+    if (l >= N) return;
+    const size_t sl = (size_t)N * D, stride = 2 * sl + N;
+    double e = 0.0, cross = 0.0;
+    for (int r = 0; r < world; ++r) {
+        e += gathered[r * stride + 2 * sl + l];
+        if (r + 1 < world) cross += dist2<D>(ldvec<D>(gathered + (r + 1) * stride, l), ldvec<D>(gathered + r * stride + sl, l));
+    }
+    eint[l] = e + 0.5 * ks * cross;
+}
+
 // Pr of distinguishable particles (xi = 0): the identity
 __global__ void __launch_bounds__(256) k_identity(int N, double *__restrict__ Pr)
 {
@@ -2160,12 +2332,6 @@ __global__ void __launch_bounds__(256) k_identity(int N, double *__restrict__ Pr
 __global__ void k_step_counter(unsigned long long *dstep, unsigned long long set, int add)
 {
     if (threadIdx.x == 0 && blockIdx.x == 0) *dstep = add ? *dstep + 1 : set;
-}
-
-__global__ void k_zero(double *p, size_t n)
-{
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) p[i] = 0.0;
 }
 
 // the device exponentials evaluated element-wise (parity tests): which = 0 exp_fast(x), 1 exp_tab(x),

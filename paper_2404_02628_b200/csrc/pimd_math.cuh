@@ -266,30 +266,6 @@ struct Lse {
     double m, s;
 };
 PIMD_DEV Lse lse_empty() { return Lse{-INFINITY, 0.0}; }
-PIMD_DEV void lse_add(Lse &a, double t, double sg)
-{
-    double dlt = t - a.m;             // +inf when the accumulator is empty
-    double e = exp_fast(-fabs(dlt));  // exp(-inf) = 0
-    if (dlt > 0.0) {
-        a.s = fma(a.s, e, sg);
-        a.m = t;
-    } else {
-        a.s = fma(sg, e, a.s);
-    }
-}
-PIMD_DEV void lse_merge(Lse &a, const Lse &b)
-{
-    if (b.m == -INFINITY) return;
-    if (a.m == -INFINITY) { a = b; return; }
-    double dlt = b.m - a.m;
-    double e = exp_fast(-fabs(dlt));
-    if (dlt > 0.0) {
-        a.s = fma(a.s, e, b.s);
-        a.m = b.m;
-    } else {
-        a.s = fma(b.s, e, a.s);
-    }
-}
 PIMD_DEV void lse_shift(Lse &a, double delta) // re-reference: all t_i -> t_i + delta
 {
     if (a.m != -INFINITY) a.m += delta;

@@ -1,0 +1,190 @@
+"""Parity of the kernels bench.py actually times -- the recursion with the previous evaluation's gauge (k_chain_spec),
+in the default launch configuration (look-ahead, workers, two streams, graph replay) -- with the CPU oracle AT THE TIMED
+SIZES: BASELINE configs 3, 4, 5 (N = 2500 .. 40000) and 5b.  Needs a B200.
+
+Every case evaluates on ONE handle: first evaluation = fresh max-plus gauge (k_chain), second evaluation at the same
+positions = stale gauge (k_chain_spec), then pimd_step(3) (graph replay + stale gauge) and a further evaluation at the
+positions reached.  pimd_get_diagnostics must report no fallback, i.e. the stale-gauge kernel's own result is what is
+compared.  Tolerance 1e-9 relative on V_B and per bead class (north_star); xi < 0: 1e-9 * kappa (R7)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from paper_2404_02628_b200 import workloads as wl  # noqa: E402
+
+RTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def binding():
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked tests need the B200 box")
+    from paper_2404_02628_b200 import binding as b
+
+    b.load()
+    return b
+
+
+def relerr(a, b):
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+def check_forces(F, Fo, tol):
+    P = F.shape[0]
+    assert relerr(F, Fo) <= tol
+    assert relerr(F[0], Fo[0]) <= tol
+    assert relerr(F[P - 1], Fo[P - 1]) <= tol
+    if P > 2:
+        assert relerr(F[1:P - 1], Fo[1:P - 1]) <= tol
+
+
+def make(binding, w, thermostat=0, seed=0):
+    return binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=thermostat, seed=seed)
+
+
+CASES = [("cfg3", s) for s in (0, 1, 2)] + [("cfg4", s) for s in (0, 1, 2)] + [("cfg5_N2500", s) for s in (0, 1, 2)] + \
+        [("cfg5_N10000", 0)]
+
+
+@pytest.mark.parametrize("name,seed", CASES, ids=["%s-seed%d" % c for c in CASES])
+def test_stale_gauge_kernel_matches_oracle_at_timed_sizes(binding, oracle, name, seed):
+    w = wl.WORKLOADS[name]
+    x, v = wl.make_state(w, seed)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    tol = RTOL if w.xi >= 0 else RTOL * oracle.conditioning(x, w.beta, w.xi)
+    Fo, vbo, sgo = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
+    for _ in range(2):          # fresh gauge, then the previous evaluation's
+        F, vb, sg = sim.forces()
+        assert sg == sgo
+        assert abs(vb - vbo) <= tol * abs(vbo)
+        check_forces(F.cpu().numpy(), Fo, tol)
+    sim.step(3)
+    xg, _ = sim.get_state()
+    xs = xg.cpu().numpy()
+    F, vb, sg = sim.forces()
+    diag = sim.get_diagnostics()
+    sim.close()
+    assert diag["fallbacks"] == 0 and diag["status_seen"] == 0
+    tol = RTOL if w.xi >= 0 else RTOL * oracle.conditioning(xs, w.beta, w.xi)
+    Fo, vbo, sgo = oracle.forces(xs, w.beta, w.omega, w.g, w.s, w.xi)
+    assert sg == sgo
+    assert abs(vb - vbo) <= tol * abs(vbo)
+    check_forces(F.cpu().numpy(), Fo, tol)
+
+
+def test_cfg5b_every_force_after_steps(binding, oracle):
+    """N = 10000 with the pair interaction on: every force component, pair part included, against
+    the oracle at the positions three MD steps on (stale-gauge recursion, NB/8 workers beside the pair kernel)."""
+    w = wl.WORKLOADS["cfg5b"]
+    x, v = wl.make_state(w, 0)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    sim.step(3)
+    xs = sim.get_state()[0].cpu().numpy()
+    F, vb, sg = sim.forces()
+    diag = sim.get_diagnostics()
+    sim.close()
+    assert diag["fallbacks"] == 0
+    Fo, vbo, sgo = oracle.forces(xs, w.beta, w.omega, w.g, w.s, w.xi)
+    assert sg == sgo == 1 and abs(vb - vbo) <= RTOL * abs(vbo)
+    check_forces(F.cpu().numpy(), Fo, RTOL)
+
+
+@pytest.mark.parametrize("name", ["cfg5_N20000", "cfg5_N40000"])
+def test_largest_sizes_against_streamed_oracle(binding, oracle, name):
+    """N = 20000 and 40000: EVERY entry of the forward (Eq. 6) and backward (Eq. 11) tables and the force on every bead of
+    sampled particles (Eq. 12-17) against the oracle's O(N)-memory evaluation, at the positions three MD steps on (the
+    stale-gauge kernel with the co-residency cap on its workers at N = 40000)."""
+    w = wl.WORKLOADS[name]
+    x, v = wl.make_state(w, 0)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    sim.step(3)
+    xs = sim.get_state()[0].cpu().numpy()
+    F, vb, sg = sim.forces()
+    vf, vbw, pn = sim.get_tables()
+    diag = sim.get_diagnostics()
+    sim.close()
+    assert diag["fallbacks"] == 0
+    rng = np.random.default_rng(1)
+    sel = np.unique(np.concatenate([[0, 1, 31, 32, 33, w.N - 2, w.N - 1], rng.integers(0, w.N, 57)])).astype(np.int32)
+    Fs, vbo, sgo, fwd, bwd = oracle.stream_forces_on(xs, w.beta, w.omega, w.g, w.s, w.xi, sel, tables=True)
+    assert sg == sgo == 1 and abs(vb - vbo) <= RTOL * abs(vbo)
+    # the tables grow like n * (spring energy per particle): relative to the table's own size, entry by entry
+    np.testing.assert_allclose(vf, fwd, rtol=RTOL, atol=1e-9)
+    np.testing.assert_allclose(vbw[1:w.N + 2], bwd[1:w.N + 2], rtol=RTOL, atol=1e-9)
+    Fg = F.cpu().numpy()[:, sel, :].transpose(1, 0, 2)          # [k][P][d]
+    scale = float(np.max(np.abs(Fg)))
+    P = w.P
+    assert np.max(np.abs(Fg - Fs)) <= RTOL * scale
+    assert np.max(np.abs(Fg[:, 0] - Fs[:, 0])) <= RTOL * float(np.max(np.abs(Fs[:, 0])))
+    assert np.max(np.abs(Fg[:, P - 1] - Fs[:, P - 1])) <= RTOL * float(np.max(np.abs(Fs[:, P - 1])))
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg3"])
+def test_ten_nve_steps_match_oracle_at_config_sizes(binding, oracle, name):
+    """SURVEY 8(d) parity protocol: 10 pimd_steps in NVE mode against orc_step, positions to 1e-9."""
+    w = wl.WORKLOADS[name]
+    x, v = wl.make_state(w, 0)
+    xo, vo = x.copy(), v.copy()
+    Fo, _, _ = oracle.forces(xo, w.beta, w.omega, w.g, w.s, w.xi)
+    oracle.step(xo, vo, Fo, None, w.beta, w.omega, w.g, w.s, w.xi, w.dt, 0, 1.0, 0, 0, 10)
+    sim = make(binding, w, thermostat=0)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    sim.step(10)
+    xg, vg = sim.get_state()
+    sim.close()
+    assert relerr(xg.cpu().numpy(), xo) <= 1e-9
+    assert relerr(vg.cpu().numpy(), vo) <= 1e-8
+
+
+def test_identical_rings_closed_form_with_stale_gauge_n40000(binding):
+    """N = 40000 identical rings (closed form for W_N, any xi): second evaluation on the handle = stale-gauge kernel."""
+    N, P, d, beta, xi = 40000, 16, 2, 3.0, 1.0
+    ring = np.random.default_rng(5).normal(0.0, 0.3, size=(P, 1, d))
+    x = np.ascontiguousarray(np.repeat(ring, N, axis=1))
+    ks = P / beta ** 2
+    diffs = np.diff(np.concatenate([ring[:, 0, :], ring[:1, 0, :]]), axis=0)
+    e_ring = 0.5 * ks * float(np.sum(diffs ** 2))
+    j = np.arange(N, dtype=np.float64)
+    vb_exact = N * e_ring - float(np.sum(np.log1p(j * xi) - np.log(j + 1.0))) / beta
+    w = wl.custom(N, P, d=d, beta=beta, g=0.0, xi=xi, init="iid")
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda())
+    xr = ring[:, 0, :]
+    f_ring = -ks * (2 * xr - np.roll(xr, 1, axis=0) - np.roll(xr, -1, axis=0)) - (w.omega ** 2 / P) * xr
+    ref = np.repeat(f_ring[:, None, :], N, axis=1)
+    for _ in range(2):
+        F, vb, sg = sim.forces()
+        assert sg == 1 and abs(vb - vb_exact) <= RTOL * abs(vb_exact)
+        assert relerr(F.cpu().numpy(), ref) <= 1e-9
+    assert sim.get_diagnostics()["fallbacks"] == 0
+    sim.close()
+
+
+def test_set_state_on_a_used_handle(binding, oracle):
+    """The gauge of the last evaluation survives pimd_set_state.  States that differ from the previous one
+    by 0.3 .. 2 length units per bead, and a different seed of the same workload, must come out right: either the stale
+    gauge is accepted and exact to 1e-9, or it is rejected (acceptance band 2^+-8) and the max-plus pass runs."""
+    w = wl.custom(700, 8, d=2, beta=3.0, g=0.2, xi=1.0, init="ring", sigma=2.0)
+    x, v = wl.make_state(w, 0)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda())
+    sim.forces()
+    rng = np.random.default_rng(17)
+    states = [x + rng.normal(0.0, a, size=x.shape) for a in (0.05, 0.3, 1.0, 2.0)]
+    states += [wl.make_state(w, 1)[0], x + rng.normal(0.0, 0.3, size=(1,) + x.shape[1:])]   # other seed; rigid particle moves
+    for y in states:
+        y = np.ascontiguousarray(y)
+        sim.set_state(torch.from_numpy(y).cuda())
+        F, vb, sg = sim.forces()
+        Fo, vbo, sgo = oracle.forces(y, w.beta, w.omega, w.g, w.s, w.xi)
+        assert sg == sgo and abs(vb - vbo) <= RTOL * abs(vbo)
+        check_forces(F.cpu().numpy(), Fo, RTOL)
+    diag = sim.get_diagnostics()
+    sim.close()
+    assert diag["fallbacks"] >= 1          # the large moves cannot fit the old gauge
