@@ -25,13 +25,26 @@ if ROOT not in sys.path:
 METRIC = "PIMD MD steps/s"
 UNIT = "steps/s"
 # algorithmic FP64 work of the pair kernel: 25 FP64 instructions per unordered bead pair at d = 2
-# (SURVEY.md 8(d)), counted as FMA-equivalents = 2 flop each
+# (SURVEY.md 8(d)), counted as FMA-equivalents = 2 flop each; the shipped kernel
+# executes 16 FP64 instructions per pair (SASS: 2 differences, 2 for r^2, 8 table exponential, 4 force FMAs)
 FLOP_PER_PAIR = 50.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/r1_d_cfg3.md for cfg3 -- unchanged since r1_b_cfg3.md --, profiles/r1_b_cfg5b.md for cfg5b); None where no
-# capture of that workload exists
-NCU_TRAFFIC = {("cfg3", "pair"): 1706240 + 0, ("cfg3", "forcepass"): 291072 + 0,
-               ("cfg5b", "pair"): 5186048 + 0, ("cfg5b", "forcepass"): 1768960 + 0}
+FLOP_PER_PAIR_EXECUTED = 32.0
+FLOP_PER_ELEMENT = 54.0   # force pass: 27 FP64 instructions per lower-triangle element and direction
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` at `workload`, from the summary of the
+    `ncu --set full` capture of the shipped code state (profiles/r2_traffic.csv: workload,kernel,read,write); None if
+    that capture has no such row."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
+            for line in f:
+                c = [t.strip() for t in line.split(",")]
+                if len(c) >= 4 and c[0] == workload and c[1] == kernel:
+                    return int(float(c[2]) + float(c[3]))
+    except OSError:
+        pass
+    return None
 
 
 def describe(w):
@@ -129,6 +142,9 @@ def load_peaks():
 # the oracle, timed on the host cores (cpu_baseline leg and --impl reference)
 # ------------------------------------------------------------------------------------------------
 def time_oracle(w, budget_s, max_steps=None):
+    """(steps/s, steps, seconds) of orc_step on a bounded sample of workload w.  One call of orc_step is one complete MD
+    step (force evaluation included).  At N >= 5000 a step takes tens of seconds: the sample is then that one step, started
+    from zero forces instead of paying a second force evaluation for the opening half kick (timing is value-independent)."""
     import numpy as np
 
     import oracle
@@ -136,11 +152,14 @@ def time_oracle(w, budget_s, max_steps=None):
 
     oracle.build()
     x, v = wl.make_state(w, 0)
-    F, _, _ = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
+    big = w.N >= 5000
+    F = np.zeros_like(x) if big else oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)[0]
     nhc = np.zeros((4, x.size))
     t0 = time.perf_counter()
     oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, w.xi, w.dt, 1, 1.0, 0, 0, 1)
     t_first = time.perf_counter() - t0
+    if big or t_first >= budget_s:
+        return 1.0 / t_first, 1, t_first
     n = max(1, int(budget_s / max(t_first, 1e-6)))
     if max_steps is not None:
         n = min(n, max_steps)
@@ -177,20 +196,113 @@ def run_reference(args, w):
     return 0
 
 
+
+
 # ------------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
-def timed_steps(torch, sim, steps, flush):
-    """Device time of `steps` MD steps, one event pair per step, an L2 flush between steps."""
+EST_EVERY = 10   # BASELINE config 3: "energy and density estimators every 10 steps", inside the timed region
+REPEATS = 3      # 3 repeats, median
+
+
+def timed_steps(torch, sim, steps, flush, w, est_every):
+    """Device time of `steps` MD steps, one event pair per step, an L2 flush (outside the events) between steps.
+    With est_every > 0 the steps whose number is a multiple of it evaluate and accumulate the estimators (pimd_run)."""
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     for a, b in evs:
         if flush is not None:
             flush.zero_()
         a.record()
-        sim.step(1)
+        if est_every:
+            sim.run(1, est_every=est_every, nbins=w.nbins, rmax=w.rmax)
+        else:
+            sim.step(1)
         b.record()
     torch.cuda.synchronize()
     return sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+
+
+def median_rate(torch, sim, steps, flush, w, est_every, world=1):
+    """median over REPEATS of steps / (max over ranks of the device time of `steps` flushed steps)"""
+    rates = []
+    for _ in range(REPEATS):
+        t = max_over_ranks(timed_steps(torch, sim, steps, flush, w, est_every), world)
+        rates.append(world * steps / t)
+    rates.sort()
+    return rates[len(rates) // 2], rates
+
+
+def roofline_of(w, kern, iso, fp64_peak):
+    """roofline object of the dominant throughput kernel of workload w from per-kernel times (ms) inside the step
+    (kern) and alone (iso); DESIGN.md section 8"""
+    pairs = w.P * w.N * (w.N - 1) / 2.0 if w.g != 0.0 else 0.0
+    if pairs and kern.get("pair"):
+        t, ta = kern["pair"] * 1e-3, iso.get("pair", 0.0) * 1e-3
+        ach = pairs * FLOP_PER_PAIR / t / 1e12
+        return {"bound": "alu", "kernel": "k_pair (pair forces, Newton's third law)", "achieved": ach, "peak": fp64_peak,
+                "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": ncu_traffic(w.name, "k_pair"),
+                "frac_algorithmic": ach / fp64_peak,
+                "frac_executed": pairs * FLOP_PER_PAIR_EXECUTED / t / 1e12 / fp64_peak,
+                "traffic_note": "DRAM bytes per launch (ncu); the algorithmic inputs are L2-resident: %d B of positions" % (w.P * w.N * w.d * 8),
+                "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
+                               "1.965 GHz x 2 = 37.2 TFLOP/s)",
+                "convention": "frac = frac_algorithmic: 50 flop (25 FP64 instructions, SURVEY.md 8(d)) per unordered bead pair, %d "
+                              "pairs per launch; frac_executed counts the 16 FP64 instructions (32 flop) per pair the shipped "
+                              "SASS executes and is the figure to hold against north_star's 50 %% (ncu FP64-pipe utilisation: "
+                              "profiles/)" % int(pairs),
+                "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
+                "alone": {"ms": iso.get("pair"), "frac": (pairs * FLOP_PER_PAIR / ta / 1e12 / fp64_peak) if ta else None,
+                          "frac_executed": (pairs * FLOP_PER_PAIR_EXECUTED / ta / 1e12 / fp64_peak) if ta else None}}
+    # non-interacting workloads: the exchange passes dominate; they recompute the closing springs
+    # instead of streaming an N x N matrix, so they are ALU bound too (DESIGN.md)
+    fp_ms = kern.get("forcepass")
+    elems = float(w.N) * (w.N + 1)  # two sweeps over the lower triangle
+    ach = elems * FLOP_PER_ELEMENT / (fp_ms * 1e-3) / 1e12 if fp_ms else None
+    return {"bound": "alu", "kernel": "k_forcepass (connection probabilities)", "achieved": ach, "peak": fp64_peak,
+            "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": ncu_traffic(w.name, "k_forcepass"),
+            "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak",
+            "convention": "54 flop (27 FP64 instructions) per matrix element, N(N+1) elements per launch",
+            "alone": {"ms": iso.get("forcepass"),
+                      "frac": (elems * FLOP_PER_ELEMENT / (iso["forcepass"] * 1e-3) / 1e12 / fp64_peak) if iso.get("forcepass") else None}}
+
+
+def kernel_profile(sim, nsteps, w):
+    """per-kernel device time (ms per launch) and the chain's phase clock over nsteps steps"""
+    sim.set_profiling(True)
+    sim.get_profile()
+    sim.get_chain_phases()
+    sim.run(nsteps, est_every=EST_EVERY, nbins=w.nbins, rmax=w.rmax)
+    prof = sim.get_profile()
+    sim.set_profiling(False)
+    return {k: ms / n for k, (ms, n) in prof.items() if n}, {k: n for k, (ms, n) in prof.items() if n}, sim.get_chain_phases()
+
+
+def e2e_rate(torch, sim, x0, v0, ne2e, world, barrier):
+    """end to end through the C ABI with HOST buffers: every step uploads the full state (x, v and the forces that belong
+    to x, as a checkpointed host-resident run would), advances one MD step, and reads x, v, F back"""
+    xh = torch.from_numpy(x0.copy()).pin_memory()
+    vh = torch.from_numpy(v0.copy()).pin_memory()
+    fh = torch.empty_like(xh).pin_memory()
+    sim.set_state_host(xh, vh)
+    sim.forces_host(fh)
+
+    def e2e_step():
+        sim.set_state_host(xh, vh)
+        sim.set_forces_host(fh)
+        sim.step(1)
+        sim.get_state_host(xh, vh)
+        sim.get_forces_host(fh)  # synchronises
+
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    te = time.perf_counter()
+    for _ in range(ne2e):
+        e2e_step()
+    barrier()
+    te = time.perf_counter() - te
+    nbytes = int(x0.nbytes + v0.nbytes + x0.nbytes)
+    return whole_job_rate(ne2e, te, world), nbytes
 
 
 def run_ours(args, w):
@@ -228,65 +340,65 @@ def run_ours(args, w):
         sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
         return sim, x, v
 
-    # replicas: every rank advances its own seeded copy of the workload
-    sim, x0, v0 = make_sim(w, rank)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    W = max(args.warmup, 3)
 
-    sim.step(max(args.warmup, 3))
-    torch.cuda.synchronize()
-    sim.set_profiling(True)
-    sim.get_profile()
-    l0 = sim.launch_count()
-    barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
-    t0 = time.time()
-    t_dev = timed_steps(torch, sim, args.steps, flush)
-    barrier()
-    t1 = time.time()
-    clocks = sampler.stop(t0, t1) if sampler else None
-    launches = sim.launch_count() - l0
-    prof = sim.get_profile()
-    sim.set_profiling(False)
-    phases = sim.get_chain_phases()
-    t_dev = max_over_ranks(t_dev, world)
-    value = world * args.steps / t_dev
+    def measure(wk, steps, seed, full):
+        """the headline protocol on workload wk: W warm-up steps; REPEATS x `steps` flushed steps from the seeded initial
+        cloud; args.equil untimed steps of equilibration on the GPU; REPEATS x `steps` flushed steps from the thermalised
+        state with the estimators every EST_EVERY steps inside the timed region (median of the repeats = value)"""
+        sim, x0, v0 = make_sim(wk, seed)
+        sim.step(W)
+        torch.cuda.synchronize()
+        barrier()
+        v_init, _ = median_rate(torch, sim, steps, flush, wk, 0, world)
+        # untimed equilibration on the GPU.  With forces -(1/P) grad U on unit-mass beads the cloud's centroid oscillates
+        # in the trap at omega / sqrt(P); the friction that damps it fastest is twice that (the default gamma = 1
+        # overdamps it: 1/e time gamma P / omega^2 = 32 time units at P = 32)
+        sim.set_gamma(2.0 * wk.omega / np.sqrt(wk.P))
+        sim.step(args.equil)
+        sim.set_gamma(1.0)
+        torch.cuda.synchronize()
+        fb0 = sim.get_diagnostics()["fallbacks"]
+        l0 = sim.launch_count()
+        barrier()
+        sampler = ClockSampler(local) if (rank == 0 and full) else None
+        t0 = time.time()
+        v_therm, reps = median_rate(torch, sim, steps, flush, wk, EST_EVERY, world)
+        barrier()
+        t1 = time.time()
+        out = {"value": v_therm, "repeats": reps, "value_initial_cloud": v_init,
+               "gpu_launches": (sim.launch_count() - l0) // REPEATS,
+               "clocks": sampler.stop(t0, t1) if sampler else None}
+        # the same steps back to back with the state left in L2 (how an MD run actually executes; graph replay)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        sim.run(steps, est_every=EST_EVERY, nbins=wk.nbins, rmax=wk.rmax)
+        b.record()
+        torch.cuda.synchronize()
+        out["steps_per_s_l2_resident"] = world * steps / (a.elapsed_time(b) * 1e-3)
+        nsamp, sp, sv, _, _ = sim.read_accumulators()
+        out["sampled"] = {"n": float(nsamp), "e_prim_mean": float(sp / max(nsamp, 1.0)), "e_vir_mean": float(sv / max(nsamp, 1.0))}
+        kern, counts, phases = kernel_profile(sim, max(5, min(steps, 20)), wk)
+        out["kernels_ms"] = kern
+        out["recursion"] = recursion_report(wk, {"chain": {"ms_avg": kern.get("chain")}}, phases, max(5, min(steps, 20)), None)
+        met, skipped = phases[11], phases[12]
+        out["recursion"]["helper_batches_skipped_frac"] = (skipped / met) if met else None
+        nbk = (wk.N + 31) // 32
+        out["recursion"]["factorised_blocks_frac"] = phases[6] / float(max(5, min(steps, 20)) * nbk)
+        out["fallbacks_in_timed_steps"] = sim.get_diagnostics()["fallbacks"] - fb0
+        if full:
+            # the same kernels timed alone (exchange and bead parts serialised on one stream): the burst figure
+            sim.set_concurrency(False)
+            iso, _, _ = kernel_profile(sim, max(5, min(steps, 20)), wk)
+            sim.set_concurrency(True)
+            out["kernels_alone_ms"] = iso
+            out["e2e_value"], out["e2e_bytes"] = e2e_rate(torch, sim, x0, v0, max(3, min(steps, 50)), world, barrier)
+        sim.close()
+        return out
 
-    # the same K steps back to back with the state left in L2 (how an MD run actually executes)
-    barrier()
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record()
-    sim.step(args.steps)
-    b.record()
-    torch.cuda.synchronize()
-    resident_sps = args.steps / (a.elapsed_time(b) * 1e-3)
-
-    # end to end through the C ABI with HOST buffers: every step uploads the full state (x, v and the forces that
-    # belong to x, as a checkpointed host-resident run would), advances one MD step, and reads x, v, F back
-    xh = torch.from_numpy(x0.copy()).pin_memory()
-    vh = torch.from_numpy(v0.copy()).pin_memory()
-    fh = torch.empty_like(xh).pin_memory()
-    sim.set_state_host(xh, vh)
-    sim.forces_host(fh)
-    ne2e = max(3, min(args.steps, 50))
-
-    def e2e_step():
-        sim.set_state_host(xh, vh)
-        sim.set_forces_host(fh)
-        sim.step(1)
-        sim.get_state_host(xh, vh)
-        sim.get_forces_host(fh)  # synchronises
-
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    te = time.perf_counter()
-    for _ in range(ne2e):
-        e2e_step()
-    barrier()
-    te = time.perf_counter() - te
-    e2e = whole_job_rate(ne2e, te, world)
-    nbytes = int(x0.nbytes + v0.nbytes + x0.nbytes)
-
+    # replicas: every rank advances its own seeded copy of the workload (DESIGN.md "Multi-GPU")
+    m = measure(w, args.steps, rank, True)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -294,85 +406,88 @@ def run_ours(args, w):
 
     peaks, peak_src = load_peaks()
     fp64_peak = binding.probe_fp64_peak()
-    # the same kernels timed alone (exchange and bead parts serialised on one stream): the burst figure
-    sim.set_concurrency(False)
-    sim.set_profiling(True)
-    sim.get_profile()
-    sim.step(max(5, min(args.steps, 20)))
-    iso = {k: ms / n for k, (ms, n) in sim.get_profile().items() if n}
-    sim.set_profiling(False)
-    sim.set_concurrency(True)
     pairs = w.P * w.N * (w.N - 1) / 2.0 if w.g != 0.0 else 0.0
-    kern = {k: {"ms_avg": (ms / n if n else None), "launches": n} for k, (ms, n) in prof.items() if n}
-    bead_ms = kern.get("pair", {}).get("ms_avg")
-    if pairs and bead_ms:
-        ach = pairs * FLOP_PER_PAIR / (bead_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "k_pair (pair forces, Newton's third law)", "achieved": ach, "peak": fp64_peak,
-                    "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": NCU_TRAFFIC.get((w.name, "pair")),
-                    "traffic_note": "DRAM bytes per launch (ncu); the algorithmic inputs are L2-resident: %d B of positions" % (w.P * w.N * w.d * 8),
-                    "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
-                                   "1.965 GHz x 2 = 37.2 TFLOP/s)",
-                    "convention": "50 flop (25 FP64 instructions, SURVEY.md 8(d)) per unordered bead pair, %d pairs per launch; "
-                                  "the shipped kernel spends 16 FP64 instructions per pair (table-driven exp), so frac can "
-                                  "exceed the FP64 pipe utilisation ncu reports" % int(pairs),
-                    "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
-                    "alone": {"ms": iso.get("pair"), "frac": pairs * FLOP_PER_PAIR / (iso["pair"] * 1e-3) / 1e12 / fp64_peak}}
-    else:
-        # non-interacting workloads: the exchange passes dominate; they recompute the closing springs
-        # instead of streaming an N x N matrix, so they are ALU bound too
-        fp_ms = kern.get("forcepass", {}).get("ms_avg")
-        elems = float(w.N) * (w.N + 1)  # two sweeps over the lower triangle
-        ach = elems * 54.0 / (fp_ms * 1e-3) / 1e12 if fp_ms else None
-        roofline = {"bound": "alu", "kernel": "k_forcepass (connection probabilities)", "achieved": ach, "peak": fp64_peak,
-                    "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": NCU_TRAFFIC.get((w.name, "forcepass")),
-                    "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak",
-                    "convention": "54 flop (27 FP64 instructions) per matrix element, N(N+1) elements per launch",
-                    "alone": {"ms": iso.get("forcepass"),
-                              "frac": (elems * 54.0 / (iso["forcepass"] * 1e-3) / 1e12 / fp64_peak) if iso.get("forcepass") else None}}
-
+    nb = m["e2e_bytes"]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": W,
+        "ms_per_step": 1e3 * world / m["value"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": describe(w), "l2": "flushed between timed steps (256 MiB device write outside the events)",
+                   "state": "thermalised on the GPU by %d untimed steps (friction 2 omega/sqrt(P), the centroid's critical damping) after the seeded initial cloud" % args.equil,
+                   "estimators": "energy + radial density every %d steps inside the timed region" % EST_EVERY,
+                   "protocol": "median of %d repeats of %d steps" % (REPEATS, args.steps),
                    "parallelism": "replicas x%d (one independent seeded copy per GPU, no collective on the data path)" % world},
-        "clocks": clocks,
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+        "clocks": m["clocks"],
+        "e2e": {"value": m["e2e_value"], "unit": UNIT, "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
                 "note": "pimd_set_state_host + pimd_set_forces_host + pimd_step(1) + pimd_get_state_host + pimd_get_forces_host per "
                         "step, pinned host buffers, wall clock"},
-        "gpu_launches": launches,
-        "pair_forces_per_s": pairs * value,
-        "steps_per_s_l2_resident": resident_sps * world,
-        "kernels": kern,
-        "kernels_alone_ms": iso,
-        "recursion": recursion_report(w, kern, phases, args.steps, clocks),
-        "roofline": roofline,
+        "gpu_launches": m["gpu_launches"],
+        "repeats": m["repeats"],
+        "value_initial_cloud": m["value_initial_cloud"],
+        "pair_forces_per_s": pairs * m["value"],
+        "steps_per_s_l2_resident": m["steps_per_s_l2_resident"],
+        "fallbacks_in_timed_steps": m["fallbacks_in_timed_steps"],
+        "sampled": m["sampled"],
+        "kernels_ms": m["kernels_ms"],
+        "kernels_alone_ms": m["kernels_alone_ms"],
+        "recursion": m["recursion"],
+        "roofline": roofline_of(w, m["kernels_ms"], m["kernels_alone_ms"], fp64_peak),
         "peaks": {"fp64_tflops_probe": fp64_peak, "hbm_gbs": peaks.get("hbm_gbs"), "source": peak_src},
     }
-    sim.close()
 
+    if world == 1 and not args.no_also:
+        # north_star states its targets at N = 10000: the same objects for config 5 (N = 10000) and 5b
+        also = []
+        for name in args.also.split(","):
+            wk = wl.WORKLOADS[name]
+            r = measure(wk, args.sweep_steps, 0, True)
+            pp = wk.P * wk.N * (wk.N - 1) / 2.0 if wk.g != 0.0 else 0.0
+            row = {"workload": describe(wk), "value": r["value"], "unit": UNIT, "value_initial_cloud": r["value_initial_cloud"],
+                   "pair_forces_per_s": pp * r["value"], "steps_per_s_l2_resident": r["steps_per_s_l2_resident"],
+                   "kernels_ms": r["kernels_ms"], "kernels_alone_ms": r["kernels_alone_ms"], "recursion": r["recursion"],
+                   "roofline": roofline_of(wk, r["kernels_ms"], r["kernels_alone_ms"], fp64_peak),
+                   "e2e": {"value": r["e2e_value"], "unit": UNIT, "h2d_bytes_per_step": r["e2e_bytes"], "d2h_bytes_per_step": r["e2e_bytes"]},
+                   "fallbacks_in_timed_steps": r["fallbacks_in_timed_steps"]}
+            if not args.no_cpu:
+                row["cpu_baseline"] = cpu_baseline(wk, 1.0)
+            also.append(row)
+        line["also"] = also
     if world == 1 and not args.no_sweep:
         sweep = []
         for name in args.sweep.split(","):
             wk = wl.WORKLOADS[name]
-            s2, _, _ = make_sim(wk, 0)
-            s2.step(3)
+            r = measure(wk, args.sweep_steps, 0, False)
+            pp = wk.P * wk.N * (wk.N - 1) / 2.0 if wk.g != 0.0 else 0.0
+            sweep.append({"workload": name, "N": wk.N, "P": wk.P, "g": wk.g, "steps_per_s": r["value"],
+                          "steps_per_s_initial_cloud": r["value_initial_cloud"], "steps_per_s_l2_resident": r["steps_per_s_l2_resident"],
+                          "pair_forces_per_s": pp * r["value"], "kernels_ms": r["kernels_ms"],
+                          "ns_per_row": r["recursion"].get("ns_per_row"),
+                          "helper_batches_skipped_frac": r["recursion"].get("helper_batches_skipped_frac"),
+                          "fallbacks_in_timed_steps": r["fallbacks_in_timed_steps"]})
+        line["sweep"] = sweep
+        line["sweep_protocol"] = "as the headline: thermalised by %d steps, L2 flushed between steps, median of %d x %d steps" % (
+            args.equil, REPEATS, args.sweep_steps)
+    if world == 1 and not args.no_batch:
+        # replica batches: B replicas of the small configurations in one set of launches
+        rows = []
+        for name, B in (("cfg1", 64), ("cfg2", 32), ("cfg4", 5)):
+            wk = wl.WORKLOADS[name]
+            xis = [wk.xi] * B if name != "cfg4" else [-0.5, -0.3, 0.3, 0.5, 1.0]
+            xs, vs = zip(*[wl.make_state(wk, b) for b in range(B)])
+            sb = binding.Pimd(wk.N, wk.P, wk.d, wk.beta, wk.omega, wk.g, wk.s, xis, wk.dt, thermostat=1, seed=list(range(B)))
+            sb.set_state(torch.from_numpy(np.stack(xs)).cuda(), torch.from_numpy(np.stack(vs)).cuda())
+            sb.step(50)
             torch.cuda.synchronize()
-            n2 = args.sweep_steps
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            nst = 400
             a.record()
-            s2.step(n2)
+            sb.run(nst, est_every=EST_EVERY, nbins=wk.nbins, rmax=wk.rmax)
             b.record()
             torch.cuda.synchronize()
-            sps = n2 / (a.elapsed_time(b) * 1e-3)
-            s2.set_profiling(True)
-            s2.get_profile()
-            s2.step(5)
-            pr = s2.get_profile()
-            pp = wk.P * wk.N * (wk.N - 1) / 2.0 if wk.g != 0.0 else 0.0
-            sweep.append({"workload": name, "N": wk.N, "P": wk.P, "g": wk.g, "steps_per_s": sps, "pair_forces_per_s": pp * sps,
-                          "kernels_ms": {k: ms / n for k, (ms, n) in pr.items() if n}})
-            s2.close()
-        line["sweep"] = sweep
+            rows.append({"workload": name, "replicas": B, "xi": sorted(set(xis)), "batch_steps_per_s": nst / (a.elapsed_time(b) * 1e-3),
+                         "replica_steps_per_s": B * nst / (a.elapsed_time(b) * 1e-3)})
+            sb.close()
+        line["replica_batches"] = rows
     if world == 1 and not args.no_nxn:
         # the paper's N x N intermediates, materialised on request (not on the hot path): HBM-write rooflines at N = 10000
         wk = wl.WORKLOADS["cfg5_N10000"]
@@ -393,7 +508,8 @@ def run_ours(args, w):
         pr3 = s3.get_profile()
         nbytes_nn = 8.0 * wk.N * wk.N
         line["nxn_passes"] = {"workload": "cfg5_N10000", "bound": "hbm", "peak": peaks.get("hbm_gbs"), "unit": "GB/s",
-                              "bytes_per_launch": nbytes_nn, "peak_source": peak_src}
+                              "bytes_per_launch": nbytes_nn, "peak_source": peak_src,
+                              "note": "on-request write-only kernels; the hot path has no N x N pass (DESIGN.md section 6)"}
         for key, name in (("emat", "k_emat (cycle energies, Eq. 7-10)"), ("prmat", "k_prmat (connection probabilities, Eq. 12-14)")):
             ms = pr3[key][0] / max(pr3[key][1], 1)
             gbs = nbytes_nn / (ms * 1e-3) / 1e9
@@ -411,13 +527,17 @@ def run_ours(args, w):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1000)
-    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--equil", type=int, default=3000, help="untimed equilibration steps before the timed region")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--sweep", default="cfg1,cfg2,cfg4,cfg5_N2500,cfg5_N10000,cfg5_N20000,cfg5_N40000,cfg5b")
+    ap.add_argument("--also", default="cfg5_N10000,cfg5b", help="workloads that get roofline + e2e + cpu_baseline beside the headline")
     ap.add_argument("--sweep-steps", type=int, default=20)
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-also", action="store_true")
+    ap.add_argument("--no-batch", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-nxn", action="store_true", help="skip the materialised N x N passes (0.8 GB at N=10000)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -425,6 +545,14 @@ def main():
     from paper_2404_02628_b200 import workloads as wl
 
     w = wl.WORKLOADS[args.workload]
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and world == 1 and "RANK" not in os.environ:
+        # asked for N GPUs without a launcher: start one rank per GPU ourselves (the driver uses the same command line)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 1000), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    if args.gpus != world and "RANK" in os.environ:
+        raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
     if args.impl == "reference":
         return run_reference(args, w)
     return run_ours(args, w)

@@ -260,7 +260,9 @@ int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
  *   [4] a helper warp has its share of the next M tile, [5] of the older column blocks too, [8] of everything
  *   ([13], [14]: two more helper warps, on the other scheduler partitions), [7] the last block's columns are published,
  *   [9] the workers' panel is fetched ([10]: reads of the panel words it took, one per block = it never waited),
- *   [15] gauges, exponent tables and prefetch of the blocks ahead are in place.
+ *   [15] gauges, exponent tables and prefetch of the blocks ahead are in place; counts, not cycles: [11] batches of
+ *   exponentials the helper warps met (older column blocks, E' tiles), [12] how many of them were skipped because every
+ *   entry lay below e^-260 of its row's gauge, [6] blocks whose exponent arguments were formed in the factorised way.
  * Evaluations with a fresh max-plus gauge (k_chain) fill [0] loop overhead, [2k-1] the dependent warp's own time
  * in phase k = 1..4 (1 max-plus pass, 2 exponentials, 3 linear pass, 4 publish), [2k] its barrier wait. */
 int pimd_get_chain_phases(pimd_t h, uint64_t *cycles_host);

@@ -34,6 +34,7 @@ struct ExchCtx {
     double *ecpart;
     RepParams *rp;
     bool gauge_valid; // p.g / p.gs hold the (T, Zhat) of a completed evaluation of nearby positions
+    int history;      // evaluations made along the current trajectory (pimd_set_state starts a new one): 2 allow extrapolation
 };
 
 } // namespace
@@ -198,6 +199,7 @@ size_t carve(pimd_t h, unsigned char *base)
                 c.p.cc[dir] = (double *)take(n * 8);
                 c.p.g[dir] = (double2 *)take((n + 1) * 16);
                 c.p.gs[dir] = (double *)take((n + 1) * 8);
+                c.p.gprev[dir] = (double2 *)take((n + 1) * 16);
                 c.p.pan_m[dir] = (double *)take(n * 8);
                 c.p.pan_s[dir] = (double *)take(n * 8);
                 c.p.panel_ready[dir] = (int *)take((size_t)c.NB * 4);
@@ -283,6 +285,7 @@ void setup_species(pimd_t h)
             c.nprep = (c.N + PREP_TB - 1) / PREP_TB;
             c.nasm = (c.N + ASM_TB - 1) / ASM_TB;
             c.gauge_valid = false;
+            c.history = 0;
             // Panel workers per direction.  A worker spins while it waits for columns and owns a whole SM, so only as many
             // as the panel work needs are launched: a worker needs about 480 NB cycles for its last row blocks and gets
             // nworkers x (one chain block, about 3000 cycles) for each, so NB/5 workers keep the panels ahead of the chain;
@@ -381,7 +384,7 @@ template <int D> int launch_prep(pimd_t h, ExchCtx &c, cudaStream_t st)
     {
         ProfScope ps(h, PIMD_PROF_PREP, st);
         k_prep<D, PREP_TB><<<dim3(c.nprep, h->B), PREP_TB * PREP_SPLIT, 0, st>>>(x, x1, xP, ein, sl, c.N, h->P, c.NB, h->ks, h->kk, c.p, c.rp,
-                                                                               h->gflags, h->rstride);
+                                                                               h->gflags, c.history >= 2 ? 1 : 0, h->rstride);
     }
     CU(cudaGetLastError());
     return PIMD_OK;
@@ -421,6 +424,7 @@ template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t
             CU(cudaLaunchCooperativeKernel(fn, grid, block, args, h->chain_smem, st));
         }
         c.gauge_valid = true;
+        c.history++;
         const int NT = (c.N + FP_TB - 1) / FP_TB;
         // NT (NT+1) tiles at or below the diagonal (both directions); with fewer than 8 per SM one thread per row leaves
         // the kernel latency bound, so four threads share a row (measured at cfg3: 0.023 -> 0.017 ms)
@@ -661,25 +665,32 @@ int run_steps(pimd_t h, int nsteps, int est_every, int nbins, double rmax)
     // open step s ; forces ; [close s + open s+1] ; forces ; ... ; close last
     rc = launch_integrate(h, false, true, 0, h->step);
     if (rc) return rc;
+    // Steps are launched one by one until the stale-gauge kernel with extrapolation is what a step runs (two
+    // evaluations along this trajectory); from then on all but the last step replay the captured graphs, the step
+    // counter of the noise living on the device meanwhile.
+    auto graph_ready = [&]() {
+        if (!h->use_graph || h->profiling) return false;
+        for (int sp = 0; sp < h->nspecies; ++sp)
+            if (!h->all_zero[0] && !(h->ex[0][sp].gauge_valid && h->ex[0][sp].history >= 2)) return false;
+        return true;
+    };
     int it = 0;
-    bool gauge_ok = true;
-    for (int sp = 0; sp < h->nspecies; ++sp) gauge_ok = gauge_ok && (h->ex[0][sp].gauge_valid || h->all_zero[0]);
-    if (h->use_graph && !h->profiling && gauge_ok && nsteps >= 3 && ensure_graphs(h, est_every > 0, nbins, rmax) == PIMD_OK) {
-        // all but the last step replay the captured graphs; the step counter of the noise lives on the device meanwhile
-        k_step_counter<<<1, 32, 0, h->s0>>>(h->dstep, (unsigned long long)h->step, 0);
-        CU(cudaGetLastError());
-        CU(cudaEventRecord(h->ev_gin, h->s0));
-        CU(cudaStreamWaitEvent(h->sg, h->ev_gin, 0));
-        for (; it < nsteps - 1; ++it) {
-            const bool e = is_est(h->step + 1);
-            CU(cudaGraphLaunch(e ? h->gexec_est : h->gexec, h->sg));
-            h->launches += e ? h->graph_est_launches : h->graph_launches;
-            h->step++;
+    while (it < nsteps) {
+        if (nsteps - it >= 3 && graph_ready() && ensure_graphs(h, est_every > 0, nbins, rmax) == PIMD_OK) {
+            k_step_counter<<<1, 32, 0, h->s0>>>(h->dstep, (unsigned long long)h->step, 0);
+            CU(cudaGetLastError());
+            CU(cudaEventRecord(h->ev_gin, h->s0));
+            CU(cudaStreamWaitEvent(h->sg, h->ev_gin, 0));
+            for (; it < nsteps - 1; ++it) {
+                const bool e = is_est(h->step + 1);
+                CU(cudaGraphLaunch(e ? h->gexec_est : h->gexec, h->sg));
+                h->launches += e ? h->graph_est_launches : h->graph_launches;
+                h->step++;
+            }
+            CU(cudaEventRecord(h->ev_gout, h->sg));
+            CU(cudaStreamWaitEvent(h->s0, h->ev_gout, 0));
+            continue;
         }
-        CU(cudaEventRecord(h->ev_gout, h->sg));
-        CU(cudaStreamWaitEvent(h->s0, h->ev_gout, 0));
-    }
-    for (; it < nsteps; ++it) {
         const bool e = is_est(h->step + 1);
         rc = eval_forces(h, false, e, nbins, rmax);
         if (rc == PIMD_OK && e) rc = launch_estimate(h, nbins, true);
@@ -688,6 +699,7 @@ int run_steps(pimd_t h, int nsteps, int est_every, int nbins, double rmax)
         rc = launch_integrate(h, true, !last, h->step, h->step + 1);
         if (rc) return rc;
         h->step++;
+        ++it;
     }
     return PIMD_OK; // the flags eval_forces set for the last step hold: F, the tables belong to the final positions
 }
@@ -964,8 +976,10 @@ static int set_state_impl(pimd_t h, const double *x, const double *v, cudaMemcpy
     h->tables_valid = false;
     h->scalars_valid = false;
     h->shard_imported = false;
+    for (int set = 0; set < 2; ++set)
+        for (int sp = 0; sp < h->nspecies; ++sp) h->ex[set][sp].history = 0; // a new trajectory: no extrapolation
     // The exchange gauge of the last evaluation is kept: the stale-gauge kernel accepts it only if every row sum stays
-    // within 2^+-8 of it (chain_cta_spec) and otherwise redoes the recursion with a fresh max-plus gauge.
+    // within 2^+-64 of it (chain_cta_spec) and otherwise redoes the recursion with a fresh max-plus gauge.
     return PIMD_OK;
 }
 

@@ -2,7 +2,7 @@
 
 Tolerances (BASELINE.json north_star): 1e-9 relative on V_B and on the forces (max-norm), FP64.
 For xi < 0 the tolerance is scaled by the conditioning kappa = sum|terms| / |sum terms| of the
-signed sums (R7); here kappa stays O(1..100) and a fixed 1e-7 bound is used.
+signed sums (R7), computed by the oracle (orc_conditioning) for the configuration at hand.
 """
 import numpy as np
 import pytest
@@ -102,9 +102,10 @@ def test_signed_fictitious_particles(binding, oracle, xi, N):
     x, _ = wl.make_state(w, 5)
     Fo, vbo, sgo = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
     F, vb, sg = gpu_forces(binding, w, x)
+    tol = RTOL * oracle.conditioning(x, w.beta, w.xi)
     assert sg == sgo
-    assert abs(vb - vbo) <= 1e-7 * abs(vbo)
-    check_forces(F, Fo, 1e-7)
+    assert abs(vb - vbo) <= tol * abs(vbo)
+    check_forces(F, Fo, tol)
 
 
 def test_tables_match_oracle(binding, oracle):
@@ -129,7 +130,7 @@ def test_paper_scale_configs(binding, oracle, name):
     x, _ = wl.make_state(w, 0)
     Fo, vbo, sgo = oracle.forces(x, w.beta, w.omega, w.g, w.s, w.xi)
     F, vb, sg = gpu_forces(binding, w, x)
-    tol = RTOL if w.xi >= 0 else 1e-7
+    tol = RTOL if w.xi >= 0 else RTOL * oracle.conditioning(x, w.beta, w.xi)
     assert sg == sgo
     assert abs(vb - vbo) <= tol * abs(vbo)
     check_forces(F, Fo, tol)
@@ -286,23 +287,6 @@ def test_full_size_invariants(binding, name):
         assert abs(-float(np.sum(x * Fint)) - 2.0 * ec) <= 1e-9 * abs(2.0 * ec)
 
 
-def test_full_size_sampled_pair_forces(binding, oracle):
-    """cfg5b (N = 10000, g = 0.2): the external (trap + pair) force on sampled beads against the oracle's
-    one-bead routine, and the sampled total force minus it against a g = 0 evaluation."""
-    w = wl.WORKLOADS["cfg5b"]
-    x, _ = wl.make_state(w, 0)
-    F, vb, sg = gpu_forces(binding, w, x)
-    F0, vb0, _ = gpu_forces(binding, w.with_(g=0.0), x)
-    assert abs(vb - vb0) <= 1e-12 * abs(vb)  # V_B does not depend on the pair interaction
-    rng = np.random.default_rng(3)
-    fmax = np.max(np.abs(F - F0))
-    for _ in range(40):
-        j, l = int(rng.integers(w.P)), int(rng.integers(w.N))
-        fe = oracle.external_force_on(x, w.omega, w.g, w.s, j, l)
-        fe0 = oracle.external_force_on(x, w.omega, 0.0, w.s, j, l)
-        assert np.max(np.abs((F[j, l] - F0[j, l]) - (fe - fe0))) <= 1e-9 * fmax
-
-
 def test_stale_gauge_evaluations_match_oracle(binding, oracle):
     """From the second evaluation on, the recursion runs with the previous evaluation's gauge (k_chain_spec).
     Forces after a few MD steps must still match the oracle at the positions reached -- for bosons, for signed
@@ -328,6 +312,8 @@ def test_stale_gauge_evaluations_match_oracle(binding, oracle):
         xs = xg.cpu().numpy()
         Fo, vbo, sgo = oracle.forces(xs, w.beta, w.omega, w.g, w.s, w.xi)
         sim.close()
+        if w.xi < 0:
+            tol = RTOL * oracle.conditioning(xs, w.beta, w.xi)
         assert sg == sgo
         assert abs(vb - vbo) <= tol * abs(vbo)
         check_forces(F.cpu().numpy(), Fo, tol)
@@ -397,7 +383,7 @@ def test_materialised_matrices_match_oracle(binding, oracle, case):
     assert np.all(np.tril(E, -1) == 0.0)
     assert np.max(np.abs(E - np.triu(Eo))) <= 1e-10 * np.max(np.abs(Eo))
     Pro = oracle.pr_matrix(x, beta, xi)
-    tol = 1e-9 if xi >= 0 else 1e-7
+    tol = 1e-9 if xi >= 0 else 1e-9 * oracle.conditioning(x, beta, xi)
     assert np.max(np.abs(Pr - Pro)) <= tol
     np.testing.assert_allclose(Pr.sum(axis=1), 1.0, atol=10 * tol)
     np.testing.assert_allclose(Pr.sum(axis=0), 1.0, atol=10 * tol)
@@ -432,36 +418,49 @@ def test_materialised_matrices_full_size(binding):
         assert abs(lhs - rhs) <= 1e-9 * abs(lhs)
 
 
-@pytest.mark.parametrize("xi,thermostat", [(1.0, 1), (0.0, 1), (1.0, 2)], ids=["bosons_langevin", "distinguishable_langevin", "bosons_nhc"])
-def test_ensemble_energy_matches_exact_ideal_gas(binding, xi, thermostat):
-    """BASELINE config 1 (N = 4, P = 16, beta = 2, non-interacting): the sampled primitive and virial energies of the
-    CUDA path agree with the exact finite-P canonical value (oracle/ideal_gas.py) within 3
-    standard errors (block averages over independent seeds), and with each other."""
+@pytest.mark.parametrize("xi,thermostat", [(1.0, 1), (0.0, 1), (1.0, 2), (0.0, 2)],
+                         ids=["bosons_langevin", "distinguishable_langevin", "bosons_nhc", "distinguishable_nhc"])
+def test_ensemble_energy_matches_exact_ideal_gas_and_oracle(binding, oracle, xi, thermostat):
+    """BASELINE config 1 (N = 4, P = 16, beta = 2, non-interacting): 64 independent replicas (one batch, own seeds and
+    initial states), 5e3 steps of equilibration, 3e5 sampled steps each with the estimators every 10 steps (pimd_run).
+    One mean per replica, so the standard error is that of 64 independent numbers.  north_star: the primitive and the
+    virial energy agree with the exact finite-P canonical value (oracle/ideal_gas.py) within 3
+    standard errors -- no further slack -- and with the same run through the oracle's orc_step (smaller budget) within 3
+    combined standard errors."""
     from oracle import ideal_gas
 
+    B = 64
     w = wl.WORKLOADS["cfg1"].with_(xi=xi)
     exact = ideal_gas.exact_energy(w.N, w.beta, w.omega, w.d, xi, w.P)
-    prim, vir = [], []
-    for seed in range(6):
-        x, v = wl.make_state(w, seed)
-        sim = binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=thermostat, seed=100 + seed)
-        sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
-        sim.step(4000)  # equilibration
-        ep_b, ev_b = [], []
-        for _ in range(8):      # 8 blocks of 250 samples, 10 steps apart
-            ep, ev = 0.0, 0.0
-            for _ in range(250):
-                sim.step(10)
-                a, b, _ = sim.estimators()
-                ep += a; ev += b
-            ep_b.append(ep / 250); ev_b.append(ev / 250)
-        sim.close()
-        prim += ep_b; vir += ev_b
-    for vals in (prim, vir):
-        vals = np.asarray(vals)
-        mean, se = vals.mean(), vals.std(ddof=1) / np.sqrt(len(vals))
-        assert abs(mean - exact) <= 3.0 * se + 0.01 * abs(exact), (mean, se, exact)
-        assert se < 0.1 * abs(exact)
+    xs, vs = zip(*[wl.make_state(w, 1000 + b) for b in range(B)])
+    sim = binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, [xi] * B, w.dt, thermostat=thermostat,
+                       seed=[5000 + b for b in range(B)])
+    sim.set_state(torch.from_numpy(np.stack(xs)).cuda(), torch.from_numpy(np.stack(vs)).cuda())
+    sim.step(5000)
+    sim.run(300000, est_every=10)
+    n, sp, sv, _, _ = sim.read_accumulators()
+    sim.close()
+    assert np.all(n == 30000)
+    # the oracle on a smaller budget: 12 seeds, 2e3 + 3e4 steps
+    o_p, o_v = [], []
+    for k in range(12):
+        x, v = wl.make_state(w, 2000 + k)
+        F, _, _ = oracle.forces(x, w.beta, w.omega, w.g, w.s, xi)
+        nhc = np.zeros((4, x.size))
+        oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, xi, w.dt, thermostat, 1.0, 7000 + k, 0, 2000)
+        a = b = 0.0
+        for i in range(3000):
+            oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, xi, w.dt, thermostat, 1.0, 7000 + k, 2000 + 10 * i, 10)
+            ep, ev, _ = oracle.estimators(x, w.beta, w.omega, w.g, w.s, xi)
+            a += ep; b += ev
+        o_p.append(a / 3000); o_v.append(b / 3000)
+    for sums, orc in ((sp, o_p), (sv, o_v)):
+        vals = sums / n
+        mean, se = vals.mean(), vals.std(ddof=1) / np.sqrt(B)
+        omean, ose = np.mean(orc), np.std(orc, ddof=1) / np.sqrt(len(orc))
+        assert se <= 0.005 * abs(exact), (mean, se, exact)      # the run is long enough to mean something
+        assert abs(mean - exact) <= 3.0 * se, (mean, se, exact)
+        assert abs(mean - omean) <= 3.0 * np.hypot(se, ose), (mean, se, omean, ose)
 
 
 def test_graph_replay_matches_step_by_step(binding):

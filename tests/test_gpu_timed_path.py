@@ -169,14 +169,14 @@ def test_identical_rings_closed_form_with_stale_gauge_n40000(binding):
 def test_set_state_on_a_used_handle(binding, oracle):
     """The gauge of the last evaluation survives pimd_set_state.  States that differ from the previous one
     by 0.3 .. 2 length units per bead, and a different seed of the same workload, must come out right: either the stale
-    gauge is accepted and exact to 1e-9, or it is rejected (acceptance band 2^+-8) and the max-plus pass runs."""
+    gauge is accepted and exact to 1e-9, or it is rejected (acceptance band 2^+-64) and the max-plus pass runs."""
     w = wl.custom(700, 8, d=2, beta=3.0, g=0.2, xi=1.0, init="ring", sigma=2.0)
     x, v = wl.make_state(w, 0)
     sim = make(binding, w)
     sim.set_state(torch.from_numpy(x).cuda())
     sim.forces()
     rng = np.random.default_rng(17)
-    states = [x + rng.normal(0.0, a, size=x.shape) for a in (0.05, 0.3, 1.0, 2.0)]
+    states = [x + rng.normal(0.0, a, size=x.shape) for a in (0.05, 0.3, 1.0, 2.0, 6.0)]
     states += [wl.make_state(w, 1)[0], x + rng.normal(0.0, 0.3, size=(1,) + x.shape[1:])]   # other seed; rigid particle moves
     for y in states:
         y = np.ascontiguousarray(y)
