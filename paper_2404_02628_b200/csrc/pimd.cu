@@ -343,10 +343,16 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
     CU(cudaGetLastError());
     if (h->g != 0.0) {
         // pair forces, added to F (Newton's third law, one potential evaluation per unordered pair)
-        const int NT = (h->N + 31) / 32;
+        // From N = 1500 on: super-tiles of 64 particles, two row particles per lane (k_pair2: half the shared-memory and
+        // shuffle traffic per pair; measured cfg3 0.0804 -> 0.0738 ms, cfg5b 1.199 -> 1.089 ms alone, but cfg4 (N = 1000)
+        // 0.0398 -> 0.0422 and cfg2 0.0087 -> 0.0137: too few warps).  PIMD_PAIR2=0/1 forces one or the other.
+        bool two_rows = h->N >= 1500;
+        if (const char *e = std::getenv("PIMD_PAIR2")) two_rows = std::atoi(e) != 0;
+        const int NT = two_rows ? (h->N + 63) / 64 : (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
-        // offsets per task: small tasks balance small grids (measured: 1 is best up to N = 2500, 4 at N = 10000; tuning knob PIMD_PAIR_CH)
-        int target = NT <= 100 ? 1 : (NT <= 200 ? 2 : 4);
+        // tile offsets per task: small tasks balance the grid (one-row kernel: 1 is best up to N = 2500, 4 at N = 10000;
+        // two-row kernel: 1 throughout, cfg5b 1.089 / 1.152 / 1.284 ms with 1 / 2 / 4); tuning knob PIMD_PAIR_CH
+        int target = two_rows ? 1 : (NT <= 100 ? 1 : (NT <= 200 ? 2 : 4));
         if (const char *e = std::getenv("PIMD_PAIR_CH")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) target = v; }
         const int nchunk = hmax > 0 ? std::max(1, (hmax + target / 2) / target) : 0;
         const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
@@ -356,7 +362,11 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         const double coef = h->pot == 0 ? 2.0 * h->g / (h->s * h->Pg) : h->g / (h->s * h->s * h->Pg);
         const double gE = h->pot == 0 ? h->g : h->g / h->s;
         ProfScope ps(h, PIMD_PROF_PAIR, st);
-#define LP(E, POT) k_pair<D, E, POT><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, gE, h->est, h->rstride)
+#define LP(E, POT)                                                                                                                    \
+    do {                                                                                                                              \
+        if (two_rows) k_pair2<D, E, POT><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, gE, h->est, h->rstride); \
+        else k_pair<D, E, POT><<<pgrid, PAIR_WARPS * 32, 0, st>>>(h->x, h->F, h->N, NT, nchunk, ch, 1.0 / h->s, coef, gE, h->est, h->rstride);           \
+    } while (0)
         if (h->pot == 0) { if (est) LP(true, 0); else LP(false, 0); }
         else { if (est) LP(true, 1); else LP(false, 1); }
 #undef LP

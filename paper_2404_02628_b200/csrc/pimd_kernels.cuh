@@ -2295,6 +2295,154 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
 }
 
 // ==========================================================================================
+// The same pair forces with TWO row particles per lane.  Tiles of 32 are paired into super-tiles of 64
+// (S covers tiles 2S, 2S+1); the cyclic scheme runs over super-tiles.  Lane t keeps particles 64S + t and 64S + 32 + t
+// and meets, at step k, column (t + k) mod 32 of both tiles of the partner super-tile: four potential evaluations per
+// step (four independent exponential chains), every column position loaded once for two rows and every travelling
+// column accumulator shuffled once for two contributions -- per pair half the LDS and SHFL traffic of k_pair, which was
+// bound by the issue port (40 warp instructions per pair, 16 of them FP64; profiles/r1_notes.md).
+// The diagonal task of a super-tile does its two 32 x 32 diagonal tiles the plain way and the cross tile with
+// Newton's third law.  grid (ceil(tasks/PAIR_WARPS), P, B), tasks = NS (nchunk + 1), NS = ceil(NT / 2).
+// ==========================================================================================
+template <int D, bool EST, int POT>
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair2(const double *__restrict__ x, double *__restrict__ F, int N, int NS,
+                                                          int nchunk, int ch, double inv_s, double coef, double g,
+                                                          EstAccum *est, size_t rs)
+{
+    x = rshift(x, (size_t)blockIdx.z * rs); F = rshift(F, (size_t)blockIdx.z * rs);
+    if constexpr (EST) est = rshift(est, (size_t)blockIdx.z * rs);
+    __shared__ double tiles[PAIR_WARPS][2][64 * D];
+    __shared__ double tab[256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int k = threadIdx.x; k < 256; k += PAIR_WARPS * 32) tab[k] = g_exp2_256[k];
+    __syncthreads();
+    const int task = blockIdx.x * PAIR_WARPS + warp;
+    if (task >= NS * (nchunk + 1)) return; // warp-uniform; no block-wide barrier below
+    const int S = task / (nchunk + 1), c = task - S * (nchunk + 1);
+    const size_t sl = (size_t)blockIdx.y * N * D;
+    const double *xs = x + sl;
+    double *Fs = F + sl;
+    double *tA = tiles[warp][0], *tB = tiles[warp][1];
+    const double *tlA = tA + lane * D, *tlB = tB + lane * D;
+
+    const int ia = S * 64 + lane, ib = ia + 32;
+    const bool va = ia < N, vb = ib < N;
+    Vec<D> ra, rb, fa, fb;
+#pragma unroll
+    for (int k = 0; k < D; ++k) { ra.v[k] = 1e150; rb.v[k] = 1e150; fa.v[k] = 0.0; fb.v[k] = 0.0; }
+    if (va) {
+        ra = ldvec<D>(xs, ia);
+#pragma unroll
+        for (int k = 0; k < D; ++k) ra.v[k] *= inv_s;
+    }
+    if (vb) {
+        rb = ldvec<D>(xs, ib);
+#pragma unroll
+        for (int k = 0; k < D; ++k) rb.v[k] *= inv_s;
+    }
+    double se = 0.0, sea = 0.0;
+
+    auto stage = [&](double *dst, int J) { // tile J of 32 particles, twice over (rotation by compile-time offsets)
+        const int jx = J * 32 + lane;
+        Vec<D> p;
+#pragma unroll
+        for (int k = 0; k < D; ++k) p.v[k] = -1e150;
+        if (jx < N) {
+            p = ldvec<D>(xs, jx);
+#pragma unroll
+            for (int k = 0; k < D; ++k) p.v[k] *= inv_s;
+        }
+#pragma unroll
+        for (int k = 0; k < D; ++k) { dst[lane * D + k] = p.v[k]; dst[(lane + 32) * D + k] = p.v[k]; }
+    };
+    auto flush = [&](int J, int col, const Vec<D> &f) {
+        const int jx = J * 32 + col;
+        if (jx < N) {
+#pragma unroll
+            for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)jx * D + k], coef * f.v[k]);
+        }
+    };
+    const int nxt = (lane + 1) & 31, lastcol = (lane + 31) & 31;
+    Vec<D> zero;
+#pragma unroll
+    for (int k = 0; k < D; ++k) zero.v[k] = 0.0;
+
+    if (c == nchunk) {
+        // diagonal super-tile: tiles (2S, 2S) and (2S+1, 2S+1) as ordered pairs (the self term has dx = 0), tile pair
+        // (2S, 2S+1) once with both partners
+        stage(tA, 2 * S);
+        stage(tB, 2 * S + 1);
+        __syncwarp();
+        double sd = 0.0, sda = 0.0;
+        Vec<D> dummy = zero, fB = zero;
+#pragma unroll 8
+        for (int k = 0; k < 32; ++k) {
+            pair_term<D, EST, POT>(ra, tlA + k * D, tab, fa, dummy, sd, sda);
+            pair_term<D, EST, POT>(rb, tlB + k * D, tab, fb, dummy, sd, sda);
+        }
+#pragma unroll
+        for (int k = 0; k < 32; ++k) {
+            pair_term<D, EST, POT>(ra, tlB + k * D, tab, fa, fB, se, sea);
+            if (k < 31) {
+#pragma unroll
+                for (int q = 0; q < D; ++q) fB.v[q] = shfl_bcast(fB.v[q], nxt);
+            }
+        }
+        flush(2 * S + 1, lastcol, fB);
+        if constexpr (EST) {
+            // ordered pairs count twice and include the self terms u(0) = 1 of the valid rows; pairs with a padding particle
+            // carry u ~ e^-708 (Gaussian) or 0
+            se += 0.5 * (sd - (va ? 1.0 : 0.0) - (vb ? 1.0 : 0.0));
+            sea += 0.5 * sda;
+        }
+    } else {
+        const int H = (NS & 1) ? (NS - 1) / 2 : (NS / 2 - 1 + (S < NS / 2 ? 1 : 0));
+        const int m0 = 1 + c * ch, m1 = min(m0 + ch - 1, H);
+        for (int m = m0; m <= m1; ++m) {
+            int Sp = S + m;
+            if (Sp >= NS) Sp -= NS;
+            __syncwarp();
+            stage(tA, 2 * Sp);
+            stage(tB, 2 * Sp + 1);
+            __syncwarp();
+            Vec<D> fA = zero, fB = zero;
+#pragma unroll
+            for (int k = 0; k < 32; ++k) {
+                pair_term<D, EST, POT>(ra, tlA + k * D, tab, fa, fA, se, sea);
+                pair_term<D, EST, POT>(rb, tlA + k * D, tab, fb, fA, se, sea);
+                pair_term<D, EST, POT>(ra, tlB + k * D, tab, fa, fB, se, sea);
+                pair_term<D, EST, POT>(rb, tlB + k * D, tab, fb, fB, se, sea);
+                if (k < 31) {
+#pragma unroll
+                    for (int q = 0; q < D; ++q) {
+                        fA.v[q] = shfl_bcast(fA.v[q], nxt);
+                        fB.v[q] = shfl_bcast(fB.v[q], nxt);
+                    }
+                }
+            }
+            flush(2 * Sp, lastcol, fA);
+            flush(2 * Sp + 1, lastcol, fB);
+        }
+    }
+    if (va) {
+#pragma unroll
+        for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)ia * D + k], coef * fa.v[k]);
+    }
+    if (vb) {
+#pragma unroll
+        for (int k = 0; k < D; ++k) atomicAdd(&Fs[(size_t)ib * D + k], coef * fb.v[k]);
+    }
+    if constexpr (EST) {
+        se = warp_sum(se);
+        sea = warp_sum(sea);
+        if (lane == 0) {
+            atomicAdd(&est->upair, g * se);
+            atomicAdd(&est->virpair, g * (se + sea));
+        }
+    }
+}
+
+// ==========================================================================================
 // Step 8: the estimators of one configuration from the sums the force kernels left behind (R9)
 //   e_prim = P d N/(2 beta) - <E_c> + Ubar,  e_vir = Ubar + 1/2 sum r . grad Ubar,  Ubar = U/P
 // and, when `accumulate` is set (pimd_run), their running sums and the running histograms.  One block per replica.
