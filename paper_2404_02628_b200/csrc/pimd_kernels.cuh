@@ -831,6 +831,8 @@ constexpr int SPEC_NCOL = (32 + SPEC_NHW - 1) / SPEC_NHW;  // columns of a tile 
 #ifndef PIMD_FACT_LIMIT
 #define PIMD_FACT_LIMIT 1024.0
 #endif
+// doubles per column entry of the helpers' tables: A_p, sigma'_p[D], t_p, dl_p, padded to an even count (LDS.128 reads)
+__host__ __device__ constexpr int SPEC_CW(int D) { return (3 + D + 1) / 2 * 2; }
 constexpr double SKIP_BELOW = -260.0;           // helper batches whose entries all lie below e^SKIP_BELOW of the row's gauge are dropped
 constexpr double FACT_LIMIT = PIMD_FACT_LIMIT; // largest tabulated term for which the factorised exponent arguments are used
 
@@ -856,8 +858,8 @@ template <int D> struct SpecSmem {
         baseP = o; o += 2 * 32;       // scaled panel for block B & 1
         zmail = o; o += 2 * 32;       // Zhat of the columns block B & 1 produced, for the io warp
         kacc = o; o += 4;             // int[8]: power of two taken out of Zhat up to the start of block B & 7
-        fmode = o; o += 1;            // int[2]: the tables of window & 1 hold the factorised terms (1) or the plain pieces (0)
-        ctab = o; o += 2 * 4 * 32 * (3 + D); // [window & 1][set][column]: (A_p, sigma'_p, t_p, dl_p), see col_row_terms
+        fmode = o; o += 2;            // int[2] (two doubles: what follows stays 16-byte aligned): the tables of window & 1 hold the factorised terms (1) or the plain pieces (0)
+        ctab = o; o += 2 * 4 * 32 * SPEC_CW(D); // [window & 1][set][column]: (A_p, sigma'_p, t_p, dl_p) padded to whole double2, see col_row_terms
         rtab = o; o += 2 * 2 * 32 * (2 + 2 * D); // [window & 1][set][row]: (B_r, 2 kk rho'_r, G_r, rho'_r)
         total = o;
     }
@@ -962,7 +964,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
     //     ((t_p - G_r) + dl_p) - kk |rho'_r - sigma'_p|^2,   t_p, G_r float-valued so that their difference is exact,
     // 3 + 2 D instructions with the accuracy of the max-plus kernel (measured: forces 1.4e-9 -> see profiles/r2_notes.md).
     auto col_row_terms = [&](int K) {
-        constexpr int W = 2 + 2 * D, CW = 3 + D;
+        constexpr int W = 2 + 2 * D, CW = SPEC_CW(D);
         double *cA = ctab_s + (K & 1) * (4 * 32 * CW), *rA = rtab_s + (K & 1) * (2 * 32 * W);
         const int B2 = K + 2, B3 = K + 3, b2 = B2 & 7, b3 = B3 & 7;
         Vec<D> o2, o3;
@@ -1030,19 +1032,31 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
     };
     // one entry's exponent argument from the column's and the row's table entries (cp, rp):
     // factorised, A_p + B_r + sum_c w_c sigma'_c -- final in a `fact` window, else good to ~1e-11, enough to tell a dead batch
-    auto entry_arg = [&](const double *cp, const double *rp) {
-        double t = cp[0] + rp[0];
+    // Table entries are read as double2 (LDS.128): the helpers' shared-memory instructions, not their arithmetic, set
+    // the block time (the SM has one pipe for LDS, STS and the dependent warp's shuffles).
+    auto ld_entry = [&](const double *q, double *v, int nd2) {
 #pragma unroll
-        for (int c = 0; c < D; ++c) t = fma(rp[1 + c], cp[1 + c], t);
+        for (int k = 0; k < 4; ++k) {
+            if (k < nd2) { const double2 t = *reinterpret_cast<const double2 *>(q + 2 * k); v[2 * k] = t.x; v[2 * k + 1] = t.y; }
+        }
+    };
+    auto entry_arg = [&](const double *cp, const double *rp) {
+        double c[8];
+        ld_entry(cp, c, (D + 2) / 2); // A_p, sigma'_p
+        double t = c[0] + rp[0];
+#pragma unroll
+        for (int k = 0; k < D; ++k) t = fma(rp[1 + k], c[1 + k], t);
         return t;
     };
     // direct, ((t_p - G_r) + dl_p) - kk |rho'_r - sigma'_p|^2
     auto entry_arg_direct = [&](const double *cp, const double *rp) {
-        double dd = rp[2 + D] - cp[1];
+        double c[8];
+        ld_entry(cp, c, (D + 4) / 2); // sigma'_p, t_p, dl_p
+        double dd = rp[2 + D] - c[1];
         double r2 = dd * dd;
 #pragma unroll
-        for (int c = 1; c < D; ++c) { dd = rp[2 + D + c] - cp[1 + c]; r2 = fma(dd, dd, r2); }
-        return fma(-kk, r2, (cp[1 + D] - rp[1 + D]) + cp[2 + D]);
+        for (int k = 1; k < D; ++k) { dd = rp[2 + D + k] - c[1 + k]; r2 = fma(dd, dd, r2); }
+        return fma(-kk, r2, (c[1 + D] - rp[1 + D]) + c[2 + D]);
     };
     auto batch_is_live = [&](const double *arg) {
         bool live = false;
@@ -1051,7 +1065,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
         return __any_sync(0xffffffffu, live) != 0;
     };
     auto helper_tasks = [&](int K, int hw) {
-        constexpr int CW = 3 + D, RW = 2 + 2 * D;
+        constexpr int CW = SPEC_CW(D), RW = 2 + 2 * D;
         const bool fact = fmode_s[(K + 1) & 1] != 0; // mode of the tables this window reads (warp-uniform)
         const bool tht = phase != nullptr && dir == 0 && lane == 0 && hw == 0;
         const long long ht0 = clock64();
@@ -1072,7 +1086,9 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
                 } else {
                     p = 31 - (lane & 15); r = 31; // 16 leftovers (each written twice, same value)
                 }
-                arg[k] = fact ? entry_arg(cA + p * CW, rA + r * RW) : entry_arg_direct(cA + p * CW, rA + r * RW);
+                double rr[8];
+                ld_entry(rA + r * RW, rr, fact ? (D + 2) / 2 : (2 + 2 * D) / 2);
+                arg[k] = fact ? entry_arg(cA + p * CW, rr) : entry_arg_direct(cA + p * CW, rr);
                 idx[k] = (pass <= 16) ? p * 32 + r : -1;
             }
 #pragma unroll
@@ -1089,9 +1105,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
         {   // ---- base(K+1)
             const int B = K + 1;
             const double *cA = ctab_s + ((K + 1) & 1) * (4 * 32 * CW), *rA = rtab_s + ((K + 1) & 1) * (2 * 32 * RW) + lane * RW;
-            double rt[1 + D];
-#pragma unroll
-            for (int c = 0; c < 1 + D; ++c) rt[c] = rA[c];
+            double rt[8];
+            ld_entry(rA, rt, (D + 2) / 2);
             // both older column blocks as one batch, so that eight independent exponentials are in flight
             double arg[2][SPEC_NCOL], z[2][SPEC_NCOL];
 #pragma unroll
@@ -1111,13 +1126,15 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
                 atomicAdd(reinterpret_cast<unsigned long long *>(&ph_s[11]), two ? 2ull : 1ull);
                 atomicAdd(reinterpret_cast<unsigned long long *>(&ph_s[12]), (live0 ? 0ull : 1ull) + ((two && !live1) ? 1ull : 0ull));
             }
-            if (!fact) { // live batches get their arguments the direct way
+            if (!fact && (live0 || live1)) { // live batches get their arguments the direct way
+                double rr[8];
+                ld_entry(rA, rr, (2 + 2 * D) / 2);
 #pragma unroll
                 for (int qq = 0; qq < 2; ++qq) {
                     if (qq ? live1 : live0) {
 #pragma unroll
                         for (int k = 0; k < SPEC_NCOL; ++k)
-                            arg[qq][k] = entry_arg_direct(cA + ((2 + qq) * 32 + min(hw + SPEC_NHW * k, 31)) * CW, rA);
+                            arg[qq][k] = entry_arg_direct(cA + ((2 + qq) * 32 + min(hw + SPEC_NHW * k, 31)) * CW, rr);
                     }
                 }
             }
@@ -1148,9 +1165,8 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
         {   // ---- E'(K+2)
             const int B = K + 2;
             const double *cA = ctab_s + ((K + 1) & 1) * (4 * 32 * CW) + 32 * CW, *rA = rtab_s + ((K + 1) & 1) * (2 * 32 * RW) + (32 + lane) * RW;
-            double rt[1 + D];
-#pragma unroll
-            for (int c = 0; c < 1 + D; ++c) rt[c] = rA[c];
+            double rt[8];
+            ld_entry(rA, rt, (D + 2) / 2);
             double *uB = ue_s + (B & 1) * 1024;
             double arg[SPEC_NCOL];
 #pragma unroll
@@ -1168,8 +1184,10 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
             }
             if (live) {
                 if (!fact) {
+                    double rr[8];
+                    ld_entry(rA, rr, (2 + 2 * D) / 2);
 #pragma unroll
-                    for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = entry_arg_direct(cA + min(hw + SPEC_NHW * k, 31) * CW, rA);
+                    for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = entry_arg_direct(cA + min(hw + SPEC_NHW * k, 31) * CW, rr);
                 }
 #pragma unroll
                 for (int k = 0; k < SPEC_NCOL; ++k) arg[k] = exp_cap_tab64(arg[k], etab64);
