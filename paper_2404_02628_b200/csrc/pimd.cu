@@ -204,6 +204,7 @@ size_t carve(pimd_t h, unsigned char *base)
                 c.p.pan_s[dir] = (double *)take(n * 8);
                 c.p.panel_ready[dir] = (int *)take((size_t)c.NB * 4);
                 c.p.acc[dir] = (double *)take(n * (D + 2) * 8);
+                c.p.pacc[dir] = (double *)take(n * (D + 1) * 8);
             }
             c.p.cols_ready = (int *)take(2 * 4);
             c.p.eint = (double *)take(n * 8);
@@ -435,27 +436,18 @@ template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t
         }
         c.gauge_valid = true;
         c.history++;
-        const int NT = (c.N + FP_TB - 1) / FP_TB;
-        // NT (NT+1) tiles at or below the diagonal (both directions); with fewer than 8 per SM one thread per row leaves
-        // the kernel latency bound, so four threads share a row (measured at cfg3: 0.023 -> 0.017 ms)
-        const long long tiles = (long long)NT * (NT + 1) * h->B;
-        const bool wide = tiles < 8LL * h->sms;
-        const dim3 fgrid(wide ? (c.N + FP_TB / 4 - 1) / (FP_TB / 4) : NT, NT, 2 * h->B);
+        // the near-diagonal band of LOOK + 1 column blocks per row block; the panel workers delivered the rest (App. A.3)
         {
             ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
-            if (wide) {
-                if (sgn) k_forcepass<D, true, 4><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
-                else k_forcepass<D, false, 4><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
-            } else {
-                if (sgn) k_forcepass<D, true, 1><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
-                else k_forcepass<D, false, 1><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->rstride);
-            }
+            const dim3 fgrid(c.NB, 2 * h->B);
+            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->look, h->rstride);
+            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->look, h->rstride);
         }
         CU(cudaGetLastError());
         {
             ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
-            if (sgn) k_assemble<D, true, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->rstride);
-            else k_assemble<D, false, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->rstride);
+            if (sgn) k_assemble<D, true, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->look, h->rstride);
+            else k_assemble<D, false, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->look, h->rstride);
         }
         CU(cudaGetLastError());
     }
@@ -790,8 +782,8 @@ static int create_impl(pimd_t *out, int B, int rank, int world, int N, int P, in
     h->ndof = h->slice * h->P;
     h->nspecies = 1;
     h->counts[0] = N;
-    h->look = 2;
-    h->look_spec = 3;
+    h->look = 3;      // column blocks kept inside the chain CTA: the same for the max-plus and the stale-gauge recursion,
+    h->look_spec = 3; // because the force pass covers exactly those blocks and the workers' panels everything older
     if (const char *e2 = std::getenv("PIMD_LOOK")) { // tuning knob: column blocks kept inside the chain CTA
         const int v = std::atoi(e2);
         if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;

@@ -180,6 +180,7 @@ struct ExchPtrs {
     int *cols_ready;      // [2]
     int *panel_ready[2];  // [NB]
     double *acc[2];       // [N][D+2]: sum w, sum w*sig (D), sum w*kk*r2
+    double *pacc[2];      // [N][D+1]: the panel's share of sum w*sig (D) and sum w*kk*r2 per row, in the units of (pan_m, pan_s)
     double *eint, *cnext, *cself, *pnext;
     double *tpart;        // [2*nprepblocks] per-block partial sums of E_int, cnext
     double2 *rfin;        // [2]
@@ -202,7 +203,7 @@ PIMD_DEV ExchPtrs rshift(ExchPtrs p, size_t off)
         p.rho[k] = rshift(p.rho[k], off); p.sig[k] = rshift(p.sig[k], off); p.cc[k] = rshift(p.cc[k], off);
         p.g[k] = rshift(p.g[k], off); p.gs[k] = rshift(p.gs[k], off); p.gprev[k] = rshift(p.gprev[k], off);
         p.pan_m[k] = rshift(p.pan_m[k], off); p.pan_s[k] = rshift(p.pan_s[k], off);
-        p.panel_ready[k] = rshift(p.panel_ready[k], off); p.acc[k] = rshift(p.acc[k], off);
+        p.panel_ready[k] = rshift(p.panel_ready[k], off); p.acc[k] = rshift(p.acc[k], off); p.pacc[k] = rshift(p.pacc[k], off);
     }
     p.cols_ready = rshift(p.cols_ready, off);
     p.eint = rshift(p.eint, off); p.cnext = rshift(p.cnext, off); p.cself = rshift(p.cself, off); p.pnext = rshift(p.pnext, off);
@@ -272,11 +273,6 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
             p.cc[1][N - 2 - l] = c;
         }
         p.cnext[l] = cn;
-#pragma unroll
-        for (int c = 0; c < D + 2; ++c) {
-            p.acc[0][(size_t)l * (D + 2) + c] = 0.0;
-            p.acc[1][(size_t)l * (D + 2) + c] = 0.0;
-        }
         if (l < NB) { p.panel_ready[0][l] = 0; p.panel_ready[1][l] = 0; }
 #pragma unroll
         for (int dir = 0; dir < 2; ++dir) { // k_chain_spec reads the panel words as their own flags
@@ -385,7 +381,7 @@ template <int D> struct ChainSmem {
 template <int D> size_t chain_smem_bytes_host(int look)
 {
     const size_t chain = ChainSmem<D>(look).total * 8;
-    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
+    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16 + (size_t)CH_WARPS * 32 * 8 * (D + 1);
     return chain > worker ? chain : worker;
 }
 
@@ -1427,6 +1423,7 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, u
     double *st_sig = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + CH_WARPS * 32 + warp * 32 * D;
     double *mg_m = reinterpret_cast<double *>(reinterpret_cast<double2 *>(smem_raw) + CH_WARPS * 32) + CH_WARPS * 32 + CH_WARPS * 32 * D;
     double *mg_s = mg_m + CH_WARPS * 32;
+    double *mg_q = mg_s + CH_WARPS * 32; // [D + 1][CH_WARPS * 32]
 
     const double *rho = rshift(a.p.rho[dir], roff), *sig = rshift(a.p.sig[dir], roff);
     const double2 *g = rshift(a.p.g[dir], roff);
@@ -1459,6 +1456,13 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, u
         const bool rows_small = __any_sync(0xffffffffu, i < N && !(-rowB < FACT_LIMIT)) == 0;
         const int ntile = K - LOOK;
         Lse acc = lse_empty();
+        // the terms w = Zhat_p exp(tau - m) of the row sum are the very weights of Eq. 15/16 (up to a factor
+        // per row that the other direction's table fixes afterwards), so sum w sigma_p and sum w beta C ride along: the
+        // panel's share of the exterior forces and of <E_c> costs D + 3 more FP64 instructions per entry here instead of a
+        // second sweep with one more exponential per entry (k_forcepass then covers only the LOOK + 1 newest column blocks)
+        double tq[D + 1];
+#pragma unroll
+        for (int c = 0; c < D + 1; ++c) tq[c] = 0.0;
         double2 ref = make_double2(0.0, 0.0);
         // unit of work = 8 columns; chunk c goes to warp c mod 16, so the four chunks of the newest tile (the
         // ones the chain is waiting for) are done by four warps at once
@@ -1552,16 +1556,33 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, u
             // maximum as a tree (three levels instead of a chain of eight)
             const double cm = fmax(fmax(fmax(tau[0], tau[1]), fmax(tau[2], tau[3])), fmax(fmax(tau[4], tau[5]), fmax(tau[6], tau[7])));
             if (cm > acc.m) {
-                acc.s *= exp_neg_tab64(-(acc.m - cm), etab64);
+                const double f = exp_neg_tab64(-(acc.m - cm), etab64);
+                acc.s *= f;
+#pragma unroll
+                for (int c = 0; c < D + 1; ++c) tq[c] *= f;
                 acc.m = cm;
             }
-            double s0 = 0.0, s1 = 0.0;
+            double s0 = 0.0, s1 = 0.0, q0[D + 1], q1[D + 1];
+#pragma unroll
+            for (int c = 0; c < D + 1; ++c) { q0[c] = 0.0; q1[c] = 0.0; }
 #pragma unroll
             for (int k = 0; k < 8; k += 2) {
-                s0 = fma(exp_neg_tab64(-(tau[k] - acc.m), etab64), st_sg[k], s0);
-                s1 = fma(exp_neg_tab64(-(tau[k + 1] - acc.m), etab64), st_sg[k + 1], s1);
+                const double w0 = exp_neg_tab64(-(tau[k] - acc.m), etab64) * st_sg[k];
+                const double w1 = exp_neg_tab64(-(tau[k + 1] - acc.m), etab64) * st_sg[k + 1];
+                s0 += w0;
+                s1 += w1;
+#pragma unroll
+                for (int c = 0; c < D; ++c) {
+                    q0[c] = fma(w0, st_sig[k * D + c], q0[c]);
+                    q1[c] = fma(w1, st_sig[(k + 1) * D + c], q1[c]);
+                }
+                // beta C = kk |rho - sigma|^2 = (T_p - T_ref) - tau
+                q0[D] = fma(w0, st_g[8 + k].y - tau[k], q0[D]);
+                q1[D] = fma(w1, st_g[8 + k + 1].y - tau[k + 1], q1[D]);
             }
             acc.s += s0 + s1;
+#pragma unroll
+            for (int c = 0; c < D + 1; ++c) tq[c] += q0[c] + q1[c];
             __syncwarp();
         }
         // common reference of the published partial: g_{32 ntile} (first "recent" column of block K)
@@ -1584,23 +1605,42 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, u
         }
         mg_m[warp * 32 + lane] = acc.m;
         mg_s[warp * 32 + lane] = acc.s;
+#pragma unroll
+        for (int c = 0; c < D + 1; ++c) mg_q[(c * CH_WARPS + warp) * 32 + lane] = tq[c];
         __syncthreads();
         if (warp == 0) {
             // 16 partials per row: maximum first, then 16 independent exponentials
             Lse t = lse_empty();
 #pragma unroll
             for (int w = 0; w < CH_WARPS; ++w) t.m = fmax(t.m, mg_m[w * 32 + lane]);
+            double fw[CH_WARPS];
+#pragma unroll
+            for (int w = 0; w < CH_WARPS; ++w) fw[w] = 0.0;
             if (t.m > -INFINITY) {
 #pragma unroll
-                for (int w = 0; w < CH_WARPS; ++w) t.s = fma(mg_s[w * 32 + lane], exp_neg_tab64(-(mg_m[w * 32 + lane] - t.m), etab64), t.s);
+                for (int w = 0; w < CH_WARPS; ++w) {
+                    fw[w] = exp_neg_tab64(-(mg_m[w * 32 + lane] - t.m), etab64);
+                    t.s = fma(mg_s[w * 32 + lane], fw[w], t.s);
+                }
             }
-            if (i < N) {
+            if (i < N) { // the chain is waiting for these two words
                 st_relaxed_f64(&rshift(a.p.pan_m[dir], roff)[i], t.m);
                 st_relaxed_f64(&rshift(a.p.pan_s[dir], roff)[i], t.s);
             }
             // no fence: bar.warp.sync + st.release.gpu is cumulative over the other lanes' stores
             __syncwarp();
             if (lane == 0) st_release(&rshift(a.p.panel_ready[dir], roff)[K], 1);
+            // the force sums of the panel, same units (k_assemble scales them); sigma' was taken about the block's origin
+            if (i < N) {
+                double *pq = rshift(a.p.pacc[dir], roff) + (size_t)i * (D + 1);
+#pragma unroll
+                for (int c = 0; c < D + 1; ++c) {
+                    double q = 0.0;
+#pragma unroll
+                    for (int w = 0; w < CH_WARPS; ++w) q = fma(mg_q[(c * CH_WARPS + w) * 32 + lane], fw[w], q);
+                    pq[c] = (c < D) ? fma(org.v[c < D ? c : 0], t.s, q) : q;
+                }
+            }
         }
         __syncthreads();
     }
@@ -1659,7 +1699,7 @@ __global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
 template <int D> size_t chain_spec_smem_bytes_host()
 {
     const size_t chain = SpecSmem<D>().total * 8;
-    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16;
+    const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16 + (size_t)CH_WARPS * 32 * 8 * (D + 1);
     return chain > worker ? chain : worker;
 }
 
@@ -1667,37 +1707,34 @@ template <int D> size_t chain_spec_smem_bytes_host()
 // Step 6: connection probabilities (Eq. 12) and the sums the
 // exterior-bead forces need (Eq. 15, 16), no N x N storage:
 //   Pr[l -> l'] = sg exp( qhat[l] + a[l'] - kk |r_l^P - r_l'^1|^2 - R_N ),  l' <= l
-// In generic form, for direction dir and lane row i:
+// In generic form, for direction dir and row i:
 //   w_ij = exp( g^{other}[N-1-i] + g^{dir}[j] - kk |rho_i - sig_j|^2 - R_N ),  j <= i
-//   acc[dir][i] = ( sum_j w, sum_j w sig_j, sum_j w kk r^2 )
+//   acc[dir][i] = ( sum_j w, sum_j w sig_j, sum_j w kk r2 )
 // dir 0 gives the row sums (bead P, Eq. 16), dir 1 the column sums (bead 1, Eq. 15).
-// grid (NT, NT, 2 B) over 128 x 128 tiles of the lower triangle; block 128.
+// The terms w_ij are, up to a factor per row, the terms of the recursion's own row sums: the panel
+// workers accumulate sum w sig and sum w kk r2 over all columns older than the LOOK newest blocks while they form the
+// panel (p.pacc), so this kernel covers only the near-diagonal band of (LOOK + 1) column blocks per row block:
+// N (LOOK + 1) 32 entries per direction instead of N^2/2.  grid (NB, 2 B), block 128.
 // ==========================================================================================
 constexpr int FP_TB = 128;
 
-template <int D, bool SGN, int NQ>
-__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, size_t rs)
+template <int D, bool SGN>
+__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, int band, size_t rs)
 {
-    // a CTA of FP_TB threads takes RT rows x FP_TB columns at or below the diagonal.  NQ = 1: RT = FP_TB, one thread per
-    // row walks the tile's columns (large N: enough tiles to fill the GPU).  NQ = 4: RT = 32, four threads per row with 32
-    // columns each, partial sums combined in shared memory before the atomics (small N: a thread per row alone leaves
-    // the SMs with a warp or two each and the kernel latency bound; four times as many, smaller CTAs also spread evenly
-    // over the SMs).
-    constexpr int CW = FP_TB / NQ, RT = FP_TB / NQ;
-    const int rt = blockIdx.x, ct = blockIdx.y, dir = blockIdx.z & 1; // grid.z = 2 * replica + direction
-    const int j0 = ct * FP_TB;
-    if (j0 > rt * RT + RT - 1) return; // above the diagonal
-    p = rshift(p, (size_t)(blockIdx.z >> 1) * rs);
-    // one thread per row (large N): 256-entry table, 8 FP64 instructions per exponential (N=10000 0.202 -> 0.195 ms);
-    // four threads per row (small N, many small CTAs): the 64-entry table, whose fill per CTA is four times cheaper
-    // (cfg3 0.0170 against 0.0173 ms with the large table)
-    constexpr int NTAB = (NQ == 1) ? 256 : 64;
-    __shared__ double etab[NTAB];
-    for (int k = threadIdx.x; k < NTAB; k += blockDim.x) etab[k] = (NQ == 1) ? g_exp2_256[k] : c_exp2_64[k];
+    // A CTA of FP_TB = 128 threads takes one block of RT = 32 rows and the (band + 1) <= 4 newest column blocks of it, the
+    // ones the recursion kept inside its chain CTA (columns j0 = 32 (K - band) .. i); the sums over all older columns come
+    // from the panel workers (p.pacc, added in k_assemble).  Four threads per row with 32 columns each, partial sums
+    // combined in shared memory.  Every row is written by exactly one CTA: plain stores.
+    constexpr int NQ = 4, CW = FP_TB / NQ, RT = FP_TB / NQ;
+    const int rt = blockIdx.x, dir = blockIdx.y & 1; // grid.y = 2 * replica + direction
+    const int j0 = max(0, 32 * (rt - band));
+    p = rshift(p, (size_t)(blockIdx.y >> 1) * rs);
+    __shared__ double etab[64];
+    for (int k = threadIdx.x; k < 64; k += blockDim.x) etab[k] = c_exp2_64[k];
     __shared__ double2 sg_g[FP_TB];
     __shared__ double sg_s[FP_TB];
     __shared__ double sg_sig[FP_TB * D];
-    __shared__ double part_s[(NQ > 1) ? NQ * (D + 2) * RT : 1];
+    __shared__ double part_s[NQ * (D + 2) * RT];
     const double2 *gd = p.g[dir], *go = p.g[1 - dir];
     const int r = threadIdx.x % RT, q = threadIdx.x / RT;
     const int i = rt * RT + r;
@@ -1739,35 +1776,25 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
             const double2 gj = sg_g[k];
             const double kr2 = kk * dist2<D>(pr, pc);
             const double targ = ((A.x + gj.x) + (A.y + gj.y)) - kr2;
-            const double w = ((NQ == 1) ? exp_cap_tab256(targ, etab) : exp_cap_tab64(targ, etab)) * sg_s[k];
+            const double w = exp_cap_tab64(targ, etab) * sg_s[k];
             sw += w;
             swc = fma(w, kr2, swc);
 #pragma unroll
             for (int c = 0; c < D; ++c) sws.v[c] = fma(w, pc.v[c], sws.v[c]);
         }
     }
-    if constexpr (NQ > 1) {
-        part_s[(q * (D + 2)) * RT + r] = osg * sw;
+    part_s[(q * (D + 2)) * RT + r] = osg * sw;
 #pragma unroll
-        for (int c = 0; c < D; ++c) part_s[(q * (D + 2) + 1 + c) * RT + r] = osg * sws.v[c];
-        part_s[(q * (D + 2) + D + 1) * RT + r] = osg * swc;
-        __syncthreads();
-        // thread (r, q) adds up components q, q + NQ, .. of row r
-        if (i < N && i >= j0) {
-            for (int c = q; c < D + 2; c += NQ) {
-                double t = 0.0;
+    for (int c = 0; c < D; ++c) part_s[(q * (D + 2) + 1 + c) * RT + r] = osg * sws.v[c];
+    part_s[(q * (D + 2) + D + 1) * RT + r] = osg * swc;
+    __syncthreads();
+    // thread (r, q) adds up components q, q + NQ, .. of row r
+    if (i < N) {
+        for (int c = q; c < D + 2; c += NQ) {
+            double t = 0.0;
 #pragma unroll
-                for (int qq = 0; qq < NQ; ++qq) t += part_s[(qq * (D + 2) + c) * RT + r];
-                atomicAdd(p.acc[dir] + (size_t)i * (D + 2) + c, t);
-            }
-        }
-    } else {
-        if (ncol > 0) {
-            double *o = p.acc[dir] + (size_t)i * (D + 2);
-            atomicAdd(&o[0], osg * sw);
-#pragma unroll
-            for (int c = 0; c < D; ++c) atomicAdd(&o[1 + c], osg * sws.v[c]);
-            atomicAdd(&o[D + 1], osg * swc);
+            for (int qq = 0; qq < NQ; ++qq) t += part_s[(qq * (D + 2) + c) * RT + r];
+            p.acc[dir][(size_t)i * (D + 2) + c] = t;
         }
     }
 }
@@ -1781,7 +1808,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 // ==========================================================================================
 template <int D, bool SGN, int TB>
 __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, const RepParams *rp, double *Fex1, double *FexP,
-                                                double *ecpart, size_t rs)
+                                                double *ecpart, int band, size_t rs)
 {
     __shared__ double red[TB / 32];
     const size_t off = (size_t)blockIdx.y * rs;
@@ -1791,11 +1818,11 @@ __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, c
     double ec = 0.0;
     if (l < N) {
         const double2 R = p.rfin[0];
-        const double rs = SGN ? p.rsgn[0] : 1.0;
+        const double rs_ = SGN ? p.rsgn[0] : 1.0;
         auto pn = [&](int m) -> double { // Pr[m -> m+1], 0 <= m <= N-2
             const double2 A = dd_sub(p.g[1][N - 1 - m], R);
             const double2 B = p.g[0][m + 1];
-            const double w = exp_fast(((A.x + B.x) + (A.y + B.y)) - p.cnext[m]) * (p.gs[1][N - 1 - m] * p.gs[0][m + 1] * rs);
+            const double w = exp_fast(((A.x + B.x) + (A.y + B.y)) - p.cnext[m]) * (p.gs[1][N - 1 - m] * p.gs[0][m + 1] * rs_);
             return 1.0 - xi * (double)(m + 1) * w;
         };
         const double pl = (l < N - 1) ? pn(l) : 0.0;
@@ -1804,19 +1831,36 @@ __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, c
         const Vec<D> xP = ldvec<D>(p.rho[0], l), x1 = ldvec<D>(p.sig[0], l);
         const double *a0 = p.acc[0] + (size_t)l * (D + 2);
         const double *a1 = p.acc[1] + (size_t)(N - 1 - l) * (D + 2);
+        // The panel's share (band >= 0): the workers left, per row i of direction dir, sum_j w_ij (sig_j, beta C_ij) over
+        // the columns j < jp = 32 (i/32 - band) with w_ij = Zhat_j exp(T_j - T_jp - kk r^2 - m_i); the weight of Eq. 12 is
+        // w_ij Zhat^{other} exp(T_jp + m_i + g^{other}[N-1-i] - R_N)  (the factor a second sweep used to apply entry by entry)
+        double pan[2][D + 1];
+#pragma unroll
+        for (int dir = 0; dir < 2; ++dir) {
+            const int i = dir ? N - 1 - l : l, jp = 32 * (i / 32 - band);
+#pragma unroll
+            for (int c = 0; c < D + 1; ++c) pan[dir][c] = 0.0;
+            if (band >= 0 && jp > 0) {
+                const double2 A = dd_sub(p.g[1 - dir][N - 1 - i], R), Tp = p.g[dir][jp];
+                double f = exp_fast((((A.x + Tp.x) + (A.y + Tp.y)) + p.pan_m[dir][i])) * p.gs[1 - dir][N - 1 - i] * rs_;
+                if (!(fabs(f) < INFINITY)) f = 0.0; // an empty panel (m = -inf) has nothing to add
+#pragma unroll
+                for (int c = 0; c < D + 1; ++c) pan[dir][c] = f * p.pacc[dir][(size_t)i * (D + 1) + c];
+            }
+        }
         Vec<D> fP, f1;
 #pragma unroll
         for (int c = 0; c < D; ++c) {
-            double sP = a0[1 + c];
+            double sP = a0[1 + c] + pan[0][c];
             if (l < N - 1) sP = fma(pl, p.sig[0][(size_t)(l + 1) * D + c], sP);
-            double s1 = a1[1 + c];
+            double s1 = a1[1 + c] + pan[1][c];
             if (l > 0) s1 = fma(pm1, p.rho[0][(size_t)(l - 1) * D + c], s1);
             fP.v[c] = -ks * (xP.v[c] - sP);
             f1.v[c] = -ks * (x1.v[c] - s1);
         }
         stvec<D>(FexP, l, fP);
         stvec<D>(Fex1, l, f1);
-        ec = a0[D + 1] + pl * p.cnext[l];
+        ec = a0[D + 1] + pan[0][D] + pl * p.cnext[l];
     }
     double s = block_sum<TB>(ec, red);
     if (threadIdx.x == 0) ecpart[blockIdx.x] = s;
