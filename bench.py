@@ -29,7 +29,7 @@ UNIT = "steps/s"
 # executes 16 FP64 instructions per pair (SASS: 2 differences, 2 for r^2, 8 table exponential, 4 force FMAs)
 FLOP_PER_PAIR = 50.0
 FLOP_PER_PAIR_EXECUTED = 32.0
-FLOP_PER_ELEMENT = 54.0   # force pass: 27 FP64 instructions per lower-triangle element and direction
+FLOP_PER_ELEMENT = 48.0   # exchange bulk: 24 FP64 instructions per lower-triangle entry and direction (fused row)
 
 
 def ncu_traffic(workload, kernel):
@@ -253,17 +253,20 @@ def roofline_of(w, kern, iso, fp64_peak):
                 "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
                 "alone": {"ms": iso.get("pair"), "frac": (pairs * FLOP_PER_PAIR / ta / 1e12 / fp64_peak) if ta else None,
                           "frac_executed": (pairs * FLOP_PER_PAIR_EXECUTED / ta / 1e12 / fp64_peak) if ta else None}}
-    # non-interacting workloads: the exchange passes dominate; they recompute the closing springs
-    # instead of streaming an N x N matrix, so they are ALU bound too
-    fp_ms = kern.get("forcepass")
-    elems = float(w.N) * (w.N + 1)  # two sweeps over the lower triangle
-    ach = elems * FLOP_PER_ELEMENT / (fp_ms * 1e-3) / 1e12 if fp_ms else None
-    return {"bound": "alu", "kernel": "k_forcepass (connection probabilities)", "achieved": ach, "peak": fp64_peak,
-            "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": ncu_traffic(w.name, "k_forcepass"),
+    # non-interacting workloads: the exchange recursion is all there is.  It recomputes the closing springs instead of
+    # streaming an N x N matrix, so its bulk is ALU work (SURVEY 8(d), row "fused / recomputed": 2 passes x N^2/2 entries x
+    # about 24 FP64 instructions); the kernel itself is bound by the latency of its N-long dependent chain up to N ~ 2e4
+    ch_ms = kern.get("chain")
+    elems = float(w.N) * (w.N + 1)  # both directions over the lower triangle
+    ach = elems * FLOP_PER_ELEMENT / (ch_ms * 1e-3) / 1e12 if ch_ms else None
+    cha = iso.get("chain")
+    return {"bound": "alu", "kernel": "k_chain_spec (forward + backward recursion, panel workers with the force sums)", "achieved": ach,
+            "peak": fp64_peak, "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": ncu_traffic(w.name, "k_chain_spec"),
             "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak",
-            "convention": "54 flop (27 FP64 instructions) per matrix element, N(N+1) elements per launch",
-            "alone": {"ms": iso.get("forcepass"),
-                      "frac": (elems * FLOP_PER_ELEMENT / (iso["forcepass"] * 1e-3) / 1e12 / fp64_peak) if iso.get("forcepass") else None}}
+            "convention": "48 flop (24 FP64 instructions, SURVEY.md 8(d) fused row) per lower-triangle entry and direction, N(N+1) "
+                          "entries per launch; the kernel is latency bound (one dependent DFMA + SHFL per row, see `recursion`) "
+                          "until the workers' bulk takes over near N = 4e4",
+            "alone": {"ms": cha, "frac": (elems * FLOP_PER_ELEMENT / (cha * 1e-3) / 1e12 / fp64_peak) if cha else None}}
 
 
 def kernel_profile(sim, nsteps, w):

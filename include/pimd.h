@@ -199,7 +199,7 @@ int pimd_reweight(pimd_t h, const double *xi_obs, double *ln_abs_r, int *sign, d
  * Springs, trap, pair forces, integrator and the bead sums of the estimators are local; the exchange part (steps 3-6,
  * O(N^2) against O(P N^2 / world) for the pair part) runs redundantly on every rank.  One exchange step per MD step: the
  * all-gather (by the caller: NCCL through torch.distributed, or a device copy between shards on one GPU) of every
- * rank's boundary pack of `pack_doubles` = 2 N d + N doubles:
+ * rank's boundary pack of `pack_doubles` = 2 N d + N doubles, rounded up to an even count:
  *     [ first local slice : N d ][ last local slice : N d ][ E_int of the springs between local slices : N ].
  *   pimd_shard_export(h, send_dev)          write this rank's pack (DEVICE out); asynchronous
  *   pimd_shard_forces(h, gathered_dev)      take the gathered packs (DEVICE, world * pack_doubles, rank-major; copied)

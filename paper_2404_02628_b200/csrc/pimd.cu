@@ -154,6 +154,10 @@ struct ProfScope {
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// doubles in a bead shard's boundary pack: first slice, last slice, partial E_int, padded to an even count so that the
+// packs of all ranks stay 16-byte aligned in the gathered buffer (the slices are read as double2 for d = 2)
+size_t pack_doubles_of(int N, int d) { return (2 * (size_t)N * d + (size_t)N + 1) / 2 * 2; }
+
 // Carve the workspace; with base == nullptr only the sizes are computed.  Layout: the global region, then B replica
 // regions of h->rstride bytes each with identical layout (kernels reach replica b through blockIdx * rstride).
 size_t carve(pimd_t h, unsigned char *base)
@@ -171,7 +175,7 @@ size_t carve(pimd_t h, unsigned char *base)
     h->fallbacks = (unsigned long long *)take(8);
     h->phase = (unsigned long long *)take(16 * 8);
     h->dstep = (unsigned long long *)take(8);
-    const size_t packn = 2 * N * D + N;
+    const size_t packn = pack_doubles_of(h->N, h->d);
     h->pack = (double *)take(h->sharded ? packn * 8 : 8);
     h->gathered = (double *)take(h->sharded ? (size_t)h->world * packn * 8 : 8);
     h->eint_tot = (double *)take(h->sharded ? N * 8 : 8);
@@ -331,7 +335,7 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
 {
     const dim3 grid((h->N + BEAD_TB - 1) / BEAD_TB, h->P, h->B), block(BEAD_TB);
     const double om2P = h->omega * h->omega / h->Pg;
-    const size_t sl = h->slice, packn = 2 * sl + (size_t)h->N;
+    const size_t sl = h->slice, packn = pack_doubles_of(h->N, h->d);
     // bead shards: the ring neighbours' boundary slices come out of the gathered packs
     const double *halo_lo = (h->sharded && h->j0 > 0) ? h->gathered + (size_t)(h->rank - 1) * packn + sl : nullptr;
     const double *halo_hi = (h->sharded && h->j0 + h->P < h->Pg) ? h->gathered + (size_t)(h->rank + 1) * packn : nullptr;
@@ -384,7 +388,7 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
 
 template <int D> int launch_prep(pimd_t h, ExchCtx &c, cudaStream_t st)
 {
-    const size_t sl = h->slice, packn = 2 * sl + (size_t)h->N, lo = (size_t)c.l0 * D;
+    const size_t sl = h->slice, packn = pack_doubles_of(h->N, h->d), lo = (size_t)c.l0 * D;
     const double *x = h->x + lo, *x1 = h->x + lo, *xP = h->x + (size_t)(h->P - 1) * sl + lo, *ein = nullptr;
     if (h->sharded) { // bead 1 = first slice of rank 0, bead P = last slice of the last rank, E_int summed over the ranks
         x = nullptr;
@@ -1353,7 +1357,7 @@ int pimd_shard_layout(pimd_t h, int *j0, int *p_local, size_t *pack_doubles)
     if (!h) return PIMD_EINVAL;
     if (j0) *j0 = h->j0;
     if (p_local) *p_local = h->P;
-    if (pack_doubles) *pack_doubles = 2 * h->slice + (size_t)h->N;
+    if (pack_doubles) *pack_doubles = pack_doubles_of(h->N, h->d);
     return PIMD_OK;
 }
 
@@ -1376,15 +1380,15 @@ int pimd_shard_export(pimd_t h, double *send_dev)
 
 static int shard_import(pimd_t h, const double *gathered_dev)
 {
-    const size_t packn = 2 * h->slice + (size_t)h->N;
+    const size_t packn = pack_doubles_of(h->N, h->d);
     CU(cudaMemcpyAsync(h->gathered, gathered_dev, (size_t)h->world * packn * 8, cudaMemcpyDeviceToDevice, h->s0));
     const unsigned grid = (unsigned)((h->N + 127) / 128);
     {
         ProfScope ps(h, PIMD_PROF_SHARD, h->s0);
         switch (h->d) {
-        case 1: k_shard_eint<1><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
-        case 2: k_shard_eint<2><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
-        default: k_shard_eint<3><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, h->ks, h->eint_tot); break;
+        case 1: k_shard_eint<1><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, packn, h->ks, h->eint_tot); break;
+        case 2: k_shard_eint<2><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, packn, h->ks, h->eint_tot); break;
+        default: k_shard_eint<3><<<grid, 128, 0, h->s0>>>(h->gathered, h->N, h->world, packn, h->ks, h->eint_tot); break;
         }
     }
     CU(cudaGetLastError());

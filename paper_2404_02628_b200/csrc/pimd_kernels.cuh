@@ -2595,7 +2595,7 @@ __global__ void __launch_bounds__(GR_TB) k_gr(const double *__restrict__ x, int 
 // Bead shards ("parallel computing ... with a large number of ... GPUs"; the
 // per-slice pair term parallelises like classical MD).  A rank holds the contiguous slices [j0, j0 + Pl) of every ring.
 // What leaves a rank per MD step is its boundary pack
-//     [ first local slice : N d ][ last local slice : N d ][ partial E_int : N ]      (2 N d + N doubles)
+//     [ first local slice : N d ][ last local slice : N d ][ partial E_int : N ]      (2 N d + N doubles, padded to even)
 // (partial E_int = the springs between two local slices, Eq. 9); the all-gather of the packs gives every rank the halo
 // slices of its ring neighbours, bead 1 (first slice of rank 0), bead P (last slice of the last rank) and, with the springs
 // that cross a rank boundary added, E_int -- everything the exchange part (steps 3-6, run redundantly on every rank)
@@ -2620,12 +2620,12 @@ __global__ void __launch_bounds__(128) k_shard_pack(const double *__restrict__ x
 }
 
 template <int D>
-__global__ void __launch_bounds__(128) k_shard_eint(const double *__restrict__ gathered, int N, int world, double ks,
-                                                   double *__restrict__ eint)
+__global__ void __launch_bounds__(128) k_shard_eint(const double *__restrict__ gathered, int N, int world, size_t stride,
+                                                   double ks, double *__restrict__ eint)
 {
     const int l = blockIdx.x * 128 + threadIdx.x;
     if (l >= N) return;
-    const size_t sl = (size_t)N * D, stride = 2 * sl + N;
+    const size_t sl = (size_t)N * D;
     double e = 0.0, cross = 0.0;
     for (int r = 0; r < world; ++r) {
         e += gathered[r * stride + 2 * sl + l];

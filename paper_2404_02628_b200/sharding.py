@@ -5,7 +5,7 @@ exchange step per MD step: the all-gather of every rank's boundary pack
 
     [ first local slice : N d ][ last local slice : N d ][ E_int of the springs between local slices : N ]
 
-(2 N d + N doubles, written by pimd_shard_export, consumed by pimd_shard_forces / pimd_shard_end_step).  Everything
+(2 N d + N doubles, padded to an even count; written by pimd_shard_export, consumed by pimd_shard_forces / pimd_shard_end_step).  Everything
 else -- springs, trap, pair forces, integrator on the local slices, the exchange recursion redundantly on every rank --
 runs inside libpimd's kernels.
 
@@ -27,7 +27,8 @@ def shard_range(P: int, rank: int, world: int):
 
 
 def pack_doubles(N: int, d: int) -> int:
-    return 2 * N * d + N
+    """doubles per boundary pack, padded to an even count (the packs stay 16-byte aligned in the gathered buffer)"""
+    return (2 * N * d + N + 1) // 2 * 2
 
 
 def pack_offsets(N: int, d: int):

@@ -221,11 +221,11 @@ def test_pair_histogram_is_the_oracles(binding, oracle, case):
 # ---------------------------------------------------------------------------------------------------------------
 # (e / f2) bead shards on one GPU: world shards of one system, the all-gather a device copy
 # ---------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("world,P", [(2, 8), (4, 8), (3, 8), (8, 8), (2, 2)])
-def test_bead_shards_match_single_gpu_and_oracle(binding, oracle, world, P):
+@pytest.mark.parametrize("world,P,N", [(2, 8, 200), (4, 8, 200), (3, 8, 200), (8, 8, 200), (2, 2, 200), (3, 6, 333), (2, 5, 97)])
+def test_bead_shards_match_single_gpu_and_oracle(binding, oracle, world, P, N):
     from paper_2404_02628_b200 import sharding
 
-    w = wl.custom(200, P, d=2, beta=3.0, g=0.3, s=0.5, xi=1.0, init="ring", sigma=1.5)
+    w = wl.custom(N, P, d=2, beta=3.0, g=0.3, s=0.5, xi=1.0, init="ring", sigma=1.5)
     x, v = wl.make_state(w, 7)
     grp = sharding.LocalShardGroup(binding, world, w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=1, seed=42)
     for r, sim in enumerate(grp.sims):      # the C library and the Python layout helper agree

@@ -43,6 +43,7 @@ def test_slices_tile_the_ring_for_every_world_size():
     with pytest.raises(ValueError):
         sharding.shard_range(4, 0, 5)
     assert sharding.pack_doubles(10, 3) == 70 and sharding.pack_offsets(10, 3) == (0, 30, 60)
+    assert sharding.pack_doubles(37, 2) == 186          # 185 rounded up: packs stay 16-byte aligned
     assert sharding.halo_sources(0, 3) == (None, (1, "first")) and sharding.halo_sources(2, 3) == ((1, "last"), None)
 
 
@@ -69,7 +70,7 @@ def _worker(rank, world, port, out):
         send = torch.zeros(n, dtype=torch.float64)
         send[o_first:o_first + N * d] = torch.from_numpy(xl[0].reshape(-1))
         send[o_last:o_last + N * d] = torch.from_numpy(xl[-1].reshape(-1))
-        send[o_eint:] = torch.from_numpy(0.5 * ks * np.sum(np.diff(xl, axis=0) ** 2, axis=(0, 2)))
+        send[o_eint:o_eint + N] = torch.from_numpy(0.5 * ks * np.sum(np.diff(xl, axis=0) ** 2, axis=(0, 2)))
         gathered = torch.zeros(world * n, dtype=torch.float64)
         dist.all_gather_into_tensor(gathered, send)
         g = gathered.numpy().reshape(world, n)
@@ -85,7 +86,7 @@ def _worker(rank, world, port, out):
         ok.append((halo_lo is None) == (j0 == 0) and (halo_hi is None) == (j0 + pl == P))
         ok.append(np.array_equal(part["first"](0), x[0]) and np.array_equal(part["last"](world - 1), x[P - 1]))
         # E_int: partial sums + the springs that cross a rank boundary (what k_shard_eint forms)
-        eint = g[:, o_eint:].sum(axis=0)
+        eint = g[:, o_eint:o_eint + N].sum(axis=0)
         for r in range(world - 1):
             eint = eint + 0.5 * ks * np.sum((part["first"](r + 1) - part["last"](r)) ** 2, axis=1)
         ok.append(np.allclose(eint, oracle.eint(x, w.beta), rtol=1e-13, atol=0))
@@ -108,6 +109,9 @@ def _worker(rank, world, port, out):
         interior = [jl for jl in range(pl) if 0 < j0 + jl < P - 1]       # beads 1 and P also take the exchange forces
         ok.append(all(np.allclose(F[jl], Fo[j0 + jl], rtol=0, atol=1e-11 * np.abs(Fo).max()) for jl in interior))
         out.put((rank, j0, pl, ok))
+    except Exception as e:  # a failing worker must not leave the parent waiting for its result
+        out.put((rank, -1, -1, [repr(e)]))
+        raise
     finally:
         dist.destroy_process_group()
 
@@ -125,7 +129,7 @@ def test_boundary_packs_over_gloo(world):
     res = sorted(q.get(timeout=180) for _ in range(world))
     for p in procs:
         p.join(timeout=60)
-        assert p.exitcode == 0
+    assert all(p.exitcode == 0 for p in procs), res
     assert sum(r[2] for r in res) == 7
     for rank, j0, pl, ok in res:
-        assert all(ok), (rank, ok)
+        assert j0 >= 0 and all(v is True or v == np.True_ for v in ok), (rank, ok)
