@@ -237,18 +237,18 @@ uint64_t pimd_launch_count(pimd_t h);
  * HOST arrays ms_host / count_host (PIMD_PROF_NSLOTS entries each; either may be NULL) and resets. */
 #define PIMD_PROF_BEAD 0      /* spring + trap forces (step 1) */
 #define PIMD_PROF_PREP 1      /* closing springs, E_int, recursion inputs (step 3) */
-#define PIMD_PROF_CHAIN 2     /* forward + backward recursions (steps 4, 5) */
-#define PIMD_PROF_FORCEPASS 3 /* connection probabilities and their sums (step 6) */
-#define PIMD_PROF_ASSEMBLE 4  /* Eq. 13 and exterior forces (step 6) */
-#define PIMD_PROF_FINALIZE 5  /* V_B, sign, <E_c>; estimator arithmetic */
-#define PIMD_PROF_INTEGRATE 6 /* velocity Verlet + thermostat (step 7) */
-#define PIMD_PROF_COMBINE 7   /* force output */
-#define PIMD_PROF_PAIR 8      /* pair forces (step 2) */
-#define PIMD_PROF_EMAT 9      /* pimd_cycle_energies: the N x N write */
-#define PIMD_PROF_PRMAT 10    /* pimd_connection_probabilities: the N x N write */
-#define PIMD_PROF_GR 11       /* pair-distance histogram (estimator steps, pimd_set_pair_histogram) */
-#define PIMD_PROF_SHARD 12    /* bead shards: boundary pack / E_int assembly */
-#define PIMD_PROF_NSLOTS 13
+#define PIMD_PROF_CHAIN 2     /* forward + backward recursions with the panel workers' force sums (steps 4, 5), and, as the
+                                 tail of the same launch, the near-diagonal force band, Eq. 13 and the exterior forces (step 6) */
+#define PIMD_PROF_ASSEMBLE 3  /* step 6 for xi = 0 (every ring closes on itself) */
+#define PIMD_PROF_FINALIZE 4  /* V_B, sign, <E_c>; estimator arithmetic */
+#define PIMD_PROF_INTEGRATE 5 /* velocity Verlet + thermostat (step 7) */
+#define PIMD_PROF_COMBINE 6   /* force output */
+#define PIMD_PROF_PAIR 7      /* pair forces (step 2) */
+#define PIMD_PROF_EMAT 8      /* pimd_cycle_energies: the N x N write */
+#define PIMD_PROF_PRMAT 9     /* pimd_connection_probabilities: the N x N write */
+#define PIMD_PROF_GR 10       /* pair-distance histogram (estimator steps, pimd_set_pair_histogram) */
+#define PIMD_PROF_SHARD 11    /* bead shards: boundary pack / E_int assembly */
+#define PIMD_PROF_NSLOTS 12
 int pimd_set_profiling(pimd_t h, int on);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
 /* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpimd.so")
 OK, EINVAL, ENOMEM, ECUDA, ENUMERIC = 0, -1, -2, -3, -4
 THERMOSTAT_NVE, THERMOSTAT_LANGEVIN, THERMOSTAT_NHC = 0, 1, 2
 NHC_LENGTH = 4
-PROF_SLOTS = ("bead", "prep", "chain", "forcepass", "assemble", "finalize", "integrate", "combine", "pair", "emat", "prmat", "gr", "shard")
+PROF_SLOTS = ("bead", "prep", "chain", "assemble", "finalize", "integrate", "combine", "pair", "emat", "prmat", "gr", "shard")
 MAX_SPECIES, MAX_BINS = 4, 4096
 PAIR_GAUSSIAN, PAIR_SOFT_COULOMB = 0, 1
 

@@ -423,6 +423,7 @@ template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t
         a.kk = h->kk; a.p = c.p; a.rp = c.rp; a.rs = h->rstride;
         a.phase = h->profiling ? h->phase : nullptr;
         a.look_fb = h->look;
+        a.ks = h->ks; a.Fex1 = Fex1 + lo; a.FexP = FexP + lo; a.ecpart = c.ecpart;
         a.gauge_misfit = h->gflags;
         a.fallbacks = h->fallbacks;
         void *args[] = {&a};
@@ -441,20 +442,8 @@ template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t
         }
         c.gauge_valid = true;
         c.history++;
-        // the near-diagonal band of LOOK + 1 column blocks per row block; the panel workers delivered the rest (App. A.3)
-        {
-            ProfScope ps(h, PIMD_PROF_FORCEPASS, st);
-            const dim3 fgrid(c.NB, 2 * h->B);
-            if (sgn) k_forcepass<D, true><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->look, h->rstride);
-            else k_forcepass<D, false><<<fgrid, FP_TB, 0, st>>>(c.N, h->kk, c.p, h->look, h->rstride);
-        }
-        CU(cudaGetLastError());
-        {
-            ProfScope ps(h, PIMD_PROF_ASSEMBLE, st);
-            if (sgn) k_assemble<D, true, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->look, h->rstride);
-            else k_assemble<D, false, ASM_TB><<<dim3(c.nasm, h->B), ASM_TB, 0, st>>>(c.N, h->ks, c.p, c.rp, Fex1 + lo, FexP + lo, c.ecpart, h->look, h->rstride);
-        }
-        CU(cudaGetLastError());
+        // the force band (LOOK + 1 newest column blocks per row block) and the assembly of the exterior forces run as
+        // the tail of the recursion kernel (exchange_tail)
     }
     if (scalars) {
         {

@@ -333,6 +333,9 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
 // the spins terminate.
 // ==========================================================================================
 constexpr int CH_THREADS = 512;
+constexpr int FP_TB = 128; // threads of a force-band / assembly task group (tail of the recursion kernels)
+// doubles of shared memory one force-band task needs (a group of FP_TB = 128 threads)
+template <int D> __host__ __device__ constexpr int fp_task_doubles() { return 2 * FP_TB + FP_TB + FP_TB * D + 4 * (D + 2) * (FP_TB / 4); }
 constexpr int CH_WARPS = CH_THREADS / 32;
 constexpr int CH_MAXLOOK = 3; // (4 L + 1) * 32 part entries are scaled by one pass of 512 threads
 
@@ -342,7 +345,9 @@ struct ChainArgs {
     ExchPtrs p;                // replica 0; replica b of a batch is rs bytes further on (grid.z = replica)
     const RepParams *rp;       // likewise: sgn xi of the replica
     size_t rs;
-    int look_fb;               // k_chain_spec: look-ahead of the max-plus recursion it falls back to
+    int look_fb;               // look-ahead of the max-plus recursion k_chain_spec falls back to (= look: the force band counts on it)
+    double ks;                 // tail: spring constant, exterior-force outputs (replica 0, species offset applied), <E_c> partials
+    double *Fex1, *FexP, *ecpart;
     int *gauge_misfit;         // k_chain_spec: one flag for the whole launch (all replicas fall back together)
     unsigned long long *fallbacks; // counts the launches that fell back
     unsigned long long *phase; // optional [16]: cycles of the forward chain CTA per phase (profiling), or NULL
@@ -382,7 +387,9 @@ template <int D> size_t chain_smem_bytes_host(int look)
 {
     const size_t chain = ChainSmem<D>(look).total * 8;
     const size_t worker = (size_t)CH_WARPS * 32 * (16 + 8 + D * 8) + (size_t)CH_WARPS * 32 * 16 + (size_t)CH_WARPS * 32 * 8 * (D + 1);
-    return chain > worker ? chain : worker;
+    const size_t tail = (size_t)(CH_THREADS / FP_TB) * fp_task_doubles<D>() * 8; // staging areas of exchange_tail
+    const size_t m = chain > worker ? chain : worker;
+    return m > tail ? m : tail;
 }
 
 PIMD_DEV void bar_sync_named(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
@@ -1646,56 +1653,6 @@ __device__ void worker_cta(const ChainArgs &a, int dir, int widx, size_t roff, u
     }
 }
 
-template <int D, bool SGN>
-__global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double etab[32], etab64[64]; // 2^(i/32), 2^(i/64)
-    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
-    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
-    __syncthreads();
-    const int dir = blockIdx.y;
-    const size_t roff = (size_t)blockIdx.z * a.rs; // replica of a batch
-    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, roff, smem_raw, etab);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
-}
-
-// the recursion with the previous evaluation's gauge (see chain_cta_spec); same grid, same workers
-template <int D, bool SGN>
-__global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double etab[32], etab64[64];
-    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
-    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
-    __syncthreads();
-    const int dir = blockIdx.y;
-    const size_t roff = (size_t)blockIdx.z * a.rs;
-    if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, roff, smem_raw, etab64);
-    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
-    // Safety net in the same launch (a second, conditional cooperative launch cost 7 us per evaluation): if a row sum
-    // left the band the stale gauge covers (in any replica of the batch), every CTA sees the misfit flag after the grid
-    // barrier and the whole grid redoes the recursion with a fresh max-plus gauge (chain_cta), which overwrites everything
-    // this pass published.
-    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
-    __threadfence();
-    grid.sync();
-    if (ld_acquire(a.gauge_misfit) == 0) return; // the same answer in every CTA
-    if (blockIdx.x == 0 && blockIdx.y == 0) {
-        int *pr0 = rshift(a.p.panel_ready[0], roff), *pr1 = rshift(a.p.panel_ready[1], roff);
-        for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { pr0[k] = 0; pr1[k] = 0; }
-        if (threadIdx.x < 2) rshift(a.p.cols_ready, roff)[threadIdx.x] = 1;
-        if (threadIdx.x == 0 && blockIdx.z == 0) atomicAdd(a.fallbacks, 1ull);
-    }
-    __threadfence();
-    grid.sync();
-    ChainArgs b = a;
-    b.look = a.look_fb;
-    b.phase = nullptr;
-    if (blockIdx.x == 0) chain_cta<D, SGN>(b, dir, roff, smem_raw, etab);
-    else worker_cta<D, SGN>(b, dir, blockIdx.x - 1, roff, smem_raw, etab64);
-}
-
 template <int D> size_t chain_spec_smem_bytes_host()
 {
     const size_t chain = SpecSmem<D>().total * 8;
@@ -1713,33 +1670,30 @@ template <int D> size_t chain_spec_smem_bytes_host()
 // dir 0 gives the row sums (bead P, Eq. 16), dir 1 the column sums (bead 1, Eq. 15).
 // The terms w_ij are, up to a factor per row, the terms of the recursion's own row sums: the panel
 // workers accumulate sum w sig and sum w kk r2 over all columns older than the LOOK newest blocks while they form the
-// panel (p.pacc), so this kernel covers only the near-diagonal band of (LOOK + 1) column blocks per row block:
-// N (LOOK + 1) 32 entries per direction instead of N^2/2.  grid (NB, 2 B), block 128.
+// panel (p.pacc), so forceband_task covers only the near-diagonal band of (LOOK + 1) column blocks per row block:
+// N (LOOK + 1) 32 entries per direction instead of N^2/2.  One task per row block and direction, run by groups of 128
+// threads in the tail of the recursion kernels (exchange_tail).
 // ==========================================================================================
-constexpr int FP_TB = 128;
 
 template <int D, bool SGN>
-__global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs p, int band, size_t rs)
+__device__ void forceband_task(int N, double kk, const ExchPtrs &p, int band, int rt, int dir, int tid, int bar_id, double *sm,
+                               const double *etab)
 {
-    // A CTA of FP_TB = 128 threads takes one block of RT = 32 rows and the (band + 1) <= 4 newest column blocks of it, the
-    // ones the recursion kept inside its chain CTA (columns j0 = 32 (K - band) .. i); the sums over all older columns come
-    // from the panel workers (p.pacc, added in k_assemble).  Four threads per row with 32 columns each, partial sums
-    // combined in shared memory.  Every row is written by exactly one CTA: plain stores.
+    // A group of FP_TB = 128 threads (tid = 0..127, its own named barrier) takes one block of RT = 32 rows and the
+    // (band + 1) <= 4 newest column blocks of it, the ones the recursion kept inside its chain CTA (columns
+    // j0 = 32 (K - band) .. i); the sums over all older columns come from the panel workers (p.pacc, added in
+    // assemble_task).  Four threads per row with 32 columns each, partial sums combined in shared memory.  Every row is
+    // written by exactly one group: plain stores.
     constexpr int NQ = 4, CW = FP_TB / NQ, RT = FP_TB / NQ;
-    const int rt = blockIdx.x, dir = blockIdx.y & 1; // grid.y = 2 * replica + direction
     const int j0 = max(0, 32 * (rt - band));
-    p = rshift(p, (size_t)(blockIdx.y >> 1) * rs);
-    __shared__ double etab[64];
-    for (int k = threadIdx.x; k < 64; k += blockDim.x) etab[k] = c_exp2_64[k];
-    __shared__ double2 sg_g[FP_TB];
-    __shared__ double sg_s[FP_TB];
-    __shared__ double sg_sig[FP_TB * D];
-    __shared__ double part_s[NQ * (D + 2) * RT];
+    double2 *sg_g = reinterpret_cast<double2 *>(sm);
+    double *sg_s = sm + 2 * FP_TB, *sg_sig = sg_s + FP_TB, *part_s = sg_sig + FP_TB * D;
     const double2 *gd = p.g[dir], *go = p.g[1 - dir];
-    const int r = threadIdx.x % RT, q = threadIdx.x / RT;
+    const int r = tid % RT, q = tid / RT;
     const int i = rt * RT + r;
+    bar_sync_named(bar_id, FP_TB); // the previous task of this group is done with the staging area
     {
-        const int j = j0 + threadIdx.x;
+        const int j = j0 + tid;
         double2 gj = make_double2(-INFINITY, 0.0);
         double sj = 1.0;
         Vec<D> sc;
@@ -1750,12 +1704,12 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
             sj = p.gs[dir][j];
             sc = ldvec<D>(p.sig[dir], j);
         }
-        sg_g[threadIdx.x] = gj;
-        sg_s[threadIdx.x] = sj;
+        sg_g[tid] = gj;
+        sg_s[tid] = sj;
 #pragma unroll
-        for (int c = 0; c < D; ++c) sg_sig[threadIdx.x * D + c] = sc.v[c];
+        for (int c = 0; c < D; ++c) sg_sig[tid * D + c] = sc.v[c];
     }
-    __syncthreads();
+    bar_sync_named(bar_id, FP_TB);
     const int k0 = q * CW;
     const int ncol = (i < N) ? min(CW, i - (j0 + k0) + 1) : 0; // columns j0+k0 .. min(j0+k0+CW-1, i)
     double sw = 0.0, swc = 0.0, osg = 0.0;
@@ -1787,7 +1741,7 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 #pragma unroll
     for (int c = 0; c < D; ++c) part_s[(q * (D + 2) + 1 + c) * RT + r] = osg * sws.v[c];
     part_s[(q * (D + 2) + D + 1) * RT + r] = osg * swc;
-    __syncthreads();
+    bar_sync_named(bar_id, FP_TB);
     // thread (r, q) adds up components q, q + NQ, .. of row r
     if (i < N) {
         for (int c = q; c < D + 2; c += NQ) {
@@ -1806,15 +1760,12 @@ __global__ void __launch_bounds__(FP_TB) k_forcepass(int N, double kk, ExchPtrs 
 // (the intra-ring halves -k_s (r^P - r^{P-1}), -k_s (r^1 - r^2) are in k_bead; rows sum to 1).
 // One thread per particle.  ecpart: per-block partial sums of sum_{l'} Pr[l->l'] beta C(l,l').
 // ==========================================================================================
-template <int D, bool SGN, int TB>
-__global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, const RepParams *rp, double *Fex1, double *FexP,
-                                                double *ecpart, int band, size_t rs)
+template <int D, bool SGN>
+__device__ void assemble_task(int N, double ks, double xi, const ExchPtrs &p, double *Fex1, double *FexP, double *ecpart, int band,
+                              int chunk, int tid, int bar_id, double *red /* 4 doubles of the group */)
 {
-    __shared__ double red[TB / 32];
-    const size_t off = (size_t)blockIdx.y * rs;
-    p = rshift(p, off); Fex1 = rshift(Fex1, off); FexP = rshift(FexP, off); ecpart = rshift(ecpart, off);
-    const double xi = rshift(rp, off)->xi;
-    const int l = blockIdx.x * TB + threadIdx.x;
+    // a group of FP_TB = 128 threads takes the particles [128 chunk, 128 chunk + 128); ecpart[chunk] = their share of <E_c>
+    const int l = chunk * FP_TB + tid;
     double ec = 0.0;
     if (l < N) {
         const double2 R = p.rfin[0];
@@ -1862,8 +1813,96 @@ __global__ void __launch_bounds__(TB) k_assemble(int N, double ks, ExchPtrs p, c
         stvec<D>(Fex1, l, f1);
         ec = a0[D + 1] + pan[0][D] + pl * p.cnext[l];
     }
-    double s = block_sum<TB>(ec, red);
-    if (threadIdx.x == 0) ecpart[blockIdx.x] = s;
+    ec = warp_sum(ec);
+    bar_sync_named(bar_id, FP_TB);
+    if ((tid & 31) == 0) red[tid >> 5] = ec;
+    bar_sync_named(bar_id, FP_TB);
+    if (tid == 0) ecpart[chunk] = (red[0] + red[1]) + (red[2] + red[3]);
+}
+
+// ==========================================================================================
+// Tail of the recursion kernels: once both directions are done (grid barrier), the CTAs of a replica share out the
+// force-band tasks (one per row block and direction), meet at a second grid barrier and assemble the exterior forces.
+// Two launches less on the critical path of a step (k_forcepass, k_assemble used to be kernels of their own:
+// profiles/r2_notes.md).  Groups of 128 threads with their own named barriers (ids 1..4) and staging areas.
+// ==========================================================================================
+template <int D, bool SGN>
+__device__ void exchange_tail(const ChainArgs &a, size_t roff, unsigned char *smem_raw, const double *etab64,
+                              cooperative_groups::grid_group &grid)
+{
+    const int grp = threadIdx.x >> 7, tid = threadIdx.x & 127, bar_id = 1 + grp;
+    const int ngrp = CH_THREADS / FP_TB;
+    const int cid = blockIdx.x + gridDim.x * blockIdx.y, ncta = gridDim.x * gridDim.y; // the CTAs of this replica
+    const ExchPtrs p = rshift(a.p, roff);
+    double *sm = reinterpret_cast<double *>(smem_raw) + grp * fp_task_doubles<D>();
+    for (int task = cid * ngrp + grp; task < 2 * a.NB; task += ncta * ngrp)
+        forceband_task<D, SGN>(a.N, a.kk, p, a.look_fb, task >> 1, task & 1, tid, bar_id, sm, etab64);
+    __threadfence();
+    grid.sync();
+    const double xi = rshift(a.rp, roff)->xi;
+    const int nchunk = (a.N + FP_TB - 1) / FP_TB;
+    for (int chunk = cid * ngrp + grp; chunk < nchunk; chunk += ncta * ngrp)
+        assemble_task<D, SGN>(a.N, a.ks, xi, p, rshift(a.Fex1, roff), rshift(a.FexP, roff), rshift(a.ecpart, roff), a.look_fb, chunk, tid,
+                              bar_id, sm);
+}
+
+
+template <int D, bool SGN>
+__global__ void __launch_bounds__(CH_THREADS, 1) k_chain(ChainArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double etab[32], etab64[64]; // 2^(i/32), 2^(i/64)
+    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __syncthreads();
+    const int dir = blockIdx.y;
+    const size_t roff = (size_t)blockIdx.z * a.rs; // replica of a batch
+    if (blockIdx.x == 0) chain_cta<D, SGN>(a, dir, roff, smem_raw, etab);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __threadfence();
+    grid.sync();
+    exchange_tail<D, SGN>(a, roff, smem_raw, etab64, grid);
+}
+
+// the recursion with the previous evaluation's gauge (see chain_cta_spec); same grid, same workers
+template <int D, bool SGN>
+__global__ void __launch_bounds__(CH_THREADS, 1) k_chain_spec(ChainArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double etab[32], etab64[64];
+    if (threadIdx.x < 32) etab[threadIdx.x] = c_exp2_32[threadIdx.x];
+    if (threadIdx.x < 64) etab64[threadIdx.x] = c_exp2_64[threadIdx.x];
+    __syncthreads();
+    const int dir = blockIdx.y;
+    const size_t roff = (size_t)blockIdx.z * a.rs;
+    if (blockIdx.x == 0) chain_cta_spec<D, SGN>(a, dir, roff, smem_raw, etab64);
+    else worker_cta<D, SGN>(a, dir, blockIdx.x - 1, roff, smem_raw, etab64);
+    // Safety net in the same launch (a second, conditional cooperative launch cost 7 us per evaluation): if a row sum
+    // left the band the stale gauge covers (in any replica of the batch), every CTA sees the misfit flag after the grid
+    // barrier and the whole grid redoes the recursion with a fresh max-plus gauge (chain_cta), which overwrites everything
+    // this pass published.
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __threadfence();
+    grid.sync();
+    if (ld_acquire(a.gauge_misfit) != 0) { // the same answer in every CTA
+        if (blockIdx.x == 0 && blockIdx.y == 0) {
+            int *pr0 = rshift(a.p.panel_ready[0], roff), *pr1 = rshift(a.p.panel_ready[1], roff);
+            for (int k = threadIdx.x; k < a.NB; k += CH_THREADS) { pr0[k] = 0; pr1[k] = 0; }
+            if (threadIdx.x < 2) rshift(a.p.cols_ready, roff)[threadIdx.x] = 1;
+            if (threadIdx.x == 0 && blockIdx.z == 0) atomicAdd(a.fallbacks, 1ull);
+        }
+        __threadfence();
+        grid.sync();
+        ChainArgs b = a;
+        b.look = a.look_fb;
+        b.phase = nullptr;
+        if (blockIdx.x == 0) chain_cta<D, SGN>(b, dir, roff, smem_raw, etab);
+        else worker_cta<D, SGN>(b, dir, blockIdx.x - 1, roff, smem_raw, etab64);
+        __threadfence();
+        grid.sync();
+    }
+    exchange_tail<D, SGN>(a, roff, smem_raw, etab64, grid);
 }
 
 // ==========================================================================================
