@@ -733,7 +733,7 @@ template <int D> static int prmat_impl(pimd_t h, double *pr_dev)
     return PIMD_OK;
 }
 
-static int create_impl(pimd_t *out, int B, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
+static int create_impl(pimd_t *out, int B, bool shard, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
                        const double *xi, double dt, int thermostat, const uint64_t *seed)
 {
     pimd_t h = nullptr;
@@ -742,7 +742,7 @@ static int create_impl(pimd_t *out, int B, int rank, int world, int N, int P, in
     if (N < 1 || P < 2 || d < 1 || d > 3) return fail(nullptr, PIMD_EINVAL, "need N >= 1, P >= 2, d in {1,2,3} (got N=%d P=%d d=%d)", N, P, d);
     if (B < 1 || !xi || !seed) return fail(nullptr, PIMD_EINVAL, "need B >= 1 replicas with xi[B] and seed[B]");
     if (world < 1 || rank < 0 || rank >= world || world > P) return fail(nullptr, PIMD_EINVAL, "need 0 <= rank < world <= P (got rank=%d world=%d P=%d)", rank, world, P);
-    if (world > 1 && B != 1) return fail(nullptr, PIMD_EINVAL, "bead shards hold one replica");
+    if (shard && B != 1) return fail(nullptr, PIMD_EINVAL, "bead shards hold one replica");
     if (!finite_all({beta, omega, g, s, dt}) || !(beta > 0) || !(s > 0) || !(dt > 0) || omega < 0)
         return fail(nullptr, PIMD_EINVAL, "need finite arguments with beta > 0, s > 0, dt > 0, omega >= 0");
     bool any0 = false, anynz = false;
@@ -761,7 +761,7 @@ static int create_impl(pimd_t *out, int B, int rank, int world, int N, int P, in
     if (!h) return fail(nullptr, PIMD_ENOMEM, "host allocation failed");
     std::memset(h, 0, sizeof(*h));
     h->B = B; h->N = N; h->d = d;
-    h->Pg = P; h->rank = rank; h->world = world; h->sharded = world > 1;
+    h->Pg = P; h->rank = rank; h->world = world; h->sharded = shard; // world = 1 is a valid (degenerate) shard
     // bead shards: rank r holds the slices [floor(P r / world), floor(P (r+1) / world))
     h->j0 = (int)((long long)P * rank / world);
     h->P = (int)((long long)P * (rank + 1) / world) - h->j0;
@@ -821,19 +821,19 @@ const char *pimd_last_error(pimd_t h) { return h ? h->err : g_create_error; }
 int pimd_create(pimd_t *out, int N, int P, int d, double beta, double omega, double g, double s, double xi, double dt,
                 int thermostat, uint64_t seed)
 {
-    return create_impl(out, 1, 0, 1, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
+    return create_impl(out, 1, false, 0, 1, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
 }
 
 int pimd_create_batch(pimd_t *out, int B, int N, int P, int d, double beta, double omega, double g, double s, const double *xi,
                       double dt, int thermostat, const uint64_t *seed)
 {
-    return create_impl(out, B, 0, 1, N, P, d, beta, omega, g, s, xi, dt, thermostat, seed);
+    return create_impl(out, B, false, 0, 1, N, P, d, beta, omega, g, s, xi, dt, thermostat, seed);
 }
 
 int pimd_create_sharded(pimd_t *out, int rank, int world, int N, int P, int d, double beta, double omega, double g, double s,
                         double xi, double dt, int thermostat, uint64_t seed)
 {
-    return create_impl(out, 1, rank, world, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
+    return create_impl(out, 1, true, rank, world, N, P, d, beta, omega, g, s, &xi, dt, thermostat, &seed);
 }
 
 int pimd_destroy(pimd_t h)

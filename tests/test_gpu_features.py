@@ -349,3 +349,55 @@ def test_error_paths(binding):
         binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, [0.0, 1.0], w.dt)
     with pytest.raises(binding.PimdError):
         make(binding, w, species=[10, 10])
+
+
+def _nccl_worker(q):
+    """one rank over NCCL on the one GPU there is: the real ShardedPimd path (pimd_shard_* + all_gather_into_tensor)"""
+    import os
+
+    import torch.distributed as dist
+
+    from paper_2404_02628_b200 import binding as b, sharding
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ.setdefault("MASTER_PORT", "29631")
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        b.load()
+        w = wl.custom(150, 6, d=2, beta=3.0, g=0.3, s=0.5, xi=1.0, init="ring", sigma=1.5)
+        x, v = wl.make_state(w, 3)
+        sh = sharding.ShardedPimd(b, w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=1, seed=11)
+        sh.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+        F = sh.forces().cpu().numpy()
+        vb, sg = sh.sim.shard_scalars()
+        sh.step(8)
+        xs, vs = [t.cpu().numpy() for t in sh.sim.get_state()]
+        sh.close()
+        one = b.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=1, seed=11)
+        one.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+        F1, vb1, sg1 = one.forces()
+        one.step(8)
+        x1, v1 = [t.cpu().numpy() for t in one.get_state()]
+        one.close()
+        q.put((relerr(F, F1.cpu().numpy()), abs(vb - vb1) / abs(vb1), sg == sg1, relerr(xs, x1), relerr(vs, v1)))
+    except Exception as e:  # the parent must not wait for a result that never comes
+        q.put(repr(e))
+        raise
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sharded_stepping_through_nccl_on_one_gpu(binding):
+    """ShardedPimd as torchrun would run it, with the one rank this box has: the boundary pack goes through a real NCCL
+    all_gather_into_tensor on the handle's stream between pimd_shard_begin_step and pimd_shard_end_step"""
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_nccl_worker, args=(q,))
+    p.start()
+    res = q.get(timeout=300)
+    p.join(timeout=120)
+    assert p.exitcode == 0 and not isinstance(res, str), res
+    ef, ev, sg_ok, ex, evel = res
+    assert ef <= 1e-12 and ev <= 1e-13 and sg_ok and ex <= 1e-11 and evel <= 1e-10
