@@ -32,8 +32,12 @@
  *   estimators     d(beta V_B)/d beta by finite differences, virial vs
  *                  primitive ensemble agreement, exact ideal-gas energy     PINNED
  *   orc_step       NVE reversibility / energy drift, <v^2> = 1/beta,
- *                  ensemble energy vs exact.  No reference trajectory
- *                  exists for the thermostat internals:                     PARITY UNPINNED
+ *                  ensemble energy vs exact; Nose-Hoover chain (nhc_half):
+ *                  reversibility under (v, v_xi) -> (-v, -v_xi) and the
+ *                  conserved extended energy to O(dt^2)                     PINNED
+ *                  The parameter CHOICES the paper leaves open (chain length
+ *                  4, Q = beta/P, gamma = 1; R10) have no reference
+ *                  to be checked against:                                   PARITY UNPINNED (parameters only)
  *   orc_philox_normal  Philox4x32-10 known-answer vector (Random123 KAT)    PINNED
  *   orc_stream_*   (O(N) memory) brute-force finite differences at small N,
  *                  identical-ring closed form at N = 3000                   PINNED

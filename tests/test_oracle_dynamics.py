@@ -157,3 +157,70 @@ def test_ensemble_primitive_equals_virial_with_interaction(oracle):
     m, se = _mean_se(ep - ev)
     assert abs(m) < 3 * se + 0.01
     assert _mean_se(ep)[0] > ig.exact_energy(3, 2.0, 1.0, 2, 1.0, 4)  # repulsion raises the energy
+
+
+# ---------------------------------------------------------------- Nose-Hoover chain pins
+def _nhc_case():
+    w = wl.custom(N=4, P=4, d=2, beta=1.5, g=0.4, s=0.6, xi=1.0, dt=0.002, sigma=0.5)
+    x0, v0 = wl.make_state(w, 5)
+    # chain velocities of thermal size, sqrt(kT/Q) = sqrt(P)/beta, all four links excited so that every coupling acts
+    nhc0 = np.random.default_rng(6).normal(0.0, math.sqrt(w.P) / w.beta, size=(4, x0.size))
+    return w, x0, v0, nhc0
+
+
+def test_nhc_is_time_reversible(oracle):
+    """The chain update is a symmetric product of exact sub-flows, each of which commutes with (v, v_xi) -> (-v, -v_xi)
+    up to inversion, so n steps, a sign flip of the particle AND the chain velocities, and n more steps must lead back to
+    the start (x, -v, -v_xi) to rounding.  This pins the structure of every link: a force G_k that depended on the link it
+    drives (e.g. vx[k] for vx[k-1] in G, checked by hand on a mutated copy of the oracle: the return error rises from
+    3e-14 to 2e-2), an update order that is not palindromic, or unequal scaling factors on the two sides of a kick are no
+    longer self-inverse under the flip and miss the start at O(dt^2) per step."""
+    w, x0, v0, nhc0 = _nhc_case()
+    x, v, nhc = x0.copy(), v0.copy(), nhc0.copy()
+    F = _forces(oracle, w, x)
+    n = 150
+    oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, w.xi, w.dt, 2, 1.0, 0, 0, n)
+    assert np.max(np.abs(x - x0)) > 1e-3  # it moved
+    v *= -1.0
+    nhc *= -1.0
+    oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, w.xi, w.dt, 2, 1.0, 0, 0, n)
+    np.testing.assert_allclose(x, x0, atol=1e-10)
+    np.testing.assert_allclose(-v, v0, atol=1e-10)
+    np.testing.assert_allclose(-nhc, nhc0, atol=1e-10)
+
+
+def test_nhc_conserves_the_extended_energy(oracle):
+    """Nose-Hoover chain dynamics conserve H' = 1/2 sum v^2 + Phi(x) + sum_dof sum_k (1/2 Q v_xi_k^2 + kT xi_k) with
+    d xi_k/dt = v_xi_k (Martyna, Klein, Tuckerman; the paper's refs at PAPER.md:299-303).  The oracle carries only the chain
+    velocities, so the thermostat positions are integrated here from the velocities it returns after every step
+    (trapezoid rule, O(dt^2) like the integrator).  H' must stay put to O(dt^2) -- the drift at dt/2 is about a quarter --
+    while each of its parts moves by far more.  A wrong factor in a kick (h/2), in a scaling (h/4 twice) or in the particle
+    scaling (h), or a G_k built from the wrong link or with a wrong Q, breaks the cancellation between neighbouring links
+    and gives an O(1) drift that does not shrink with dt (checked on mutated copies of the oracle: 0.25 -> 0.5 in the
+    scaling gives a drift of 14.6, 0.5 -> 0.25 in a kick 1.2, h -> h/2 in the particle scaling 2.4, vx[k-1] -> vx[k] in G
+    7.2, against 7e-5 at dt = 0.004 and 1.8e-5 at dt = 0.002 for the oracle as it stands)."""
+    w, x0, v0, nhc0 = _nhc_case()
+    kT, Q = 1.0 / w.beta, w.beta / w.P
+
+    def run(dt, T=0.3):
+        x, v, nhc = x0.copy(), v0.copy(), nhc0.copy()
+        F = _forces(oracle, w, x)
+        xi_sum = 0.0  # sum over dof and links of xi_k
+        def parts():
+            return (0.5 * np.sum(v**2), oracle.potential(x, w.beta, w.omega, w.g, w.s, w.xi), 0.5 * Q * np.sum(nhc**2), kT * xi_sum)
+        p0 = parts()
+        worst, swing = 0.0, 0.0
+        for it in range(int(round(T / dt))):
+            before = nhc.sum()
+            oracle.step(x, v, F, nhc, w.beta, w.omega, w.g, w.s, w.xi, dt, 2, 1.0, 0, it, 1)
+            xi_sum += 0.5 * dt * (before + nhc.sum())
+            p = parts()
+            worst = max(worst, abs(sum(p) - sum(p0)))
+            swing = max(swing, max(abs(a - b) for a, b in zip(p, p0)))
+        return worst, swing
+
+    d1, swing = run(0.004)
+    d2, _ = run(0.002)
+    assert swing > 1.0            # energy does flow between particles, potential and chains ...
+    assert d1 < 2e-3 * swing      # ... while the sum stays put
+    assert d2 < 0.35 * d1         # O(dt^2)
