@@ -154,6 +154,42 @@ int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext);
 int pimd_cycle_energies(pimd_t h, double *e_dev);
 int pimd_connection_probabilities(pimd_t h, double *pr_dev);
 
+/* The cycle energies of Eq. 7-10 without a handle and without any allocation.
+ *
+ * Who this is for.  Every other compute call of this header needs a handle, and making a handle allocates: device memory
+ * for the workspace (cudaMalloc, unless pimd_set_workspace supplies it), pinned host memory, streams and events.  Some
+ * programs cannot afford that at the point where they need the result:
+ *   - a host application (an MD driver, a Python framework with a caching allocator) that has already claimed all the
+ *     device memory it is allowed to use, so that a cudaMalloc made behind its back fails or pushes it over its budget;
+ *   - a time-step loop with several streams in flight: cudaMalloc and cudaFree make the whole device wait, every stream
+ *     stalls and the overlap the loop was built for is gone;
+ *   - a plug-in or callback that runs where its host forbids allocation calls (a fixed memory plan made at start-up).
+ * Such a caller passes only its own input and output buffers; the four O(N) intermediate tables (E_int, the closing
+ * springs beta C(l,l+1) and their prefix sums S, T) live in a fixed array inside the library image, which the CUDA driver
+ * places on each GPU when the library is loaded there and keeps until the process exits: 4 x PIMD_NOALLOC_MAX_N doubles =
+ * 512 KiB per GPU, whether or not this function is ever called.
+ *
+ *   cuda_stream  cudaStream_t to enqueue on (NULL = default stream).  The call is ASYNCHRONOUS: it enqueues three kernels
+ *                and returns; the result is complete when the stream reaches that point.
+ *   x_dev        DEVICE in, [P][N][d] doubles, the state layout of this header; 16-byte aligned.  Not modified.
+ *   N, P, d      1 <= N <= PIMD_NOALLOC_MAX_N, P >= 2, d in {1,2,3};  beta > 0 (k_s = P/beta^2 as everywhere here).
+ *   e_dev        DEVICE out, N*N doubles, row-major: e[u*N + v] = E^{[u+1,v+1]} for u <= v, 0 below the diagonal
+ *                (same contents as pimd_cycle_energies).
+ * Returns PIMD_OK, or PIMD_EINVAL (bad argument; N > PIMD_NOALLOC_MAX_N is refused with a message that says so, nothing
+ * is launched) or PIMD_ECUDA; text through pimd_last_error(NULL).
+ *
+ * Rules that follow from the shared array:
+ *   - The first call on each device looks up the device address of the array (cudaGetSymbolAddress with that device
+ *     current; it allocates nothing, but it may make the runtime load the library's kernels onto the device).  Make that
+ *     first call during set-up, before any stream capture is begun.  Later calls on the device reuse the address.
+ *   - The array is one per GPU, not per call or per stream, and keeps what the last call left in it.  A call writes every
+ *     table entry before reading it, so stale contents are harmless, but two calls that can run on the GPU at the same
+ *     time (different streams, or two host threads) overwrite each other's tables and both results are garbage.  Calls
+ *     enqueued on one stream are ordered and safe.
+ *   - The device that is current when the call is made must be the one that x_dev, e_dev and the stream belong to. */
+#define PIMD_NOALLOC_MAX_N 16384
+int pimd_cycle_energies_noalloc(void *cuda_stream, const double *x_dev, int N, int P, int d, double beta, double *e_dev);
+
 /* Advance nsteps MD steps (asynchronous on the stream):
  *   thermostat half step ; v += dt/2 F ; x += dt v ; F = F(x) ; v += dt/2 F ; thermostat half step
  * Forces of the starting state are evaluated first if they are not cached.  For nsteps >= 3 (profiling off) all

@@ -17,6 +17,7 @@ THERMOSTAT_NVE, THERMOSTAT_LANGEVIN, THERMOSTAT_NHC = 0, 1, 2
 NHC_LENGTH = 4
 PROF_SLOTS = ("bead", "prep", "chain", "assemble", "finalize", "integrate", "combine", "pair", "emat", "prmat", "gr", "shard")
 MAX_SPECIES, MAX_BINS = 4, 4096
+NOALLOC_MAX_N = 16384
 PAIR_GAUSSIAN, PAIR_SOFT_COULOMB = 0, 1
 
 # every symbol include/pimd.h declares: (restype, argtypes)
@@ -65,6 +66,7 @@ _SYMBOLS = {
     "pimd_get_tables": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
     "pimd_cycle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pimd_connection_probabilities": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pimd_cycle_energies_noalloc": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]),
     "pimd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "pimd_estimators": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_double]),
     "pimd_launch_count": (C.c_uint64, [C.c_void_p]),
@@ -406,6 +408,27 @@ def selftest_exp(which, x_dev, stream=None):
     if rc != OK:
         raise PimdError(rc, lib.pimd_last_error(None).decode())
     return y
+
+
+def cycle_energies_noalloc(x_dev, beta, out, stream=None):
+    """pimd_cycle_energies_noalloc: E[u, v] = E^{[u+1,v+1]} of the positions x_dev ([P][N][d] CUDA float64 tensor) written
+    into the caller's `out` ([N][N] CUDA float64 tensor).  No handle; the library allocates nothing (its O(N) tables sit
+    in a fixed 512 KiB device array, N <= NOALLOC_MAX_N), and this wrapper allocates nothing either: both tensors are the
+    caller's.  Asynchronous on `stream` (default: torch's current stream).  See include/pimd.h for who needs this and for
+    the sharing rules (one array per GPU: do not let two calls overlap)."""
+    import torch
+
+    lib = load()
+    P, N, d = x_dev.shape
+    if not (x_dev.is_cuda and out.is_cuda and x_dev.is_contiguous() and out.is_contiguous()
+            and x_dev.dtype == torch.float64 and out.dtype == torch.float64 and out.numel() == N * N):
+        raise ValueError("cycle_energies_noalloc: contiguous CUDA float64 tensors x [P][N][d] and out [N][N] are required")
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = lib.pimd_cycle_energies_noalloc(C.c_void_p(stream), _ptr(x_dev), int(N), int(P), int(d), float(beta), _ptr(out))
+    if rc != OK:
+        raise PimdError(rc, lib.pimd_last_error(None).decode())
+    return out
 
 
 def version():

@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1534,3 +1535,107 @@ int pimd_probe_fp64_peak(void *cuda_stream, double *tflops)
 }
 
 } // extern "C"
+
+// ==========================================================================================================================
+// pimd_cycle_energies_noalloc: the cycle-energy matrix of Eq. 7-10 for callers that must not allocate (include/pimd.h).
+//
+// The handle path (pimd_cycle_energies) keeps four O(N) tables in the handle's workspace: E_int, beta C(l,l+1), and their
+// prefix sums S, T.  Here the same four tables live in the file-scope device array below, which is part of the library
+// image: the driver sets it aside on every GPU when the library's module is loaded there and releases it when the process
+// ends.  No cudaMalloc / cudaFree / cudaMallocHost, no stream or event creation, no handle.
+//
+// `g_noalloc_scratch` as host code sees it is only a stand-in for the device array (its host address means nothing to a
+// kernel), so the entry point asks the runtime for the real device address -- cudaGetSymbolAddress, once per device, with that
+// device current -- and hands that pointer to the kernels.
+//
+// Every table entry a call reads (indices < N) is written earlier in the same call, so nothing needs clearing between calls
+// even though the array keeps the previous call's contents.  All calls on one GPU share the array: two calls whose kernels
+// can overlap on the GPU (different streams, or two host threads) overwrite each other's tables.
+// ==========================================================================================================================
+// E_int | beta C(l,l+1) | S | T, PIMD_NOALLOC_MAX_N doubles each: 4 x 16384 x 8 B = 512 KiB on every GPU that loads the library
+static __device__ __align__(256) double g_noalloc_scratch[4 * (size_t)PIMD_NOALLOC_MAX_N];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+double *g_noalloc_ptr[NOALLOC_MAX_DEVICES]; // device address of g_noalloc_scratch on device i, or nullptr: not looked up yet
+
+// Variant of k_prep (step 3) that keeps only what Eq. 7-10 need and writes it to the scratch tables: E_int of every ring
+// (Eq. 9) and the closing spring to the next particle, beta C(l,l+1) = kk |r_l^P - r_{l+1}^1|^2 (0 for the
+// last particle).  x is [P][N][D]; one thread per particle.
+template <int D>
+__global__ void __launch_bounds__(128) k_noalloc_eint(const double *__restrict__ x, int N, int P, double ks, double kk,
+                                                      double *__restrict__ eint, double *__restrict__ cnext_beta)
+{
+    const int l = blockIdx.x * 128 + threadIdx.x;
+    if (l >= N) return;
+    const size_t sl = (size_t)N * D;
+    Vec<D> prev = ldvec<D>(x, l);
+    double acc = 0.0;
+    for (int j = 1; j < P; ++j) {
+        const Vec<D> cur = ldvec<D>(x + (size_t)j * sl, l);
+        acc += dist2<D>(cur, prev);
+        prev = cur;
+    }
+    eint[l] = 0.5 * ks * acc;
+    cnext_beta[l] = (l < N - 1) ? kk * dist2<D>(prev, ldvec<D>(x, l + 1)) : 0.0; // prev = bead P of particle l
+}
+
+// device address of the scratch array on the current device (looked up on the first call per device)
+int noalloc_scratch(double **out)
+{
+    pimd_t h = nullptr;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(nullptr, PIMD_EINVAL, "pimd_cycle_energies_noalloc: device ordinal %d not supported", dev);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return fail(nullptr, PIMD_ECUDA, "pimd_cycle_energies_noalloc: cudaGetSymbolAddress returned a null address");
+        g_noalloc_ptr[dev] = (double *)p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return PIMD_OK;
+}
+
+template <int D> int cycle_energies_noalloc_impl(cudaStream_t st, const double *x_dev, int N, int P, double beta, double *scratch, double *e_dev)
+{
+    pimd_t h = nullptr;
+    const double ks = (double)P / (beta * beta), kk = (double)P / (2.0 * beta); // as in create_impl
+    double *eint = scratch, *cnb = scratch + PIMD_NOALLOC_MAX_N, *S = scratch + 2 * (size_t)PIMD_NOALLOC_MAX_N,
+           *T = scratch + 3 * (size_t)PIMD_NOALLOC_MAX_N;
+    k_noalloc_eint<D><<<(N + 127) / 128, 128, 0, st>>>(x_dev, N, P, ks, kk, eint, cnb);
+    CU(cudaGetLastError());
+    k_prefix_st<<<1, 1024, 0, st>>>(N, beta, eint, cnb, S, T);
+    CU(cudaGetLastError());
+    // bead P / bead 1 slices straight from the caller's x (the handle path reads its own copies rho[0] / sig[0])
+    k_emat<D><<<dim3((N + 1023) / 1024, N), 256, 0, st>>>(N, ks, x_dev + (size_t)(P - 1) * N * D, x_dev, S, T, e_dev);
+    CU(cudaGetLastError());
+    return PIMD_OK;
+}
+
+} // namespace
+
+extern "C" int pimd_cycle_energies_noalloc(void *cuda_stream, const double *x_dev, int N, int P, int d, double beta, double *e_dev)
+{
+    if (!x_dev || !e_dev) return fail(nullptr, PIMD_EINVAL, "pimd_cycle_energies_noalloc: x_dev and e_dev must not be NULL");
+    if (N < 1 || P < 2 || d < 1 || d > 3 || !std::isfinite(beta) || !(beta > 0))
+        return fail(nullptr, PIMD_EINVAL, "pimd_cycle_energies_noalloc: need N >= 1, P >= 2, d in {1,2,3}, beta > 0 (got N=%d P=%d d=%d beta=%g)", N, P, d, beta);
+    if (N > PIMD_NOALLOC_MAX_N)
+        return fail(nullptr, PIMD_EINVAL,
+                    "pimd_cycle_energies_noalloc: N = %d exceeds PIMD_NOALLOC_MAX_N = %d, the size of the built-in scratch tables; "
+                    "use pimd_cycle_energies (handle with a workspace) for larger systems", N, PIMD_NOALLOC_MAX_N);
+    if ((((size_t)x_dev) & 15) != 0 || (((size_t)e_dev) & 7) != 0)
+        return fail(nullptr, PIMD_EINVAL, "pimd_cycle_energies_noalloc: x_dev must be 16-byte aligned, e_dev 8-byte aligned");
+    double *scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    switch (d) {
+    case 1: return cycle_energies_noalloc_impl<1>(st, x_dev, N, P, beta, scratch, e_dev);
+    case 2: return cycle_energies_noalloc_impl<2>(st, x_dev, N, P, beta, scratch, e_dev);
+    default: return cycle_energies_noalloc_impl<3>(st, x_dev, N, P, beta, scratch, e_dev);
+    }
+}
