@@ -30,7 +30,8 @@
  *   - One handle is not thread-safe; different handles are independent.
  *   - Environment knobs read by pimd_create() (tuning / debugging only): PIMD_LOOK (column blocks kept inside the
  *     chain CTA, 1..3), PIMD_WORKERS (panel worker CTAs per direction), PIMD_NOSPEC=1 (always run the max-plus
- *     recursion kernel, never the stale-gauge one), PIMD_PAIR_CH (tile offsets per pair-kernel task), PIMD_GRAPH=0
+ *     recursion kernel, never the stale-gauge one), PIMD_PAIR_CH (tile offsets per pair-kernel task), PIMD_PAIR2=0/1 (pair
+ *     kernel with one / two row particles per lane instead of the choice by size: two from N = 1500 on), PIMD_GRAPH=0
  *     (pimd_step launches every kernel itself instead of replaying a captured CUDA graph).
  *   - There is no CPU fallback: without a CUDA device pimd_create() fails with PIMD_ECUDA.
  */
@@ -75,8 +76,11 @@ int pimd_destroy(pimd_t h);
  * used for fictitious particles: simulate at several xi >= 0 and extrapolate / reweight; it also
  * fills the GPU at small N.  Either every xi[b] is 0 or none is.  With a batch every state / force array of this header
  * is [B][P][N][d] and every per-evaluation HOST output (vb, sign, e_prim, e_vir, hist, ...) has B entries (hist: [B][nbins]);
- * pimd_create() is the batch with B = 1.  B is limited by the co-resident CTAs of the recursion kernel (2 per replica and
- * direction at small N; 74 replicas at N <= 128 on a B200). */
+ * pimd_create() is the batch with B = 1.  B is limited by the CTAs of the recursion kernel that must be co-resident (one
+ * 512-thread CTA per SM): 2 per replica while every species has at most 32*(PIMD_LOOK+1) = 128 particles, 4 per replica
+ * (chain + at least one panel worker per direction) beyond that.  On a B200 (148 SMs): 74 replicas at N <= 128, 37 for
+ * larger N; a larger batch is refused with PIMD_EINVAL (by pimd_create_batch, or by pimd_set_species if the species
+ * partition is what needs the workers). */
 int pimd_create_batch(pimd_t *out, int B, int N, int P, int d, double beta, double omega, double g, double s,
                       const double *xi, double dt, int thermostat, const uint64_t *seed);
 
@@ -114,7 +118,10 @@ int pimd_get_state(pimd_t h, double *x_dev, double *v_dev);
 int pimd_set_state_host(pimd_t h, const double *x_host, const double *v_host);
 int pimd_get_state_host(pimd_t h, double *x_host, double *v_host);
 /* Resume support: MD step counter (the Philox counter of the Langevin noise) and the Nose-Hoover
- * chain variables nhc[PIMD_NHC_LENGTH][P*N*d] (DEVICE pointer). */
+ * chain variables nhc[PIMD_NHC_LENGTH][P*N*d] (DEVICE pointer).  A run continued in a new handle from
+ * (pimd_set_state, pimd_set_forces, pimd_set_step_count, pimd_set_nhc -- in this order: setting the state zeroes the chain
+ * variables) draws the same noise and follows the original trajectory to rounding (1e-12 after 10 steps in the tests), not
+ * to the bit: the new handle's first evaluation has no gauge history and the pair forces are accumulated with atomics. */
 int pimd_get_step_count(pimd_t h, uint64_t *step_host);
 int pimd_set_step_count(pimd_t h, uint64_t step);
 int pimd_get_nhc(pimd_t h, double *nhc_dev);
@@ -143,6 +150,8 @@ int pimd_set_forces_host(pimd_t h, const double *f_host);
  *   vbwd[u] = V_xi^{[u,N]}, u = 1..N+1 stored at index u (N+2 doubles, index 0 unused; Eq. 11)
  *   pnext[l] = Pr[G(l) = l+1], l = 1..N stored at l-1 (N doubles; Eq. 13). */
 int pimd_get_tables(pimd_t h, double *vfwd, double *vbwd, double *pnext);
+/* A diagnostic call, not part of the hot path: the device holds the tables as per-block gauges plus residuals; this call
+ * copies them out and finishes vfwd / vbwd with HOST arithmetic (long double prefix sums) inside the library. */
 
 /* The paper's N x N intermediates, materialised on request into caller memory (DEVICE, N*N doubles, row-major;
  * the hot path never stores them).  Both synchronise.  N <= 65535.
@@ -285,9 +294,15 @@ uint64_t pimd_launch_count(pimd_t h);
 #define PIMD_PROF_GR 10       /* pair-distance histogram (estimator steps, pimd_set_pair_histogram) */
 #define PIMD_PROF_SHARD 11    /* bead shards: boundary pack / E_int assembly */
 #define PIMD_PROF_NSLOTS 12
-int pimd_set_profiling(pimd_t h, int on);
+/* mode 0: off.  PIMD_PROFILE_EVENTS: event pairs only -- the kernels run exactly as in a production step, so these are
+ * the per-kernel times to quote.  PIMD_PROFILE_PHASES: also arms the clock64 phase counters inside the chain CTA
+ * (pimd_get_chain_phases); the instrumented recursion kernel runs a few per cent slower, so its event time is an upper
+ * bound in this mode.  Either mode turns graph replay off (every kernel is launched individually). */
+#define PIMD_PROFILE_EVENTS 1
+#define PIMD_PROFILE_PHASES 2
+int pimd_set_profiling(pimd_t h, int mode);
 int pimd_get_profile(pimd_t h, double *ms_host, uint64_t *count_host);
-/* Phase clock of the recursion (steps 4, 5).  While profiling is on, the forward chain CTA adds up SM
+/* Phase clock of the recursion (steps 4, 5).  In profiling mode PIMD_PROFILE_PHASES the forward chain CTA adds up SM
  * cycles per phase of its 32-row blocks (HOST out, 16 entries, accumulated since the previous call, then reset).
  * Evaluations that ran with the previous evaluation's gauge (k_chain_spec: every evaluation of a handle but its
  * first) fill

@@ -18,6 +18,7 @@ NHC_LENGTH = 4
 PROF_SLOTS = ("bead", "prep", "chain", "assemble", "finalize", "integrate", "combine", "pair", "emat", "prmat", "gr", "shard")
 MAX_SPECIES, MAX_BINS = 4, 4096
 NOALLOC_MAX_N = 16384
+PROFILE_EVENTS, PROFILE_PHASES = 1, 2
 PAIR_GAUSSIAN, PAIR_SOFT_COULOMB = 0, 1
 
 # every symbol include/pimd.h declares: (restype, argtypes)
@@ -368,8 +369,10 @@ class Pimd:
         self._check(self._lib.pimd_get_diagnostics(self._h, out))
         return {"fallbacks": int(out[0]), "status_seen": int(out[1]), "workers": int(out[2]), "replica_stride": int(out[3])}
 
-    def set_profiling(self, on):
-        self._check(self._lib.pimd_set_profiling(self._h, int(bool(on))))
+    def set_profiling(self, on, phases=True):
+        """off / PIMD_PROFILE_PHASES (events + the chain CTA's phase clock; default) / PIMD_PROFILE_EVENTS (phases=False:
+        event pairs only, the uninstrumented kernels)"""
+        self._check(self._lib.pimd_set_profiling(self._h, (PROFILE_PHASES if phases else PROFILE_EVENTS) if on else 0))
 
     def get_profile(self):
         """{slot name: (total ms, launches)} since the previous call."""

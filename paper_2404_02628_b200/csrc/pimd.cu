@@ -30,6 +30,7 @@ constexpr int MAX_BINS = GR_MAXBINS;
 // (the sampling xi, or the second xi of pimd_reweight).  Pointers are those of replica 0.
 struct ExchCtx {
     int N, l0, NB, nprep, nasm, nworkers;
+    int sp; // species index: slot of this problem's gauge-misfit word in gflags (one launch = one species, all replicas)
     ExchPtrs p;
     Scalars *scal;
     double *ecpart;
@@ -55,6 +56,7 @@ struct pimd_s {
     double ks, kk;
     size_t ndof, slice;
     int look, look_spec, sms;
+    int pair2_knob, pair_ch_knob; // PIMD_PAIR2 (-1: by size) and PIMD_PAIR_CH (0: by size), read once at creation
     // streams
     cudaStream_t s0, s1;
     cudaEvent_t ev_fork, ev_join;
@@ -98,7 +100,8 @@ struct pimd_s {
     int nbins_gr;
     double rmax_gr;
     // per-kernel device timing (pimd_set_profiling)
-    bool profiling;
+    bool profiling;    // kernel launches bracketed by events
+    bool phase_clock;  // ... and the chain CTA's clock64 instrumentation armed (PIMD_PROFILE_PHASES)
     std::vector<cudaEvent_t> *prof_ev; // pairs (start, stop)
     std::vector<int> *prof_slot;
     double prof_ms[PIMD_PROF_NSLOTS];
@@ -172,7 +175,7 @@ size_t carve(pimd_t h, unsigned char *base)
     const size_t N = (size_t)h->N, D = (size_t)h->d, nd = h->ndof, B = (size_t)h->B;
     // ---- global region
     h->Fout = (double *)take(B * nd * 8);
-    h->gflags = (int *)take(4 * 4);
+    h->gflags = (int *)take(PIMD_MAX_SPECIES * 4);
     h->fallbacks = (unsigned long long *)take(8);
     h->phase = (unsigned long long *)take(16 * 8);
     h->dstep = (unsigned long long *)take(8);
@@ -279,7 +282,7 @@ int ensure_ws(pimd_t h)
 }
 
 // species ranges -> exchange problems (both parameter sets); worker counts need the co-residency limit
-void setup_species(pimd_t h)
+int setup_species(pimd_t h)
 {
     int l0 = 0;
     for (int sp = 0; sp < h->nspecies; ++sp) {
@@ -287,6 +290,7 @@ void setup_species(pimd_t h)
             ExchCtx &c = h->ex[set][sp];
             c.N = h->counts[sp];
             c.l0 = l0;
+            c.sp = sp;
             c.NB = (c.N + 31) / 32;
             c.nprep = (c.N + PREP_TB - 1) / PREP_TB;
             c.nasm = (c.N + ASM_TB - 1) / ASM_TB;
@@ -305,10 +309,18 @@ void setup_species(pimd_t h)
                 if (v >= 1) need = v;
             }
             if (need > cap) need = cap;
+            // Row blocks beyond the look-ahead take their old columns from a panel worker, and the chain CTA waits for that
+            // panel: with no room for even one worker per replica and direction the cooperative kernel would never finish.
+            if (want > 0 && cap < 1)
+                return fail(h, PIMD_EINVAL,
+                            "a batch of %d replicas with %d particles in a species (more than %d) needs %d co-resident recursion CTAs "
+                            "(chain + one panel worker, per direction and replica); the device holds %d: at most %d replicas",
+                            h->B, c.N, 32 * (h->look + 1), 4 * h->B, h->coop_max_blocks, h->coop_max_blocks / 4);
             c.nworkers = want <= 0 ? 0 : std::max(0, std::min(want, need));
         }
         l0 += h->counts[sp];
     }
+    return PIMD_OK;
 }
 
 template <int D> int setup_chain_attr(pimd_t h)
@@ -353,14 +365,13 @@ template <int D> int launch_bead(pimd_t h, cudaStream_t st, bool est, int nbins,
         // From N = 1500 on: super-tiles of 64 particles, two row particles per lane (k_pair2: half the shared-memory and
         // shuffle traffic per pair; measured cfg3 0.0804 -> 0.0738 ms, cfg5b 1.199 -> 1.089 ms alone, but cfg4 (N = 1000)
         // 0.0398 -> 0.0422 and cfg2 0.0087 -> 0.0137: too few warps).  PIMD_PAIR2=0/1 forces one or the other.
-        bool two_rows = h->N >= 1500;
-        if (const char *e = std::getenv("PIMD_PAIR2")) two_rows = std::atoi(e) != 0;
+        const bool two_rows = h->pair2_knob >= 0 ? h->pair2_knob != 0 : h->N >= 1500;
         const int NT = two_rows ? (h->N + 63) / 64 : (h->N + 31) / 32;
         const int hmax = (NT & 1) ? (NT - 1) / 2 : NT / 2;
         // tile offsets per task: small tasks balance the grid (one-row kernel: 1 is best up to N = 2500, 4 at N = 10000;
         // two-row kernel: 1 throughout, cfg5b 1.089 / 1.152 / 1.284 ms with 1 / 2 / 4); tuning knob PIMD_PAIR_CH
         int target = two_rows ? 1 : (NT <= 100 ? 1 : (NT <= 200 ? 2 : 4));
-        if (const char *e = std::getenv("PIMD_PAIR_CH")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) target = v; }
+        if (h->pair_ch_knob > 0) target = h->pair_ch_knob;
         const int nchunk = hmax > 0 ? std::max(1, (hmax + target / 2) / target) : 0;
         const int ch = nchunk > 0 ? (hmax + nchunk - 1) / nchunk : 1;
         const long long tasks = (long long)NT * (nchunk + 1);
@@ -401,7 +412,7 @@ template <int D> int launch_prep(pimd_t h, ExchCtx &c, cudaStream_t st)
     {
         ProfScope ps(h, PIMD_PROF_PREP, st);
         k_prep<D, PREP_TB><<<dim3(c.nprep, h->B), PREP_TB * PREP_SPLIT, 0, st>>>(x, x1, xP, ein, sl, c.N, h->P, c.NB, h->ks, h->kk, c.p, c.rp,
-                                                                               h->gflags, c.history >= 2 ? 1 : 0, h->rstride);
+                                                                               h->gflags + c.sp, c.history >= 2 ? 1 : 0, h->rstride);
     }
     CU(cudaGetLastError());
     return PIMD_OK;
@@ -422,10 +433,10 @@ template <int D> int launch_exchange(pimd_t h, ExchCtx &c, int set, cudaStream_t
         ChainArgs a;
         a.N = c.N; a.NB = c.NB; a.look = h->look; a.nworkers = c.nworkers;
         a.kk = h->kk; a.p = c.p; a.rp = c.rp; a.rs = h->rstride;
-        a.phase = h->profiling ? h->phase : nullptr;
+        a.phase = h->phase_clock ? h->phase : nullptr;
         a.look_fb = h->look;
         a.ks = h->ks; a.Fex1 = Fex1 + lo; a.FexP = FexP + lo; a.ecpart = c.ecpart;
-        a.gauge_misfit = h->gflags;
+        a.gauge_misfit = h->gflags + c.sp; // a species that rejects its gauge must not make the later ones redo theirs
         a.fallbacks = h->fallbacks;
         void *args[] = {&a};
         const dim3 grid(1 + c.nworkers, 2, h->B), block(CH_THREADS);
@@ -783,6 +794,10 @@ static int create_impl(pimd_t *out, int B, bool shard, int rank, int world, int 
         const int v = std::atoi(e2);
         if (v >= 1 && v <= CH_MAXLOOK) h->look = h->look_spec = v;
     }
+    h->pair2_knob = -1;
+    if (const char *e2 = std::getenv("PIMD_PAIR2")) h->pair2_knob = std::atoi(e2) != 0 ? 1 : 0;
+    h->pair_ch_knob = 0;
+    if (const char *e2 = std::getenv("PIMD_PAIR_CH")) { const int v = std::atoi(e2); if (v >= 1 && v <= 64) h->pair_ch_knob = v; }
     h->concurrent = true;
     h->use_graph = !(std::getenv("PIMD_GRAPH") && std::atoi(std::getenv("PIMD_GRAPH")) == 0);
     h->use_spec = !(std::getenv("PIMD_NOSPEC") && std::atoi(std::getenv("PIMD_NOSPEC")) != 0);
@@ -796,7 +811,8 @@ static int create_impl(pimd_t *out, int B, bool shard, int rank, int world, int 
     default: rc = setup_chain_attr<3>(h); break;
     }
     if (rc) return bail(rc);
-    setup_species(h);
+    rc = setup_species(h);
+    if (rc) return bail(rc);
     const size_t nst = (size_t)B * (1 + 2 * PIMD_MAX_SPECIES);
     if (cudaStreamCreateWithFlags(&h->s1, cudaStreamNonBlocking) != cudaSuccess ||
         cudaStreamCreateWithFlags(&h->sg, cudaStreamNonBlocking) != cudaSuccess ||
@@ -918,10 +934,21 @@ int pimd_set_species(pimd_t h, int nspecies, const int *counts)
         tot += counts[k];
     }
     if (tot != h->N) return fail(h, PIMD_EINVAL, "species counts add up to %lld, not N = %d", tot, h->N);
+    const int old_n = h->nspecies;
+    int old_counts[PIMD_MAX_SPECIES];
+    for (int k = 0; k < PIMD_MAX_SPECIES; ++k) old_counts[k] = h->counts[k];
     h->nspecies = nspecies;
     for (int k = 0; k < nspecies; ++k) h->counts[k] = counts[k];
-    setup_species(h);
-    return PIMD_OK;
+    const int rc = setup_species(h);
+    if (rc) { // the batch leaves no room for the panel workers these species need: keep the previous partition
+        char msg[512];
+        std::snprintf(msg, sizeof msg, "%s", h->err);
+        h->nspecies = old_n;
+        for (int k = 0; k < PIMD_MAX_SPECIES; ++k) h->counts[k] = old_counts[k];
+        setup_species(h);
+        std::snprintf(h->err, sizeof h->err, "%s", msg);
+    }
+    return rc;
 }
 
 int pimd_set_pair_potential(pimd_t h, int kind)
@@ -1454,7 +1481,9 @@ uint64_t pimd_launch_count(pimd_t h) { return h ? h->launches : 0; }
 int pimd_set_profiling(pimd_t h, int on)
 {
     if (!h) return PIMD_EINVAL;
+    if (on < 0 || on > PIMD_PROFILE_PHASES) return fail(h, PIMD_EINVAL, "pimd_set_profiling: mode must be 0, PIMD_PROFILE_EVENTS or PIMD_PROFILE_PHASES");
     h->profiling = on != 0;
+    h->phase_clock = on == PIMD_PROFILE_PHASES;
     return PIMD_OK;
 }
 

@@ -59,11 +59,13 @@ class ShardedPimd:
         n = self.sim.pack_doubles
         self.send = torch.empty(n, dtype=torch.float64, device="cuda")
         self.gathered = torch.empty(self.world * n, dtype=torch.float64, device="cuda")
+        self._have_forces = False  # the library holds forces of the current positions (set_state invalidates them)
 
     def set_state(self, x_global, v_global=None):
         """global [P][N][d] device tensors; the local slices are taken"""
         sl = slice(self.j0, self.j0 + self.P_local)
         self.sim.set_state(x_global[sl].contiguous(), None if v_global is None else v_global[sl].contiguous())
+        self._have_forces = False
 
     def _all_gather(self):
         self._dist.all_gather_into_tensor(self.gathered, self.send, group=self.group)
@@ -72,16 +74,16 @@ class ShardedPimd:
         self.sim.shard_export(self.send)
         self._all_gather()
         self.sim.shard_forces(self.gathered)
+        self._have_forces = True
         return self.sim.get_forces()
 
     def step(self, nsteps=1):
-        if nsteps > 0 and not getattr(self, "_have_forces", False):
+        if nsteps > 0 and not self._have_forces:
             self.forces()
         for _ in range(nsteps):
             self.sim.shard_begin_step(self.send)
             self._all_gather()
             self.sim.shard_end_step(self.gathered)
-        self._have_forces = True
 
     def close(self):
         self.sim.close()

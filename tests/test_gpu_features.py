@@ -179,9 +179,11 @@ def test_species_match_oracle(binding, oracle, counts, xi):
     sim.close()
 
 
-@pytest.mark.parametrize("d", [2, 3])
-def test_soft_coulomb_potential_matches_oracle(binding, oracle, d):
-    w = wl.custom(130, 6, d=d, beta=2.0, g=0.4, s=0.5, xi=1.0, init="iid", sigma=1.0)
+@pytest.mark.parametrize("N,P,d", [(130, 6, 2), (130, 6, 3), (1550, 3, 2), (1517, 2, 3)], ids=["n130_d2", "n130_d3", "n1550_d2", "n1517_d3"])
+def test_soft_coulomb_potential_matches_oracle(binding, oracle, N, P, d):
+    """N = 130 runs k_pair<., ., 1>; from N = 1500 on the two-rows-per-lane kernel k_pair2<., ., 1> (its diagonal tiles drop
+    the self term and its last super-tile is padded: N is not a multiple of 64), forces and estimator variants alike."""
+    w = wl.custom(N, P, d=d, beta=2.0, g=0.4, s=0.5, xi=1.0, init="iid", sigma=1.0 if N < 1000 else 4.0)
     x, _ = wl.make_state(w, 2)
     sim = make(binding, w, pair_potential=binding.PAIR_SOFT_COULOMB)
     sim.set_state(torch.from_numpy(x).cuda())
@@ -303,6 +305,33 @@ def test_set_gamma_takes_effect_on_replayed_steps(binding):
     assert relerr(out[0][0], out[1][0]) <= 1e-12 and relerr(out[0][1], out[1][1]) <= 1e-11
 
 
+@pytest.mark.timeout(240, method="thread")
+def test_batch_size_limit_of_the_recursion_kernel(binding, oracle):
+    """Above 128 particles every replica needs a chain CTA and at least one panel worker per direction, all co-resident:
+    a B200 holds 148 / 4 = 37 such replicas.  A larger batch used to start a cooperative kernel whose chain CTAs waited
+    for panels nobody computed; it is refused at creation now, and the largest batch that fits runs and is right."""
+    w = wl.custom(200, 4, d=2, beta=2.0, g=0.0, xi=1.0, init="ring", sigma=1.0)
+    with pytest.raises(binding.PimdError) as e:
+        binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, [1.0] * 40, w.dt)
+    assert e.value.code == binding.EINVAL and "replicas" in str(e.value)
+    small = wl.custom(128, 4, d=2, beta=2.0, g=0.0, xi=1.0, init="ring", sigma=1.0)   # no workers needed: 74 replicas fit
+    binding.Pimd(small.N, small.P, small.d, small.beta, small.omega, small.g, small.s, [1.0] * 40, small.dt).close()
+    B = 37
+    xis = [1.0 if b % 2 == 0 else 0.5 for b in range(B)]
+    sim = binding.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, xis, w.dt)
+    assert sim.get_diagnostics()["workers"] >= 1
+    xs = np.stack([wl.make_state(w, 100 + b)[0] for b in range(B)])
+    sim.set_state(torch.from_numpy(xs).cuda())
+    for _ in range(2):   # the second evaluation runs the stale-gauge kernel
+        F, vb, sg = sim.forces()
+    F = F.cpu().numpy()
+    sim.close()
+    for b in (0, 17, 36):
+        Fo, vbo, sgo = oracle.forces(xs[b], w.beta, w.omega, w.g, w.s, xis[b])
+        assert sg[b] == sgo and abs(vb[b] - vbo) <= RTOL * abs(vbo)
+        check_forces(F[b], Fo, RTOL)
+
+
 def test_error_paths(binding):
     w = wl.custom(40, 4, d=2, beta=2.0, g=0.1, xi=1.0, init="iid", sigma=0.7)
     x, _ = wl.make_state(w, 0)
@@ -372,14 +401,21 @@ def _nccl_worker(q):
         vb, sg = sh.sim.shard_scalars()
         sh.step(8)
         xs, vs = [t.cpu().numpy() for t in sh.sim.get_state()]
+        # a second set_state drops the cached forces: the next step() must make its own export / all-gather / forces first
+        sh.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+        sh.step(3)
+        xs2 = sh.sim.get_state()[0].cpu().numpy()
         sh.close()
         one = b.Pimd(w.N, w.P, w.d, w.beta, w.omega, w.g, w.s, w.xi, w.dt, thermostat=1, seed=11)
         one.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
         F1, vb1, sg1 = one.forces()
         one.step(8)
         x1, v1 = [t.cpu().numpy() for t in one.get_state()]
+        one.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+        one.step(3)
+        x2 = one.get_state()[0].cpu().numpy()
         one.close()
-        q.put((relerr(F, F1.cpu().numpy()), abs(vb - vb1) / abs(vb1), sg == sg1, relerr(xs, x1), relerr(vs, v1)))
+        q.put((relerr(F, F1.cpu().numpy()), abs(vb - vb1) / abs(vb1), sg == sg1, relerr(xs, x1), relerr(vs, v1), relerr(xs2, x2)))
     except Exception as e:  # the parent must not wait for a result that never comes
         q.put(repr(e))
         raise
@@ -399,5 +435,5 @@ def test_sharded_stepping_through_nccl_on_one_gpu(binding):
     res = q.get(timeout=300)
     p.join(timeout=120)
     assert p.exitcode == 0 and not isinstance(res, str), res
-    ef, ev, sg_ok, ex, evel = res
-    assert ef <= 1e-12 and ev <= 1e-13 and sg_ok and ex <= 1e-11 and evel <= 1e-10
+    ef, ev, sg_ok, ex, evel, ex2 = res
+    assert ef <= 1e-12 and ev <= 1e-13 and sg_ok and ex <= 1e-11 and evel <= 1e-10 and ex2 <= 1e-11

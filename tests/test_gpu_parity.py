@@ -482,3 +482,46 @@ def test_graph_replay_matches_step_by_step(binding):
         # identical kernels and arguments; atomics in the pair / force-pass kernels make the last bits order dependent
         assert relerr(xs, out[0][0]) <= 1e-12
         assert relerr(vs, out[0][1]) <= 1e-11
+
+
+@pytest.mark.parametrize("thermostat", [1, 2], ids=["langevin", "nhc"])
+def test_resume_through_the_thermostats(binding, thermostat):
+    """Checkpoint / resume with a thermostat: 20 steps on one handle against 10 steps, a snapshot of
+    (x, v, F, step counter, Nose-Hoover chain variables) moved into a SECOND handle, and 10 more steps there.  The Langevin
+    noise is keyed by (seed, degree of freedom, step counter), so pimd_set_step_count is what lines the noise up; the chain
+    variables go through pimd_get_nhc / pimd_set_nhc (after pimd_set_state, which zeroes them).  Agreement is to rounding,
+    not to the bit: the second handle's first evaluation has no gauge history and the pair forces are summed with atomics
+    (pimd.h says so).  Leaving the counter / the chain variables out must visibly change the trajectory."""
+    w = wl.custom(97, 6, d=2, beta=2.0, g=0.3, xi=1.0, init="iid", sigma=0.8)
+    x, v = wl.make_state(w, 6)
+    a = make(binding, w, thermostat=thermostat, seed=21)
+    a.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    a.step(10)
+    xa, va = a.get_state()
+    Fa = a.get_forces()
+    count = a.get_step_count()
+    assert count == 10
+    nhc = a.get_nhc() if thermostat == 2 else None
+    a.step(10)
+    x20, v20 = [t.cpu().numpy() for t in a.get_state()]
+    a.close()
+
+    def resume(full):
+        b = make(binding, w, thermostat=thermostat, seed=21)
+        b.set_state(xa, va)
+        b.set_forces(Fa)
+        if full:
+            b.set_step_count(count)
+            if nhc is not None:
+                b.set_nhc(nhc)
+        b.step(10)
+        out = [t.cpu().numpy() for t in b.get_state()]
+        n = b.get_step_count()
+        b.close()
+        return out, n
+
+    (xb, vb_), n = resume(True)
+    assert n == 20
+    assert relerr(xb, x20) <= 1e-12 and relerr(vb_, v20) <= 1e-11
+    (xc, vc), _ = resume(False)
+    assert relerr(vc, v20) > 1e-3
