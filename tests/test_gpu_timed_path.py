@@ -188,3 +188,112 @@ def test_set_state_on_a_used_handle(binding, oracle):
     diag = sim.get_diagnostics()
     sim.close()
     assert diag["fallbacks"] >= 1          # the large moves cannot fit the old gauge
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# The state bench.py times: thermalised on the GPU (3000 Langevin steps at the centroid's critical damping).  In the
+# non-interacting workloads (config 5) the stale-gauge kernel then forms its exponent arguments the factorised way and skips
+# hardly any helper batch -- branches the seeded initial cloud + 3 steps above does not reach; which branch ran is read
+# from the phase clock and asserted.
+# ---------------------------------------------------------------------------------------------------------------
+EQUIL = 3000
+
+
+def thermalised(binding, w, seed=0):
+    """handle + positions after bench.py's equilibration (bench.py `measure`: gamma = 2 omega / sqrt(P), EQUIL steps)"""
+    sim = make(binding, w, thermostat=binding.THERMOSTAT_LANGEVIN, seed=seed)
+    x, v = wl.make_state(w, seed)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    sim.set_gamma(2.0 * w.omega / np.sqrt(w.P))
+    sim.step(EQUIL)
+    sim.set_gamma(1.0)
+    return sim
+
+
+def evaluate_with_phases(sim):
+    """one more force evaluation at the reached positions with the phase clock on: (x, F, vb, sign, phases, fallbacks in it)"""
+    xs = sim.get_state()[0].cpu().numpy()
+    fb0 = sim.get_diagnostics()["fallbacks"]
+    sim.set_profiling(True)
+    sim.get_chain_phases()
+    F, vb, sg = sim.forces()
+    ph = sim.get_chain_phases()
+    sim.set_profiling(False)
+    return xs, F.cpu().numpy(), vb, sg, ph, sim.get_diagnostics()["fallbacks"] - fb0
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg5_N2500", "cfg5_N10000", "cfg5b"])
+def test_thermalised_state_matches_oracle(binding, oracle, name):
+    w = wl.WORKLOADS[name]
+    sim = thermalised(binding, w)
+    xs, F, vb, sg, ph, fb = evaluate_with_phases(sim)
+    sim.close()
+    assert fb == 0                       # the stale-gauge kernel's own result is what is compared
+    assert ph[11] > 0                    # helper batches met
+    if name.startswith("cfg5_"):
+        # the ideal clouds contract to the trap's ground state: every block takes the factorised exponent arguments and
+        # next to no helper batch is negligible (measured: 79 / 313 factorised blocks = all, 0 of 2106 / 8424 batches skipped)
+        assert ph[6] == (w.N + 31) // 32
+        assert ph[12] <= 0.02 * ph[11]
+    else:
+        # with the pair repulsion the thermalised cloud stays spread out: the direct arguments are used and most batches
+        # are dropped (measured: 0 factorised blocks, 940 of 1323 / 6607 of 8424 batches skipped), like the initial cloud
+        assert ph[12] > 0
+    Fo, vbo, sgo = oracle.forces(xs, w.beta, w.omega, w.g, w.s, w.xi)
+    assert sg == sgo == 1 and abs(vb - vbo) <= RTOL * abs(vbo)
+    check_forces(F, Fo, RTOL)
+
+
+@pytest.mark.parametrize("name", ["cfg5_N20000", "cfg5_N40000"])
+def test_thermalised_largest_sizes_against_streamed_oracle(binding, oracle, name):
+    w = wl.WORKLOADS[name]
+    sim = thermalised(binding, w)
+    xs, F, vb, sg, ph, fb = evaluate_with_phases(sim)
+    sim.close()
+    assert fb == 0 and ph[6] > 0
+    rng = np.random.default_rng(3)
+    sel = np.unique(np.concatenate([[0, 1, 31, 32, 33, w.N - 2, w.N - 1], rng.integers(0, w.N, 41)])).astype(np.int32)
+    Fs, vbo, sgo = oracle.stream_forces_on(xs, w.beta, w.omega, w.g, w.s, w.xi, sel)[:3]
+    assert sg == sgo == 1 and abs(vb - vbo) <= RTOL * abs(vbo)
+    Fg = F[:, sel, :].transpose(1, 0, 2)
+    P = w.P
+    assert np.max(np.abs(Fg - Fs)) <= RTOL * float(np.max(np.abs(Fg)))
+    assert np.max(np.abs(Fg[:, 0] - Fs[:, 0])) <= RTOL * float(np.max(np.abs(Fs[:, 0])))
+    assert np.max(np.abs(Fg[:, P - 1] - Fs[:, P - 1])) <= RTOL * float(np.max(np.abs(Fs[:, P - 1])))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# BASELINE configs[3]: N = 1000 fictitious particles "also run at xi = -0.3 and xi = 0"; the xi = 0 run against the
+# distinguishable-particle result (0^0 = 1, PAPER.md:42: every ring closes on itself; V = sum_l E^{[l,l]} + ln N!/beta)
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("xi", [-0.3, 0.0])
+def test_cfg4_variants_match_oracle(binding, oracle, xi):
+    w = wl.WORKLOADS["cfg4"].with_(xi=xi)
+    x, v = wl.make_state(w, 0)
+    sim = make(binding, w)
+    sim.set_state(torch.from_numpy(x).cuda(), torch.from_numpy(v).cuda())
+    for stage in range(2):               # the seeded cloud (twice: fresh, then stale gauge), then three MD steps on
+        xs = sim.get_state()[0].cpu().numpy()
+        tol = RTOL if xi >= 0 else RTOL * oracle.conditioning(xs, w.beta, xi)
+        Fo, vbo, sgo = oracle.forces(xs, w.beta, w.omega, w.g, w.s, xi)
+        for _ in range(2):
+            F, vb, sg = sim.forces()
+            assert sg == sgo and abs(vb - vbo) <= tol * abs(vbo)
+            check_forces(F.cpu().numpy(), Fo, tol)
+        if xi == 0.0:
+            # distinguishable particles, written out here: closed rings only
+            ks = w.P / w.beta ** 2
+            ring = np.concatenate([xs, xs[:1]], axis=0)
+            from math import lgamma
+            v_closed = 0.5 * ks * float(np.sum(np.diff(ring, axis=0) ** 2)) + lgamma(w.N + 1.0) / w.beta
+            assert sg == 1 and abs(vb - v_closed) <= RTOL * abs(v_closed)
+            f_spring = -ks * (2 * xs - np.roll(xs, 1, axis=0) - np.roll(xs, -1, axis=0))
+            f_trap = -(w.omega ** 2 / w.P) * xs
+            # the pair part does not depend on xi: taken from the oracle's bosonic evaluation, not from its xi = 0 path
+            f_pair = oracle.forces(xs, w.beta, 0.0, w.g, w.s, 1.0)[0] - oracle.forces(xs, w.beta, 0.0, 0.0, w.s, 1.0)[0]
+            assert relerr(F.cpu().numpy(), f_spring + f_trap + f_pair) <= RTOL
+        sim.step(3)
+    diag = sim.get_diagnostics()
+    sim.close()
+    assert diag["status_seen"] == 0
+
