@@ -32,16 +32,36 @@ FLOP_PER_PAIR_EXECUTED = 32.0
 FLOP_PER_ELEMENT = 48.0   # exchange bulk: 24 FP64 instructions per lower-triangle entry and direction (fused row)
 
 
+TRAFFIC_CSV = "r3_traffic.csv"
+TRAFFIC_SOURCE = ("from the committed ncu --set full capture profiles/%s (command and code state in profiles/r3_traffic.md), "
+                  "not measured in this run" % TRAFFIC_CSV)
+
+
 def ncu_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` at `workload`, from the summary of the
-    `ncu --set full` capture of the shipped code state (profiles/r2_traffic.csv: workload,kernel,read,write); None if
+    `ncu --set full` capture of the shipped code state (profiles/r3_traffic.csv: workload,kernel,read,write); None if
     that capture has no such row."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as f:
             for line in f:
                 c = [t.strip() for t in line.split(",")]
                 if len(c) >= 4 and c[0] == workload and c[1] == kernel:
                     return int(float(c[2]) + float(c[3]))
+    except OSError:
+        pass
+    return None
+
+
+def exact_energy(name):
+    """exact canonical energy of the non-interacting workloads at finite P (tests/golden/ideal_gas_energies.txt, written by a
+    committed script from oracle/ideal_gas.py; BASELINE configs[4] "energy versus the exact ideal-Bose value"); None if the
+    workload interacts or is not listed"""
+    try:
+        with open(os.path.join(ROOT, "tests", "golden", "ideal_gas_energies.txt")) as f:
+            for ln in f:
+                c = ln.split()
+                if c and c[0] == name:
+                    return float(c[6])
     except OSError:
         pass
     return None
@@ -232,52 +252,90 @@ def median_rate(torch, sim, steps, flush, w, est_every, world=1):
     return rates[len(rates) // 2], rates
 
 
-def roofline_of(w, kern, iso, fp64_peak):
-    """roofline object of the dominant throughput kernel of workload w from per-kernel times (ms) inside the step
-    (kern) and alone (iso); DESIGN.md section 8"""
+def pair_roofline(w, kern, iso, fp64_peak):
+    """ALU roofline of the pair kernel (None for g = 0) from its time inside the step (kern) and alone (iso), ms"""
     pairs = w.P * w.N * (w.N - 1) / 2.0 if w.g != 0.0 else 0.0
-    if pairs and kern.get("pair"):
-        t, ta = kern["pair"] * 1e-3, iso.get("pair", 0.0) * 1e-3
-        ach = pairs * FLOP_PER_PAIR / t / 1e12
-        return {"bound": "alu", "kernel": "k_pair (pair forces, Newton's third law)", "achieved": ach, "peak": fp64_peak,
-                "unit": "TFLOP/s", "frac": ach / fp64_peak, "traffic": ncu_traffic(w.name, "k_pair"),
-                "frac_algorithmic": ach / fp64_peak,
-                "frac_executed": pairs * FLOP_PER_PAIR_EXECUTED / t / 1e12 / fp64_peak,
-                "traffic_note": "DRAM bytes per launch (ncu); the algorithmic inputs are L2-resident: %d B of positions" % (w.P * w.N * w.d * 8),
-                "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
-                               "1.965 GHz x 2 = 37.2 TFLOP/s)",
-                "convention": "frac = frac_algorithmic: 50 flop (25 FP64 instructions, SURVEY.md 8(d)) per unordered bead pair, %d "
-                              "pairs per launch; frac_executed counts the 16 FP64 instructions (32 flop) per pair the shipped "
-                              "SASS executes and is the figure to hold against north_star's 50 %% (ncu FP64-pipe utilisation: "
-                              "profiles/)" % int(pairs),
-                "timed": "inside the step, sharing the GPU with the recursion kernel on another stream",
-                "alone": {"ms": iso.get("pair"), "frac": (pairs * FLOP_PER_PAIR / ta / 1e12 / fp64_peak) if ta else None,
-                          "frac_executed": (pairs * FLOP_PER_PAIR_EXECUTED / ta / 1e12 / fp64_peak) if ta else None}}
-    # non-interacting workloads: the exchange recursion is all there is.  It recomputes the closing springs instead of
-    # streaming an N x N matrix, so its bulk is ALU work (SURVEY 8(d), row "fused / recomputed": 2 passes x N^2/2 entries x
-    # about 24 FP64 instructions); the kernel itself is bound by the latency of its N-long dependent chain up to N ~ 2e4
+    if not (pairs and kern.get("pair")):
+        return None
+    t, ta = kern["pair"] * 1e-3, iso.get("pair", 0.0) * 1e-3
+    ach = pairs * FLOP_PER_PAIR_EXECUTED / t / 1e12
+    return {"bound": "alu", "kernel": "k_pair2 / k_pair (pair forces, Newton's third law)", "ms_in_step": kern["pair"],
+            "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,
+            "frac_executed": ach / fp64_peak,
+            "frac_algorithmic": pairs * FLOP_PER_PAIR / t / 1e12 / fp64_peak,
+            "traffic": ncu_traffic(w.name, "k_pair"), "traffic_source": TRAFFIC_SOURCE,
+            "traffic_note": "DRAM bytes per launch (ncu); the algorithmic inputs are L2-resident: %d B of positions" % (w.P * w.N * w.d * 8),
+            "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak (nominal 148 SM x 64 FMA/clk x "
+                           "1.965 GHz x 2 = 37.2 TFLOP/s)",
+            "convention": "frac = frac_executed: the 16 FP64 instructions (32 flop) per unordered bead pair the shipped SASS executes, "
+                          "%d pairs per launch -- the figure to hold against north_star's 50 %%; frac_algorithmic counts SURVEY.md "
+                          "8(d)'s 25 instructions (50 flop) per pair and over-counts the exponential (it can read above 1)" % int(pairs),
+            "timed": "inside the step, sharing the GPU with the recursion kernel on another stream (event pairs only, no "
+                     "instrumentation)",
+            "alone": {"ms": iso.get("pair"), "frac": (pairs * FLOP_PER_PAIR_EXECUTED / ta / 1e12 / fp64_peak) if ta else None,
+                      "frac_executed": (pairs * FLOP_PER_PAIR_EXECUTED / ta / 1e12 / fp64_peak) if ta else None,
+                      "frac_algorithmic": (pairs * FLOP_PER_PAIR / ta / 1e12 / fp64_peak) if ta else None}}
+
+
+def chain_roofline(w, kern, iso, fp64_peak, recursion):
+    """The recursion kernel.  It recomputes the closing springs instead of streaming an N x N matrix, so its bulk is ALU
+    work (SURVEY 8(d), row "fused / recomputed": 2 passes x N^2/2 entries x about 24 FP64 instructions), but up to
+    N ~ 2e4 the kernel is bound by the latency of its N-long dependent chain: the ALU fraction is reported beside the
+    latency figures (ns per row, cycles per 32-row block against the 32 x 38 cycle floor)."""
     ch_ms = kern.get("chain")
+    if not ch_ms:
+        return None
     elems = float(w.N) * (w.N + 1)  # both directions over the lower triangle
-    ach = elems * FLOP_PER_ELEMENT / (ch_ms * 1e-3) / 1e12 if ch_ms else None
+    ach = elems * FLOP_PER_ELEMENT / (ch_ms * 1e-3) / 1e12
     cha = iso.get("chain")
-    return {"bound": "alu", "kernel": "k_chain_spec (forward + backward recursion, panel workers with the force sums)", "achieved": ach,
-            "peak": fp64_peak, "unit": "TFLOP/s", "frac": (ach / fp64_peak if ach else None), "traffic": ncu_traffic(w.name, "k_chain_spec"),
+    cyc = (recursion or {}).get("cycles_per_block") or {}
+    return {"bound": "latency", "kernel": "k_chain_spec (forward + backward recursion, panel workers with the force sums, force band "
+                                          "and exterior forces as its tail)",
+            "ms_in_step": ch_ms, "achieved": ach, "peak": fp64_peak, "unit": "TFLOP/s", "frac": ach / fp64_peak,
+            "ns_per_row": ch_ms * 1e6 / w.N, "cycles_per_block": cyc.get("sum"), "floor_cycles_per_block": 32 * 38,
+            "traffic": ncu_traffic(w.name, "k_chain_spec"), "traffic_source": TRAFFIC_SOURCE,
             "peak_source": "FP64 FMA issue rate measured live by pimd_probe_fp64_peak",
-            "convention": "48 flop (24 FP64 instructions, SURVEY.md 8(d) fused row) per lower-triangle entry and direction, N(N+1) "
-                          "entries per launch; the kernel is latency bound (one dependent DFMA + SHFL per row, see `recursion`) "
-                          "until the workers' bulk takes over near N = 4e4",
+            "convention": "achieved / frac: 48 flop (24 FP64 instructions, SURVEY.md 8(d) fused row) per lower-triangle entry and "
+                          "direction, N(N+1) entries per launch, over the kernel's time inside the step; neither roofline binds the "
+                          "kernel below N ~ 2e4 -- one dependent DFMA + SHFL per row (ns_per_row; cycles_per_block from the phase "
+                          "clock of a separate instrumented run, floor 32 x 38) -- the workers' bulk takes over near N = 4e4",
             "alone": {"ms": cha, "frac": (elems * FLOP_PER_ELEMENT / (cha * 1e-3) / 1e12 / fp64_peak) if cha else None}}
 
 
-def kernel_profile(sim, nsteps, w):
-    """per-kernel device time (ms per launch) and the chain's phase clock over nsteps steps"""
-    sim.set_profiling(True)
+def rooflines_of(w, kern, iso, fp64_peak, recursion=None):
+    """(roofline of the kernel that sets the step, [every hot kernel's roofline]): the dominant one is the kernel with the
+    larger duration inside the step (the two run concurrently on two streams)"""
+    rows = [r for r in (chain_roofline(w, kern, iso, fp64_peak, recursion), pair_roofline(w, kern, iso, fp64_peak)) if r]
+    if not rows:
+        return None, []
+    top = max(rows, key=lambda r: r["ms_in_step"])
+    for r in rows:
+        r["dominant"] = r is top
+    return top, rows
+
+
+def kernel_profile(sim, nsteps, w, phases=True):
+    """per-kernel device time (ms per launch) over nsteps steps with event pairs only (the kernels run uninstrumented), and
+    -- from a second run of nsteps steps with the clock64 instrumentation armed -- the chain's phase clock and the
+    instrumented chain time (an upper bound, reported separately)"""
+    sim.set_profiling(True, phases=False)
     sim.get_profile()
-    sim.get_chain_phases()
     sim.run(nsteps, est_every=EST_EVERY, nbins=w.nbins, rmax=w.rmax)
     prof = sim.get_profile()
+    ph, chain_instr = [0] * 16, None
+    if phases:
+        sim.set_profiling(True, phases=True)
+        sim.get_chain_phases()
+        sim.run(nsteps, est_every=EST_EVERY, nbins=w.nbins, rmax=w.rmax)
+        p2 = sim.get_profile()
+        ph = sim.get_chain_phases()
+        if p2.get("chain", (0, 0))[1]:
+            chain_instr = p2["chain"][0] / p2["chain"][1]
     sim.set_profiling(False)
-    return {k: ms / n for k, (ms, n) in prof.items() if n}, {k: n for k, (ms, n) in prof.items() if n}, sim.get_chain_phases()
+    kern = {k: ms / n for k, (ms, n) in prof.items() if n}
+    if chain_instr is not None:
+        kern["chain_with_phase_clock"] = chain_instr
+    return kern, {k: n for k, (ms, n) in prof.items() if n}, ph
 
 
 def e2e_rate(torch, sim, x0, v0, ne2e, world, barrier):
@@ -381,7 +439,10 @@ def run_ours(args, w):
         torch.cuda.synchronize()
         out["steps_per_s_l2_resident"] = world * steps / (a.elapsed_time(b) * 1e-3)
         nsamp, sp, sv, _, _ = sim.read_accumulators()
-        out["sampled"] = {"n": float(nsamp), "e_prim_mean": float(sp / max(nsamp, 1.0)), "e_vir_mean": float(sv / max(nsamp, 1.0))}
+        out["sampled"] = {"n": float(nsamp), "e_prim_mean": float(sp / max(nsamp, 1.0)), "e_vir_mean": float(sv / max(nsamp, 1.0)),
+                          "energy_exact": exact_energy(wk.name),
+                          "note": "means over the few estimator samples of the timed steps (no error bar: tests/test_gpu_timed_path.py "
+                                  "holds the ensemble check against energy_exact)"}
         kern, counts, phases = kernel_profile(sim, max(5, min(steps, 20)), wk)
         out["kernels_ms"] = kern
         out["recursion"] = recursion_report(wk, {"chain": {"ms_avg": kern.get("chain")}}, phases, max(5, min(steps, 20)), None)
@@ -393,7 +454,7 @@ def run_ours(args, w):
         if full:
             # the same kernels timed alone (exchange and bead parts serialised on one stream): the burst figure
             sim.set_concurrency(False)
-            iso, _, _ = kernel_profile(sim, max(5, min(steps, 20)), wk)
+            iso, _, _ = kernel_profile(sim, max(5, min(steps, 20)), wk, phases=False)
             sim.set_concurrency(True)
             out["kernels_alone_ms"] = iso
             out["e2e_value"], out["e2e_bytes"] = e2e_rate(torch, sim, x0, v0, max(3, min(steps, 50)), world, barrier)
@@ -434,7 +495,8 @@ def run_ours(args, w):
         "kernels_ms": m["kernels_ms"],
         "kernels_alone_ms": m["kernels_alone_ms"],
         "recursion": m["recursion"],
-        "roofline": roofline_of(w, m["kernels_ms"], m["kernels_alone_ms"], fp64_peak),
+        "roofline": rooflines_of(w, m["kernels_ms"], m["kernels_alone_ms"], fp64_peak, m["recursion"])[0],
+        "rooflines": rooflines_of(w, m["kernels_ms"], m["kernels_alone_ms"], fp64_peak, m["recursion"])[1],
         "peaks": {"fp64_tflops_probe": fp64_peak, "hbm_gbs": peaks.get("hbm_gbs"), "source": peak_src},
     }
 
@@ -448,13 +510,21 @@ def run_ours(args, w):
             row = {"workload": describe(wk), "value": r["value"], "unit": UNIT, "value_initial_cloud": r["value_initial_cloud"],
                    "pair_forces_per_s": pp * r["value"], "steps_per_s_l2_resident": r["steps_per_s_l2_resident"],
                    "kernels_ms": r["kernels_ms"], "kernels_alone_ms": r["kernels_alone_ms"], "recursion": r["recursion"],
-                   "roofline": roofline_of(wk, r["kernels_ms"], r["kernels_alone_ms"], fp64_peak),
+                   "roofline": rooflines_of(wk, r["kernels_ms"], r["kernels_alone_ms"], fp64_peak, r["recursion"])[0],
+                   "rooflines": rooflines_of(wk, r["kernels_ms"], r["kernels_alone_ms"], fp64_peak, r["recursion"])[1],
                    "e2e": {"value": r["e2e_value"], "unit": UNIT, "h2d_bytes_per_step": r["e2e_bytes"], "d2h_bytes_per_step": r["e2e_bytes"]},
                    "fallbacks_in_timed_steps": r["fallbacks_in_timed_steps"]}
             if not args.no_cpu:
                 row["cpu_baseline"] = cpu_baseline(wk, 1.0)
             also.append(row)
         line["also"] = also
+        for row in also:   # north_star: >= 50 % of the FP64 roofline on the pair kernel at N = 10000 -- in the step AND alone
+            pr = [r for r in row["rooflines"] if r["kernel"].startswith("k_pair")]
+            if pr and "cfg5b" in row["workload"]:
+                line["pair_kernel_N10000"] = {"workload": "cfg5b", "frac_executed_in_step": pr[0]["frac_executed"],
+                                              "frac_executed_alone": pr[0]["alone"]["frac_executed"],
+                                              "ms_in_step": pr[0]["ms_in_step"], "ms_alone": pr[0]["alone"]["ms"],
+                                              "peak_tflops": fp64_peak, "target": 0.5}
     if world == 1 and not args.no_sweep:
         sweep = []
         for name in args.sweep.split(","):
@@ -466,6 +536,7 @@ def run_ours(args, w):
                           "pair_forces_per_s": pp * r["value"], "kernels_ms": r["kernels_ms"],
                           "ns_per_row": r["recursion"].get("ns_per_row"),
                           "helper_batches_skipped_frac": r["recursion"].get("helper_batches_skipped_frac"),
+                          "sampled": r["sampled"],
                           "fallbacks_in_timed_steps": r["fallbacks_in_timed_steps"]})
         line["sweep"] = sweep
         line["sweep_protocol"] = "as the headline: thermalised by %d steps, L2 flushed between steps, median of %d x %d steps" % (
@@ -516,7 +587,13 @@ def run_ours(args, w):
         for key, name in (("emat", "k_emat (cycle energies, Eq. 7-10)"), ("prmat", "k_prmat (connection probabilities, Eq. 12-14)")):
             ms = pr3[key][0] / max(pr3[key][1], 1)
             gbs = nbytes_nn / (ms * 1e-3) / 1e9
-            line["nxn_passes"][key] = {"kernel": name, "ms": ms, "achieved": gbs, "frac": gbs / peaks.get("hbm_gbs")}
+            dram = ncu_traffic("cfg5_N10000", "k_" + key)
+            line["nxn_passes"][key] = {"kernel": name, "ms": ms, "achieved": gbs, "frac": gbs / peaks.get("hbm_gbs"),
+                                       "convention": "achieved = 8 N^2 bytes written / kernel time; by_dram_bytes = the DRAM bytes ncu "
+                                                     "saw inside one launch (part of the output is still in L2 when it ends) / the same time",
+                                       "by_dram_bytes": ({"traffic": dram, "achieved": dram / (ms * 1e-3) / 1e9,
+                                                          "frac": dram / (ms * 1e-3) / 1e9 / peaks.get("hbm_gbs"),
+                                                          "traffic_source": TRAFFIC_SOURCE} if dram else None)}
         del buf
         s3.close()
     if world == 1 and not args.no_cpu:

@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(TB *PREP_SPLIT) k_prep(const double *__restric
         // change since the evaluation before is added once more.  A cloud that contracts or expands moves g by tens of
         // units per step, smoothly in time: the first-order prediction keeps the new solution within e^{O(1)} of the
         // gauge (measured: N = 40000 while the initial cloud falls into the trap, 48 rejected gauges in 120 steps -> see
-        // profiles/r2_notes.md).  Only a gauge: any value is correct, a bad one is caught by the acceptance band.
+        // profiles/r2_measurements.md).  Only a gauge: any value is correct, a bad one is caught by the acceptance band.
 #pragma unroll
         for (int dir = 0; dir < 2; ++dir) {
             const double z = p.gs[dir][l + 1];
@@ -965,7 +965,7 @@ __device__ void chain_cta_spec(const ChainArgs &a, int dir, size_t roff, unsigne
     // thermalised cloud: kk R^2 ~ 10^1..10^2); otherwise -- the spread-out initial clouds of the BASELINE configurations,
     // kk R^2 ~ 10^4 -- the window's tables hold the plain pieces and the entries are formed the direct way,
     //     ((t_p - G_r) + dl_p) - kk |rho'_r - sigma'_p|^2,   t_p, G_r float-valued so that their difference is exact,
-    // 3 + 2 D instructions with the accuracy of the max-plus kernel (measured: forces 1.4e-9 -> see profiles/r2_notes.md).
+    // 3 + 2 D instructions with the accuracy of the max-plus kernel (measured: forces 1.4e-9 -> see profiles/r2_measurements.md).
     auto col_row_terms = [&](int K) {
         constexpr int W = 2 + 2 * D, CW = SPEC_CW(D);
         double *cA = ctab_s + (K & 1) * (4 * 32 * CW), *rA = rtab_s + (K & 1) * (2 * 32 * W);
@@ -1824,7 +1824,7 @@ __device__ void assemble_task(int N, double ks, double xi, const ExchPtrs &p, do
 // Tail of the recursion kernels: once both directions are done (grid barrier), the CTAs of a replica share out the
 // force-band tasks (one per row block and direction), meet at a second grid barrier and assemble the exterior forces.
 // Two launches less on the critical path of a step (k_forcepass, k_assemble used to be kernels of their own:
-// profiles/r2_notes.md).  Groups of 128 threads with their own named barriers (ids 1..4) and staging areas.
+// profiles/r2_measurements.md).  Groups of 128 threads with their own named barriers (ids 1..4) and staging areas.
 // ==========================================================================================
 template <int D, bool SGN>
 __device__ void exchange_tail(const ChainArgs &a, size_t roff, unsigned char *smem_raw, const double *etab64,
@@ -2401,7 +2401,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(const double *__restri
 // and meets, at step k, column (t + k) mod 32 of both tiles of the partner super-tile: four potential evaluations per
 // step (four independent exponential chains), every column position loaded once for two rows and every travelling
 // column accumulator shuffled once for two contributions -- per pair half the LDS and SHFL traffic of k_pair, which was
-// bound by the issue port (40 warp instructions per pair, 16 of them FP64; profiles/r1_notes.md).
+// bound by the issue port (40 warp instructions per pair, 16 of them FP64; profiles/r1_measurements.md).
 // The diagonal task of a super-tile does its two 32 x 32 diagonal tiles the plain way and the cross tile with
 // Newton's third law.  grid (ceil(tasks/PAIR_WARPS), P, B), tasks = NS (nchunk + 1), NS = ceil(NT / 2).
 // ==========================================================================================
